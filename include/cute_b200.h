@@ -1,0 +1,201 @@
+/*
+ * cute_b200.h -- C ABI of the B200-native pair-counting hot path of CUTE (arXiv 1210.1833).
+ *
+ * Problem statement (sec. III.A): "DD, DR and RR are computed by autocorrelating
+ * or crosscorrelating each pair of catalogs ... calculating the distance between each pair of
+ * objects, determining the bin corresponding to that distance and increasing the histogram count
+ * on that bin", i.e. Eq. 11; with neighbour searching by cubical cells or pixels
+ * (sec. III.C) and the estimators of Eqs. 13-15 on the host.
+ *
+ * Conventions (readings of the paper are listed in DESIGN.md):
+ *  - Every function returns an int status: 0 = CUTE_OK, < 0 error, > 0 warning.  No exceptions,
+ *    no abort, no stdout.  cute_strerror() gives a static string.
+ *  - "device" pointers are CUDA device pointers owned by the caller (PyTorch tensors in this
+ *    repository); the library never allocates or frees device memory.  "host" pointers are plain
+ *    host memory.  Streams are passed as void* (a cudaStream_t; NULL = legacy default stream).
+ *  - Auto-correlation (second grid NULL or equal to the first) counts UNORDERED pairs i<j;
+ *    cross-correlation counts all N1*N2 pairs (forced by Eq. 15).
+ *  - Bin k holds pairs with e_k <= v < e_{k+1}; out-of-range pairs are dropped.  2-D histograms
+ *    are stored first-variable-major: index = k1 * n2 + k2.
+ *  - Histograms are uint64 ("long integers").
+ *  - The GPU histogram equals the float64 definition exactly except for pairs whose binned variable
+ *    lies at float64-rounding distance of a bin edge.
+ */
+#ifndef CUTE_B200_H
+#define CUTE_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CUTE_ABI_VERSION 1
+
+/* status codes */
+#define CUTE_OK 0
+#define CUTE_ERR_INVALID_ARG (-1)
+#define CUTE_ERR_UNSUPPORTED (-2)
+#define CUTE_ERR_WORKSPACE_TOO_SMALL (-3)
+#define CUTE_ERR_CUDA (-4)
+#define CUTE_ERR_OVERFLOW (-5)
+#define CUTE_ERR_POINT_OUT_OF_BOX (-6)
+#define CUTE_ERR_GRID_MISMATCH (-7)
+#define CUTE_WARN_EMPTY_BIN 1
+
+/* kinds of correlation function ("CUTE calculates 4 different correlation functions (3-D,
+ * monopole, angular and radial)") */
+#define CUTE_ANGULAR 0  /* w(theta): v = theta [rad]                     */
+#define CUTE_MONOPOLE 1 /* xi_0(r): v = r; periodic box: PAPER.md:245-249       */
+#define CUTE_RMU 2      /* xi(r,mu): v = (r, mu), mid-point line of sight */
+#define CUTE_RADIAL 3   /* xi_r(zbar,dz): pairs with theta < aperture, v = (zbar, dz) */
+
+/* catalogue coordinates */
+#define CUTE_COORD_XYZ 0     /* c0,c1,c2 = x,y,z (Mpc/h)              -> MONOPOLE, RMU */
+#define CUTE_COORD_RADEC 1   /* c0,c1 = RA,Dec in degrees; c2 ignored -> ANGULAR       */
+#define CUTE_COORD_RADECZ 2  /* c0,c1 = RA,Dec in degrees; c2 = z     -> RADIAL (and ANGULAR) */
+#define CUTE_F32 0
+#define CUTE_F64 1
+
+/* neighbour-search modes */
+#define CUTE_GRID_NONE 0   /* no cells: brute force, every pair is evaluated       */
+#define CUTE_GRID_BOX3D 1  /* cubical cells                                        */
+#define CUTE_GRID_SPHERE 2 /* pixels with constant limits in (sin dec, RA)     */
+
+/* A catalogue in structure-of-arrays form (as in the paper's listing).
+ * Pointers are DEVICE pointers for cute_make_grid and HOST pointers for cute_count_pairs_host.
+ * z -> comoving distance is the caller's job (float64 on the host). */
+typedef struct cute_catalog {
+    size_t struct_size; /* = sizeof(cute_catalog) */
+    int64_t n;          /* number of objects, >= 0 */
+    int coord;          /* CUTE_COORD_*            */
+    int dtype;          /* CUTE_F32 | CUTE_F64     */
+    const void *c0, *c1, *c2;
+} cute_catalog;
+
+/* How to build the cell list.
+ *  BOX3D : origin[3], size[3] in Mpc/h (size[d] <= 0: bounding box of the catalogue, computed on the
+ *          device; for a cross-correlation pass the same explicit box to both grids), ncell[3]
+ *          (ncell[d] <= 0: chosen by the library from rmax), periodic != 0 => origin must be 0 and
+ *          size[0]=size[1]=size[2]=L.
+ *  SPHERE: axis 0 = RA: origin[0] = RA0 [deg], size[0] = span [deg] (< 360: RA is taken modulo 360
+ *          relative to RA0, so a footprint straddling RA=0 is fine); axis 1 = sin(Dec): origin[1],
+ *          size[1] (dimensionless, within [-1,1]); ncell[0], ncell[1]; axis 2 unused.
+ *  rmax  : largest separation that will be asked for with this grid: r [Mpc/h] for BOX3D,
+ *          theta [rad] for SPHERE (the radial aperture or the last theta edge).
+ *  Two grids used together in a cross-correlation must carry identical specs. */
+typedef struct cute_grid_spec {
+    size_t struct_size;
+    int mode;      /* CUTE_GRID_* */
+    int periodic;  /* BOX3D only  */
+    double origin[3];
+    double size[3];
+    int ncell[3];
+    double rmax;
+} cute_grid_spec;
+
+/* Binning.  Variable 1: theta [rad] (ANGULAR), r (MONOPOLE, RMU), zbar (RADIAL); linear or, if
+ * log1 != 0, logarithmic: e_k = lo1 (hi1/lo1)^(k/n1) ("logarithmic binning").
+ * Variable 2 (n2 = 0 for 1-D kinds): mu in [lo2,hi2] (RMU; mu = 1 belongs to the last bin when
+ * hi2 >= 1), dz (RADIAL); always linear.  aperture_rad: RADIAL only, strict theta < aperture.
+ * box_L > 0: periodic box of side L, minimum-image separations (MONOPOLE only; needs hi1 <= L/2). */
+typedef struct cute_bin_spec {
+    size_t struct_size;
+    int n1; double lo1, hi1; int log1;
+    int n2; double lo2, hi2;
+    double aperture_rad;
+    double box_L;
+} cute_bin_spec;
+
+/* Optional launch controls (NULL = defaults).  All fields 0 = default. */
+typedef struct cute_count_opts {
+    size_t struct_size;
+    int blocks;            /* persistent CTAs to launch (default: 2 per SM)                          */
+    int64_t item_begin;    /* shard of the work-item list [item_begin, item_end) handled by this call */
+    int64_t item_end;      /* (0,0 = all). Items partition the pairs, so shards add up exactly       */
+    double tau_scale;      /* multiplies the refine half-width (>1 refines more pairs; results must   */
+                           /* not change).  0 = 1.0                                                   */
+    int force_refine;      /* != 0: every in-range pair is recomputed in float64                      */
+    int flush_items;       /* flush the shared-memory histogram every this many work items (testing   */
+                           /* the uint32 epoch logic); 0 = only when the epoch bound requires it      */
+} cute_count_opts;
+
+/* Facts about a built grid (for tests and reports). */
+typedef struct cute_grid_info {
+    size_t struct_size;
+    int64_t n;
+    int mode, periodic, kind_coord, dtype, has_lo, has_f64;
+    int ncell[3];
+    double origin[3], cell[3];
+    int64_t ncells, nrows, nchunks;
+    const void *d_hi;         /* float4[n]   cell-sorted (x,y,z,w)                */
+    const void *d_lo;         /* float4[n]   low parts (or NULL)                  */
+    const void *d_perm;       /* uint32[n]   sorted slot -> original index        */
+    const void *d_cell_start; /* uint32[ncells+1]                                 */
+    double build_bytes;       /* algorithmic HBM bytes of the build   */
+} cute_grid_info;
+
+typedef struct cute_grid cute_grid; /* opaque host handle; holds pointers INTO the caller's workspace */
+
+int cute_version(void);
+const char *cute_strerror(int status);
+
+/* Size of the device workspace cute_make_grid needs for this catalogue and spec (256-byte granular). */
+int cute_grid_workspace_bytes(const cute_catalog *cat, const cute_grid_spec *spec, size_t *bytes);
+
+/* Cell-list build ("To each cell we associate the positions of all the objects that
+ * fall inside it"): canonicalise (unit vectors, hi/lo split), cell index + cell histogram, exclusive
+ * scan, scatter into cell-sorted float4 arrays, chunk table.  Runs on `stream`; synchronises the
+ * stream once to read back the error word and the chunk count.  cat pointers are DEVICE pointers and
+ * are not referenced after the call returns.  *out must be released with cute_free_grid, which
+ * never frees device memory.  mode NONE gives a single-cell grid (brute force). */
+int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_workspace, size_t bytes,
+                   void *stream, cute_grid **out);
+void cute_free_grid(cute_grid *g);
+int cute_grid_get_info(const cute_grid *g, cute_grid_info *info);
+
+/* Scratch the pair counter needs (work queue, per-CTA uint64 partial histograms, status word). */
+int cute_count_scratch_bytes(const cute_bin_spec *bins, const cute_count_opts *opts, size_t *bytes);
+
+/* The pair count (CUDA prior art PAPER.md:159-192).  d_hist: DEVICE uint64[n1*max(n2,1)],
+ * overwritten.  g2 == NULL or g2 == g1: auto-correlation.  Enqueued on `stream`; returns after
+ * enqueue.  Deferred device errors are read with cute_count_status. */
+int cute_count_pairs(int kind, const cute_grid *g1, const cute_grid *g2, const cute_bin_spec *bins,
+                     uint64_t *d_hist, void *d_scratch, size_t scratch_bytes,
+                     const cute_count_opts *opts, void *stream);
+
+/* Synchronises `stream` and returns the deferred status of the last cute_count_pairs that used
+ * d_scratch.  stats (host, may be NULL): [0] separations evaluated, [1] pairs recomputed in float64,
+ * [2] work items, [3] shared-memory histogram flushes. */
+int cute_count_status(void *d_scratch, void *stream, uint64_t stats[4]);
+
+/* Duration in ms of the last pair kernel + reduction enqueued with this scratch (CUDA events recorded
+ * on the launch stream by cute_count_pairs; valid after cute_count_status). */
+int cute_count_last_ms(void *d_scratch, float *ms_pair, float *ms_reduce);
+
+/* End-to-end entry point with HOST buffers: copies the catalogue(s) to the device, builds the
+ * grid(s), counts, copies the histogram back.  cat2 == NULL: auto.  d_workspace: DEVICE, at least
+ * cute_host_workspace_bytes().  Synchronous. */
+int cute_host_workspace_bytes(const cute_catalog *cat1, const cute_catalog *cat2, const cute_grid_spec *spec,
+                              const cute_bin_spec *bins, size_t *bytes);
+int cute_count_pairs_host(int kind, const cute_catalog *cat1, const cute_catalog *cat2, const cute_grid_spec *spec,
+                          const cute_bin_spec *bins, uint64_t *h_hist, void *d_workspace, size_t bytes, void *stream);
+
+/* ---- host-side helpers (all pointers HOST) ---- */
+/* Bin edges, the single definition: n+1 doubles for axis 0 or 1. */
+int cute_bin_edges(const cute_bin_spec *bins, int axis, double *edges_out);
+/* Landy-Szalay estimator, Eq. 15. Bins with RR = 0 get xi = 0 and CUTE_WARN_EMPTY_BIN. */
+int cute_landy_szalay(const uint64_t *dd, const uint64_t *dr, const uint64_t *rr, uint64_t nd, uint64_t nr,
+                      int nbins, double *xi);
+/* Natural estimator, Eq. 14. */
+int cute_natural_estimator(const uint64_t *dd, const uint64_t *rr, uint64_t nd, uint64_t nr, int nbins, double *xi);
+/* Expected unordered pairs of a uniform periodic box, N(N-1)/2 * (4pi/3)(e_{k+1}^3-e_k^3)/L^3
+ * (Eqs. 12-13, exact shell volume), and xi = DD/RR - 1. */
+int cute_periodic_rr(uint64_t n, double L, const cute_bin_spec *bins, double *rr);
+int cute_periodic_xi(const uint64_t *dd, uint64_t n, double L, const cute_bin_spec *bins, double *xi);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CUTE_B200_H */

@@ -1,0 +1,163 @@
+"""ctypes front end of the ORACLE (oracle/cute_oracle.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this.  It neither imports nor is imported
+by the CUDA path (paper_1210_1833_b200).  See the C file's header for what is computed and
+the paper passages it follows.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "cute_oracle.c")
+_LIB = os.path.join(_HERE, "libcute_oracle.so")
+
+KINDS = {"angular": 0, "monopole": 1, "rmu": 2, "radial": 3}
+
+# float64, no FMA contraction, no fast-math: the arithmetic is the definition's
+CFLAGS = ["-O2", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC", "-std=c11"]
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", *CFLAGS, "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+class _Bins(C.Structure):
+    _fields_ = [("n1", C.c_int), ("lo1", C.c_double), ("hi1", C.c_double), ("log1", C.c_int),
+                ("n2", C.c_int), ("lo2", C.c_double), ("hi2", C.c_double),
+                ("aperture", C.c_double), ("box_L", C.c_double)]
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        dp = C.POINTER(C.c_double)
+        up = C.POINTER(C.c_uint64)
+        _lib.orc_count.argtypes = [C.c_int, C.c_int, C.c_int64, dp, dp, dp, C.c_int64, dp, dp, dp,
+                                   C.POINTER(_Bins), C.c_int64, C.c_int64, C.c_int, up, up, up, up, up]
+        _lib.orc_edges.argtypes = [C.POINTER(_Bins), C.c_int, dp]
+        _lib.orc_landy_szalay.argtypes = [up, up, up, C.c_uint64, C.c_uint64, C.c_int, dp]
+        _lib.orc_natural.argtypes = [up, up, C.c_uint64, C.c_uint64, C.c_int, dp]
+        _lib.orc_periodic_rr.argtypes = [C.c_uint64, C.c_double, C.POINTER(_Bins), dp]
+    return _lib
+
+
+def _bins(b: dict) -> _Bins:
+    return _Bins(int(b["n1"]), float(b["lo1"]), float(b["hi1"]), int(b.get("log1", 0)),
+                 int(b.get("n2", 0)), float(b.get("lo2", 0.0)), float(b.get("hi2", 0.0)),
+                 float(b.get("aperture", 0.0)), float(b.get("box_L", 0.0)))
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _up(a):
+    return a.ctypes.data_as(C.POINTER(C.c_uint64))
+
+
+def _cols(cat, kind):
+    need = 2 if kind == "angular" else 3
+    cols = [np.ascontiguousarray(np.asarray(c, dtype=np.float64)) for c in cat[:need]]
+    while len(cols) < 3:
+        cols.append(cols[0])
+    return cols
+
+
+def max_threads() -> int:
+    return int(_load().orc_max_threads())
+
+
+def edges(bins: dict, axis: int = 0) -> np.ndarray:
+    b = _bins(bins)
+    n = b.n1 if axis == 0 else b.n2
+    e = np.zeros(n + 1)
+    rc = _load().orc_edges(C.byref(b), axis, _dp(e))
+    if rc:
+        raise ValueError(f"orc_edges failed ({rc})")
+    return e
+
+
+def count(kind: str, cat1, cat2, bins: dict, mode: str = "plain", i_range=None, nthreads: int = 0):
+    """Histogram of the pairs of cat1 x cat2 (cat2 None: unordered pairs of cat1).
+
+    Returns dict(hist, amb_cell, amb_e1, amb_e2, npairs); hist has n1*max(n2,1) uint64 entries
+    (first variable major); amb_cell has one extra trailing entry for the out-of-range cell.
+    """
+    lib = _load()
+    b = _bins(bins)
+    c1 = _cols(cat1, kind)
+    n1 = c1[0].size
+    if cat2 is None:
+        c2, n2 = None, 0
+    else:
+        c2 = _cols(cat2, kind)
+        n2 = c2[0].size
+    ncell = b.n1 * max(b.n2, 1)
+    hist = np.zeros(ncell, dtype=np.uint64)
+    amb_cell = np.zeros(ncell + 1, dtype=np.uint64)
+    amb_e1 = np.zeros(b.n1 + 1, dtype=np.uint64)
+    amb_e2 = np.zeros(b.n2 + 2, dtype=np.uint64)
+    npairs = np.zeros(1, dtype=np.uint64)
+    i0, i1 = (0, n1) if i_range is None else i_range
+    null = C.POINTER(C.c_double)()
+    rc = lib.orc_count(KINDS[kind], {"plain": 0, "celled": 1}[mode],
+                       n1, _dp(c1[0]), _dp(c1[1]), _dp(c1[2]),
+                       n2, _dp(c2[0]) if c2 else null, _dp(c2[1]) if c2 else null, _dp(c2[2]) if c2 else null,
+                       C.byref(b), int(i0), int(i1), int(nthreads),
+                       _up(hist), _up(amb_cell), _up(amb_e1), _up(amb_e2), _up(npairs))
+    if rc:
+        raise ValueError(f"orc_count failed ({rc})")
+    return dict(hist=hist, amb_cell=amb_cell, amb_e1=amb_e1, amb_e2=amb_e2, npairs=int(npairs[0]))
+
+
+def landy_szalay(dd, dr, rr, nd: int, nr: int):
+    dd, dr, rr = (np.ascontiguousarray(np.asarray(a, dtype=np.uint64)).ravel() for a in (dd, dr, rr))
+    xi = np.zeros(dd.size)
+    empty = _load().orc_landy_szalay(_up(dd), _up(dr), _up(rr), int(nd), int(nr), dd.size, _dp(xi))
+    return xi, int(empty)
+
+
+def natural(dd, rr, nd: int, nr: int):
+    dd, rr = (np.ascontiguousarray(np.asarray(a, dtype=np.uint64)).ravel() for a in (dd, rr))
+    xi = np.zeros(dd.size)
+    empty = _load().orc_natural(_up(dd), _up(rr), int(nd), int(nr), dd.size, _dp(xi))
+    return xi, int(empty)
+
+
+def periodic_rr(n: int, L: float, bins: dict) -> np.ndarray:
+    b = _bins(bins)
+    rr = np.zeros(b.n1)
+    rc = _load().orc_periodic_rr(int(n), float(L), C.byref(b), _dp(rr))
+    if rc:
+        raise ValueError(f"orc_periodic_rr failed ({rc})")
+    return rr
+
+
+def parity_ok(gpu_hist, orc: dict):
+    """The north star's parity rule: exact per cell and in total, except for flagged pairs.
+    Returns (ok, message)."""
+    g = np.asarray(gpu_hist).astype(np.int64).ravel()
+    h = orc["hist"].astype(np.int64)
+    amb = orc["amb_cell"].astype(np.int64)
+    if g.size != h.size:
+        return False, f"size {g.size} != {h.size}"
+    d = np.abs(g - h)
+    bad = np.nonzero(d > amb[:-1])[0]
+    if bad.size:
+        k = int(bad[0])
+        return False, f"cell {k}: gpu {g[k]} oracle {h[k]} amb {amb[k]} ({bad.size} cells differ)"
+    if abs(int(g.sum()) - int(h.sum())) > int(amb[-1]):
+        return False, f"total: gpu {g.sum()} oracle {h.sum()} amb_out {amb[-1]}"
+    return True, f"ok (sum {h.sum()}, cells differing within flags: {int((d > 0).sum())})"

@@ -1,0 +1,330 @@
+"""Pins of the oracle: closed forms, exact enumerations, invariants.
+
+None of these re-types the oracle's formula or calls it twice: each compares it with something
+the paper or the mathematics fixes independently.  CPU only.
+"""
+import itertools
+import math
+
+import numpy as np
+import pytest
+
+from conftest import load_golden
+from paper_1210_1833_b200 import synth
+
+GOLDEN = ["monopole_345.txt", "monopole_periodic.txt", "monopole_cross.txt", "angular_equator.txt",
+          "angular_log.txt", "rmu_345.txt", "rmu_los.txt", "radial_ladder.txt"]
+
+
+def _cat(pts):
+    a = np.array(pts, dtype=np.float64).T
+    return tuple(a) if a.shape[0] == 3 else (a[0], a[1], np.zeros_like(a[0]))
+
+
+# ---------------------------------------------------------------- V3 hand-enumerated catalogues
+@pytest.mark.parametrize("name", GOLDEN)
+@pytest.mark.parametrize("mode", ["plain", "celled"])
+def test_golden_hand_enumerated(oracle, name, mode):
+    kind, bins, pts, pts2, expect = load_golden(name)
+    res = oracle.count(kind, _cat(pts), _cat(pts2) if pts2 else None, bins, mode=mode)
+    want = np.zeros_like(res["hist"])
+    for k, v in expect.items():
+        want[k] = v
+    assert np.array_equal(res["hist"], want), (name, res["hist"].nonzero(), res["hist"][res["hist"] > 0])
+    # hand fixtures keep every separation away from the edges except r = 0 / mu = 0,1 on outer edges
+    assert res["amb_cell"][:-1].sum() <= 2 * 2
+
+
+# ---------------------------------------------------------------- V2 exact lattice counts
+def test_lattice_periodic_exact(oracle):
+    """Points on an n^3 lattice in a periodic box: DD_k = N/2 * #{integer vectors v in the torus with
+    h|v| in bin k}; the vectors are enumerated here, independently of the oracle (Eq. 11, PAPER.md:85;
+    periodic wrap PAPER.md:94)."""
+    n, h = 6, 1.5
+    L = n * h
+    g = np.arange(n) * h + 0.25  # offset: the lattice need not sit on the box corner
+    x = np.array(list(itertools.product(g, g, g))).T
+    rng = np.random.default_rng(5)
+    x = x[:, rng.permutation(x.shape[1])]
+    bins = dict(n1=29, lo1=0.05 * h, hi1=2.95 * h, box_L=L)
+    edges = bins["lo1"] + (bins["hi1"] - bins["lo1"]) * np.arange(30) / 29
+    want = np.zeros(29, dtype=np.int64)
+    rep = range(-n // 2, n // 2)  # torus representatives [-n/2, n/2)
+    for v in itertools.product(rep, rep, rep):
+        m = v[0] ** 2 + v[1] ** 2 + v[2] ** 2
+        if m == 0:
+            continue
+        # minimum image of component -n/2 has the same |.|, so |v| is the minimum-image distance
+        r = h * math.sqrt(m)
+        k = np.searchsorted(edges, r, side="right") - 1
+        if 0 <= k < 29 and r < edges[-1]:
+            want[k] += 1
+    N = n ** 3
+    assert np.all((want * N) % 2 == 0)
+    want = want * N // 2
+    for mode in ("plain", "celled"):
+        res = oracle.count("monopole", tuple(x), None, bins, mode=mode)
+        assert np.array_equal(res["hist"].astype(np.int64), want)
+        assert res["amb_cell"].sum() == 0  # lattice distances sit far from the edges
+
+
+# ---------------------------------------------------------------- V1 analytic RR (statistical)
+def test_analytic_rr_uniform_periodic_box(oracle):
+    """C1 itself: uniform N=20000 in [0,1000)^3, E[DD_k] = N(N-1)/2 * 4pi/3 (e_{k+1}^3-e_k^3)/L^3
+    (north star (a); Eqs. 12-13)."""
+    w = synth.workload(1)
+    N = w.data[0].size
+    res = oracle.count("monopole", w.data, None, w.bins, mode="plain")
+    e = np.linspace(0.0, 150.0, 51)
+    rr = N * (N - 1) / 2 * 4 * math.pi / 3 * (e[1:] ** 3 - e[:-1] ** 3) / 1000.0 ** 3
+    dd = res["hist"].astype(np.float64)
+    pull = (dd - rr) / np.sqrt(rr)
+    assert np.all(np.abs(pull) < 5.0), pull
+    chi2 = float((pull ** 2).mean())
+    assert 0.4 < chi2 < 1.8, chi2
+    assert res["npairs"] == N * (N - 1) // 2
+    # the oracle's own periodic_rr is the same closed form
+    assert np.allclose(oracle.periodic_rr(N, 1000.0, w.bins), rr, rtol=1e-13)
+    # and celled mode (27 cells, wrap) agrees exactly on the same catalogue
+    res2 = oracle.count("monopole", w.data, None, w.bins, mode="celled")
+    assert np.array_equal(res2["hist"], res["hist"])
+
+
+# ---------------------------------------------------------------- V4 totals, symmetry, permutation
+def test_totals_and_symmetries(oracle):
+    rng = np.random.default_rng(11)
+    a = tuple(rng.random((3, 700)) * 50.0)
+    b = tuple(rng.random((3, 450)) * 50.0 + 10.0)
+    wide = dict(n1=37, lo1=0.0, hi1=200.0)
+    assert oracle.count("monopole", a, None, wide)["hist"].sum() == 700 * 699 // 2
+    hab = oracle.count("monopole", a, b, wide)["hist"]
+    hba = oracle.count("monopole", b, a, wide)["hist"]
+    assert hab.sum() == 700 * 450
+    assert np.array_equal(hab, hba)
+    p = rng.permutation(700)
+    ap = tuple(c[p] for c in a)
+    fine = dict(n1=64, lo1=0.0, hi1=30.0)
+    assert np.array_equal(oracle.count("monopole", a, None, fine)["hist"],
+                          oracle.count("monopole", ap, None, fine)["hist"])
+    # rmu: totals with bins covering everything (mu in [0,1] closed top)
+    shift = tuple(c + 1000.0 for c in a)
+    rm = dict(n1=7, lo1=0.0, hi1=200.0, n2=9, lo2=0.0, hi2=1.0)
+    assert oracle.count("rmu", shift, None, rm)["hist"].sum() == 700 * 699 // 2
+    # angular: theta in [0, pi] covers every pair
+    ra, dec = synth.uniform_cap(600, 30000.0, 3)
+    ang = dict(n1=50, lo1=0.0, hi1=3.2)
+    assert oracle.count("angular", (ra, dec), None, ang)["hist"].sum() == 600 * 599 // 2
+    # periodic translation invariance (up to the flagged pairs)
+    L = 50.0
+    per = dict(n1=20, lo1=0.0, hi1=25.0, box_L=L)
+    h0 = oracle.count("monopole", a, None, per)
+    a2 = tuple(np.mod(c + 17.3, L) for c in a)
+    h1 = oracle.count("monopole", a2, None, per)
+    ok, msg = oracle.parity_ok(h1["hist"], h0)
+    assert ok, msg
+
+
+# ---------------------------------------------------------------- V5 additivity
+@pytest.mark.parametrize("kind", ["monopole", "angular", "rmu", "radial"])
+def test_additivity_auto_cross(oracle, kind):
+    """auto(A u B) = auto(A) + auto(B) + cross(A, B) per bin (follows from Eq. 11)."""
+    rng = np.random.default_rng(21)
+    if kind in ("monopole", "rmu"):
+        pts = rng.random((3, 900)) * 60.0 + (500.0 if kind == "rmu" else 0.0)
+        bins = dict(n1=12, lo1=0.0, hi1=30.0)
+        if kind == "rmu":
+            bins.update(n2=5, lo2=0.0, hi2=1.0)
+    else:
+        ra, dec = synth.uniform_cap(900, 4.0, 8)
+        z = 0.2 + rng.random(900)
+        pts = np.stack([ra, dec, z])
+        if kind == "angular":
+            bins = dict(n1=16, lo1=math.radians(0.01), hi1=math.radians(1.5), log1=1)
+        else:
+            bins = dict(n1=5, lo1=0.2, hi1=1.2, n2=8, lo2=0.0, hi2=0.4, aperture=math.radians(0.1))
+    A, B = tuple(pts[:, :500]), tuple(pts[:, 500:])
+    full = oracle.count(kind, tuple(pts), None, bins)["hist"]
+    parts = (oracle.count(kind, A, None, bins)["hist"] + oracle.count(kind, B, None, bins)["hist"]
+             + oracle.count(kind, A, B, bins)["hist"])
+    assert full.sum() > 100
+    assert np.array_equal(full, parts)
+
+
+# ---------------------------------------------------------------- V6 celled == plain
+def test_celled_equals_plain_all_kinds(oracle):
+    rng = np.random.default_rng(31)
+    # periodic monopole, clustered
+    x = synth.thomas_box(3000, 120.0, 2.0, 8.0, 77)
+    y = synth.uniform_box(2500, 120.0, 78)
+    b = dict(n1=25, lo1=0.0, hi1=17.0, box_L=120.0)
+    for c2 in (None, tuple(y)):
+        p = oracle.count("monopole", tuple(x), c2, b, mode="plain")
+        c = oracle.count("monopole", tuple(x), c2, b, mode="celled")
+        assert np.array_equal(p["hist"], c["hist"]) and np.array_equal(p["amb_cell"], c["amb_cell"])
+        assert c["npairs"] < p["npairs"]
+    # non-periodic rmu with different bounding boxes for the two catalogues
+    a = tuple(rng.random((3, 2000)) * 80.0 + 900.0)
+    bb = tuple(rng.random((3, 1500)) * 100.0 + 880.0)
+    rb = dict(n1=10, lo1=0.0, hi1=12.0, n2=6, lo2=0.0, hi2=1.0)
+    for c2 in (None, bb):
+        p = oracle.count("rmu", a, c2, rb, mode="plain")
+        c = oracle.count("rmu", a, c2, rb, mode="celled")
+        assert np.array_equal(p["hist"], c["hist"])
+    # angular: footprint straddling RA = 0/360 and one containing the pole
+    for center in ((0.5, 10.0), (120.0, 89.2), (200.0, -89.5)):
+        ra, dec = synth.uniform_cap(2500, 40.0, 5, center=center)
+        ra2, dec2 = synth.thomas_cap(2000, 40.0, 0.05, 6.0, 6, center=center)
+        ab = dict(n1=20, lo1=math.radians(0.003), hi1=math.radians(0.8), log1=1)
+        for c2 in (None, (ra2, dec2)):
+            p = oracle.count("angular", (ra, dec), c2, ab, mode="plain")
+            c = oracle.count("angular", (ra, dec), c2, ab, mode="celled")
+            assert p["hist"].sum() > 1000
+            assert np.array_equal(p["hist"], c["hist"]), center
+    # radial
+    ra, dec, z = synth.gaussian_nz_cap(6000, 3.0, 0.7, 0.2, 0.2, 1.2, 9)
+    rb = dict(n1=6, lo1=0.2, hi1=1.2, n2=10, lo2=0.0, hi2=0.3, aperture=math.radians(2.0 / 60))
+    p = oracle.count("radial", (ra, dec, z), None, rb, mode="plain")
+    c = oracle.count("radial", (ra, dec, z), None, rb, mode="celled")
+    assert p["hist"].sum() > 50
+    assert np.array_equal(p["hist"], c["hist"])
+
+
+def test_islice_partitions_the_count(oracle):
+    """i-slices (used by the timed CPU baseline and the sharding test) add up to the whole."""
+    x = tuple(synth.uniform_box(1500, 100.0, 3))
+    b = dict(n1=10, lo1=0.0, hi1=40.0, box_L=100.0)
+    full = oracle.count("monopole", x, None, b)["hist"]
+    parts = sum(oracle.count("monopole", x, None, b, i_range=r, mode=m)["hist"]
+                for r, m in (((0, 400), "plain"), ((400, 1100), "celled"), ((1100, 1500), "plain")))
+    assert np.array_equal(full, parts)
+
+
+# ---------------------------------------------------------------- V7 theta: chord route == arccos route, paper's series
+def test_theta_equals_arccos_of_dot(oracle):
+    """theta = arccos(n1.n2) (Eq. 7) computed independently with numpy for theta > 1 deg,
+    where arccos is well conditioned, must land in the oracle's bins."""
+    ra, dec = synth.uniform_cap(900, 8000.0, 13, center=(40.0, -20.0))
+    bins = dict(n1=59, lo1=math.radians(1.0), hi1=math.radians(60.0))
+    res = oracle.count("angular", (ra, dec), None, bins)
+    a, d = np.radians(ra), np.radians(dec)
+    n = np.stack([np.cos(d) * np.cos(a), np.cos(d) * np.sin(a), np.sin(d)])
+    dot = np.clip(n.T @ n, -1.0, 1.0)
+    iu = np.triu_indices(ra.size, 1)
+    th = np.arccos(dot[iu])
+    want, _ = np.histogram(th, bins=np.linspace(bins["lo1"], bins["hi1"], 60))
+    ok, msg = oracle.parity_ok(want, res)  # arccos is only good to ~1e-15/sin(theta): allow flagged pairs
+    assert ok, msg
+    assert want.sum() > 50000
+
+
+def test_paper_arccos_series_pins_chord_mapping():
+    """arccos(1-x) ~ sqrt(2x + x^2/3 + 4x^3/45), '1 part in 10^4 below 40 deg'.
+    With x = chord^2/2 this pins theta = 2 asin(chord/2) <-> chord^2 = 4 sin^2(theta/2)."""
+    for deg, tol in ((0.5, 1e-12), (10.0, 1e-7), (40.0, 2e-4)):
+        th = math.radians(deg)
+        chord2 = 4.0 * math.sin(th / 2) ** 2
+        x = chord2 / 2.0
+        assert abs(x - (1.0 - math.cos(th))) < 1e-15
+        series = math.sqrt(2 * x + x * x / 3 + 4 * x ** 3 / 45)
+        assert abs(series / th - 1.0) < tol
+        assert abs(2.0 * math.asin(math.sqrt(chord2) / 2.0) / th - 1.0) < 1e-14
+
+
+# ---------------------------------------------------------------- V8 Eq. 9 identity
+def test_rmu_matches_eq9(oracle):
+    """r(z1,z2,theta), mu(z1,z2,theta) of Eq. 9 fix the mid-point line of sight."""
+    rng = np.random.default_rng(41)
+    nr, nm = 64, 64
+    bins = dict(n1=nr, lo1=0.0, hi1=400.0, n2=nm, lo2=0.0, hi2=1.0)
+    checked = 0
+    for _ in range(300):
+        c1, c2 = 1000.0 + 600.0 * rng.random(2)
+        th = 0.15 * rng.random()
+        r9 = math.sqrt(c1 * c1 + c2 * c2 - 2 * c1 * c2 * math.cos(th))
+        mu9 = abs(c1 * c1 - c2 * c2) / math.sqrt((c1 * c1 + c2 * c2) ** 2 - 4 * c1 * c1 * c2 * c2 * math.cos(th) ** 2)
+        # two directions separated by theta, randomly oriented
+        u = rng.normal(size=3); u /= np.linalg.norm(u)
+        v = rng.normal(size=3); v -= v.dot(u) * u; v /= np.linalg.norm(v)
+        x1 = c1 * u
+        x2 = c2 * (math.cos(th) * u + math.sin(th) * v)
+        res = oracle.count("rmu", tuple(np.array([x1, x2]).T), None, bins)
+        if r9 >= 400.0:
+            assert res["hist"].sum() == 0
+            continue
+        tr, tm = r9 / 400.0 * nr, mu9 * nm
+        if min(tr % 1, 1 - tr % 1, tm % 1, 1 - tm % 1) < 1e-6:
+            continue
+        cell = int(tr) * nm + min(int(tm), nm - 1)
+        assert res["hist"][cell] == 1, (r9, mu9)
+        checked += 1
+    assert checked > 200
+
+
+# ---------------------------------------------------------------- V9 / V10 estimators
+def test_landy_szalay_algebra_and_poisson(oracle):
+    rng = np.random.default_rng(51)
+    dd = rng.integers(1, 10 ** 6, 40).astype(np.uint64)
+    dr = rng.integers(1, 10 ** 6, 40).astype(np.uint64)
+    rr = rng.integers(1, 10 ** 6, 40).astype(np.uint64)
+    nd, nr = 12345, 67890
+    xi, empty = oracle.landy_szalay(dd, dr, rr, nd, nr)
+    ndd, ndr, nrr = nd * (nd - 1) / 2, nd * nr, nr * (nr - 1) / 2
+    ref = (dd / ndd - 2 * dr / ndr + rr / nrr) / (rr / nrr)  # normalised-counts form (derived from Eq. 15)
+    assert empty == 0 and np.allclose(xi, ref, rtol=1e-12, atol=1e-12)
+    xin, _ = oracle.natural(dd, rr, nd, nr)
+    assert np.allclose(xin, (dd / ndd) / (rr / nrr) - 1, rtol=1e-12)
+    rr0 = rr.copy(); rr0[3] = 0
+    xi0, empty0 = oracle.landy_szalay(dd, dr, rr0, nd, nr)
+    assert empty0 == 1 and xi0[3] == 0.0
+    # Poisson data and randoms on the same footprint: xi ~ 0 (north star (d))
+    d = tuple(rng.random((3, 3000)) * 100.0)
+    r = tuple(rng.random((3, 6000)) * 100.0)
+    b = dict(n1=10, lo1=2.0, hi1=30.0)
+    DD = oracle.count("monopole", d, None, b)["hist"]
+    DR = oracle.count("monopole", d, r, b)["hist"]
+    RR = oracle.count("monopole", r, None, b)["hist"]
+    xi, _ = oracle.landy_szalay(DD, DR, RR, 3000, 6000)
+    assert np.all(np.abs(xi) < 5.0 * (1.0 + np.abs(xi)) / np.sqrt(DD.astype(float))), xi
+
+
+# ---------------------------------------------------------------- edges, half-open bins, ambiguity flags
+def test_edges_and_halfopen_bins(oracle):
+    b = dict(n1=8, lo1=1e-3, hi1=10.0, log1=1)
+    e = oracle.edges(b)
+    assert e[0] == 1e-3 and e[-1] == 10.0
+    assert np.allclose(e, 1e-3 * (10.0 / 1e-3) ** (np.arange(9) / 8), rtol=1e-14)
+    bl = dict(n1=5, lo1=1.0, hi1=6.0)
+    assert np.array_equal(oracle.edges(bl), [1, 2, 3, 4, 5, 6])
+    # a pair exactly on an edge belongs to the upper bin; r = hi is out; r = lo is in
+    def one(r):
+        return oracle.count("monopole", (np.array([0.0, r]), np.zeros(2), np.zeros(2)), None, bl)
+    assert one(3.0)["hist"].tolist() == [0, 0, 1, 0, 0]
+    assert one(6.0)["hist"].sum() == 0
+    assert one(1.0)["hist"].tolist() == [1, 0, 0, 0, 0]
+    assert one(0.999)["hist"].sum() == 0
+    # flags: within relative 2^-20 of an edge -> both neighbouring cells (or the virtual out cell)
+    r = one(3.0 * (1 + 2.0 ** -21))
+    assert r["amb_cell"].tolist() == [0, 1, 1, 0, 0, 0] and r["amb_e1"].tolist() == [0, 0, 1, 0, 0, 0]
+    r = one(3.0 * (1 + 2.0 ** -19))
+    assert r["amb_cell"].sum() == 0
+    r = one(6.0 * (1 - 2.0 ** -21))
+    assert r["hist"][4] == 1 and r["amb_cell"].tolist() == [0, 0, 0, 0, 1, 1]
+    r = one(1.0 * (1 - 2.0 ** -21))
+    assert r["hist"].sum() == 0 and r["amb_cell"].tolist() == [1, 0, 0, 0, 0, 1]
+    # parity rule helper
+    ok, _ = oracle.parity_ok(np.array([1, 0, 0, 0, 0]), r)
+    assert ok
+    ok, _ = oracle.parity_ok(np.array([0, 1, 0, 0, 0]), r)
+    assert not ok
+
+
+def test_radial_aperture_is_strict_and_flagged(oracle):
+    ap = math.radians(1.0 / 60)
+    b = dict(n1=2, lo1=0.0, hi1=2.0, n2=2, lo2=0.0, hi2=1.0, aperture=ap)
+    def pair(sep_rad):
+        return oracle.count("radial", (np.array([10.0, 10.0]), np.array([0.0, math.degrees(sep_rad)]),
+                                       np.array([0.5, 0.8])), None, b)
+    assert pair(ap * 0.999)["hist"].tolist() == [1, 0, 0, 0]
+    assert pair(ap * 1.001)["hist"].sum() == 0
+    r = pair(ap * (1 + 2.0 ** -22))
+    assert r["amb_cell"][0] == 1 and r["amb_cell"][-1] == 1 and r["amb_e2"][-1] == 1
