@@ -93,6 +93,8 @@ typedef struct cute_grid_spec {
     double size[3];
     int ncell[3];
     double rmax;
+    int kind_mask; /* bit k set: the grid will be used for kind k (CUTE_ANGULAR=0 ...); 0 = any kind the   */
+                   /* coordinates allow.  Lets the build skip arrays a kind does not read (the low parts). */
 } cute_grid_spec;
 
 /* Binning.  Variable 1: theta [rad] (ANGULAR), r (MONOPOLE, RMU), zbar (RADIAL); linear or, if
@@ -111,7 +113,7 @@ typedef struct cute_bin_spec {
 /* Optional launch controls (NULL = defaults).  All fields 0 = default. */
 typedef struct cute_count_opts {
     size_t struct_size;
-    int blocks;            /* persistent CTAs to launch (default: 2 per SM)                          */
+    int blocks;            /* persistent CTAs to launch (default: one per SM)                        */
     int64_t item_begin;    /* shard of the work-item list [item_begin, item_end) handled by this call */
     int64_t item_end;      /* (0,0 = all). Items partition the pairs, so shards add up exactly       */
     double tau_scale;      /* multiplies the refine half-width (>1 refines more pairs; results must   */
@@ -119,6 +121,8 @@ typedef struct cute_count_opts {
     int force_refine;      /* != 0: every in-range pair is recomputed in float64                      */
     int flush_items;       /* flush the shared-memory histogram every this many work items (testing   */
                            /* the uint32 epoch logic); 0 = only when the epoch bound requires it      */
+    int warps;             /* warps per CTA (1,2,4,6,8,12,16); 0 = chosen by the library              */
+    int hist_cols;         /* private histogram columns per warp: 32 (one per lane), 8 or 1; 0 = auto */
 } cute_count_opts;
 
 /* Facts about a built grid (for tests and reports). */
@@ -141,6 +145,12 @@ typedef struct cute_grid cute_grid; /* opaque host handle; holds pointers INTO t
 int cute_version(void);
 const char *cute_strerror(int status);
 
+/* Bounding box of the raw coordinates ("a box encompassing the whole catalog is first
+ * determined"): bounds[0..2] = minima of c0,c1,c2, bounds[3..5] = maxima (HOST, out).  cat pointers are
+ * DEVICE pointers; d_tmp is a DEVICE buffer of >= 64 bytes.  Synchronises the stream.  Used to give the
+ * two grids of a cross-correlation one common explicit box. */
+int cute_catalog_bounds(const cute_catalog *cat, void *d_tmp, void *stream, double bounds[6]);
+
 /* Size of the device workspace cute_make_grid needs for this catalogue and spec (256-byte granular). */
 int cute_grid_workspace_bytes(const cute_catalog *cat, const cute_grid_spec *spec, size_t *bytes);
 
@@ -155,7 +165,7 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
 void cute_free_grid(cute_grid *g);
 int cute_grid_get_info(const cute_grid *g, cute_grid_info *info);
 
-/* Scratch the pair counter needs (work queue, per-CTA uint64 partial histograms, status word). */
+/* Scratch the pair counter needs (work-queue counter, status word, statistics, bin edges). */
 int cute_count_scratch_bytes(const cute_bin_spec *bins, const cute_count_opts *opts, size_t *bytes);
 
 /* The pair count (CUDA prior art PAPER.md:159-192).  d_hist: DEVICE uint64[n1*max(n2,1)],
@@ -165,14 +175,15 @@ int cute_count_pairs(int kind, const cute_grid *g1, const cute_grid *g2, const c
                      uint64_t *d_hist, void *d_scratch, size_t scratch_bytes,
                      const cute_count_opts *opts, void *stream);
 
+/* Number of work items cute_count_pairs enumerates for these arguments (they partition the pairs: shards
+ * [item_begin, item_end) given through cute_count_opts add up exactly to the full histogram). */
+int cute_count_items(int kind, const cute_grid *g1, const cute_grid *g2, const cute_bin_spec *bins,
+                     const cute_count_opts *opts, int64_t *nitems);
+
 /* Synchronises `stream` and returns the deferred status of the last cute_count_pairs that used
  * d_scratch.  stats (host, may be NULL): [0] separations evaluated, [1] pairs recomputed in float64,
  * [2] work items, [3] shared-memory histogram flushes. */
 int cute_count_status(void *d_scratch, void *stream, uint64_t stats[4]);
-
-/* Duration in ms of the last pair kernel + reduction enqueued with this scratch (CUDA events recorded
- * on the launch stream by cute_count_pairs; valid after cute_count_status). */
-int cute_count_last_ms(void *d_scratch, float *ms_pair, float *ms_reduce);
 
 /* End-to-end entry point with HOST buffers: copies the catalogue(s) to the device, builds the
  * grid(s), counts, copies the histogram back.  cat2 == NULL: auto.  d_workspace: DEVICE, at least

@@ -1,0 +1,807 @@
+// cute_api.cu -- the C ABI of include/cute_b200.h: validation, workspace layout, launch planning,
+// the float32 error model that decides which pairs are recomputed in float64, and the host-side
+// estimators (Eqs. 13-15).
+#include "cute_internal.h"
+#include <math.h>
+#include <new>
+#include <stdlib.h>
+#include <string.h>
+#include <vector>
+
+using namespace cute;
+
+namespace {
+
+constexpr double kPi = 3.14159265358979323846264338327950288;
+constexpr double kU = 1.0 / 16777216.0;   // 2^-24: float32 unit round-off
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+inline int sm_count()
+{
+    static int n = 0;
+    if (!n) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+    }
+    return n;
+}
+
+// ---- workspace layout of one grid -------------------------------------------------------------
+struct Layout {
+    size_t hi, lo, p64, perm, cid_sorted, cell_id, rank, count, cell_start, scan_tmp, row_nchunks, row_chunk_start, chunks,
+        row_kx, row_ylo, row_yhi, status, bbox, total;
+    uint32_t n_pad;
+    int64_t max_cells, max_rows, max_chunks;
+};
+
+inline int64_t cell_cap(int64_t n) { return n * 2 > 4096 ? n * 2 : 4096; }
+
+Layout make_layout(int64_t n, int want_lo, int want_f64, int64_t max_cells, int64_t max_rows)
+{
+    Layout L;
+    memset(&L, 0, sizeof(L));
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+    L.n_pad = (uint32_t)align_up((size_t)(n > 0 ? n : 1), 32);
+    L.max_cells = max_cells; L.max_rows = max_rows;
+    L.max_chunks = n / kChunk + max_rows + 1;
+    L.status = take(16);
+    L.bbox = take(8 * 8);
+    L.hi = take((size_t)L.n_pad * 16);
+    L.lo = want_lo ? take((size_t)L.n_pad * 16) : 0;
+    L.p64 = want_f64 ? take((size_t)L.n_pad * 32) : 0;
+    L.perm = take((size_t)L.n_pad * 4);
+    L.cid_sorted = take((size_t)L.n_pad * 4);
+    L.cell_id = take((size_t)L.n_pad * 4);
+    L.rank = take((size_t)L.n_pad * 4);
+    L.count = take((size_t)(max_cells + 2) * 4);
+    L.cell_start = take((size_t)(max_cells + 2) * 4);
+    int64_t m = max_cells > max_rows ? max_cells : max_rows;
+    L.scan_tmp = take((size_t)(m / 4096 + 2) * 4);
+    L.row_nchunks = take((size_t)(max_rows + 2) * 4);
+    L.row_chunk_start = take((size_t)(max_rows + 2) * 4);
+    L.chunks = take((size_t)L.max_chunks * sizeof(Chunk));
+    L.row_kx = take((size_t)(max_rows + 1) * 4);
+    L.row_ylo = take((size_t)(max_rows + 1) * 4);
+    L.row_yhi = take((size_t)(max_rows + 1) * 4);
+    L.total = off;
+    return L;
+}
+
+int check_catalog(const cute_catalog *c)
+{
+    if (!c || c->struct_size != sizeof(cute_catalog)) return CUTE_ERR_INVALID_ARG;
+    if (c->n < 0 || c->n > 0x7fffffff) return CUTE_ERR_INVALID_ARG;
+    if (c->coord < CUTE_COORD_XYZ || c->coord > CUTE_COORD_RADECZ) return CUTE_ERR_INVALID_ARG;
+    if (c->dtype != CUTE_F32 && c->dtype != CUTE_F64) return CUTE_ERR_INVALID_ARG;
+    if (c->n > 0) {
+        if (!c->c0 || !c->c1) return CUTE_ERR_INVALID_ARG;
+        if (c->coord != CUTE_COORD_RADEC && !c->c2) return CUTE_ERR_INVALID_ARG;
+    }
+    return CUTE_OK;
+}
+
+int check_grid_spec(const cute_catalog *c, const cute_grid_spec *s)
+{
+    if (!s || s->struct_size != sizeof(cute_grid_spec)) return CUTE_ERR_INVALID_ARG;
+    if (s->mode < CUTE_GRID_NONE || s->mode > CUTE_GRID_SPHERE) return CUTE_ERR_INVALID_ARG;
+    if (s->mode == CUTE_GRID_BOX3D && c->coord != CUTE_COORD_XYZ) return CUTE_ERR_INVALID_ARG;
+    if (s->mode == CUTE_GRID_SPHERE && c->coord == CUTE_COORD_XYZ) return CUTE_ERR_INVALID_ARG;
+    if (s->mode != CUTE_GRID_NONE && !(s->rmax > 0.0)) return CUTE_ERR_INVALID_ARG;
+    if (s->mode == CUTE_GRID_BOX3D && s->periodic) {
+        if (!(s->size[0] > 0.0) || s->size[1] != s->size[0] || s->size[2] != s->size[0]) return CUTE_ERR_INVALID_ARG;
+        if (s->origin[0] != 0.0 || s->origin[1] != 0.0 || s->origin[2] != 0.0) return CUTE_ERR_INVALID_ARG;
+    }
+    if (s->mode == CUTE_GRID_SPHERE) {
+        if (!(s->size[0] > 0.0) || s->size[0] > 360.0 || !(s->size[1] > 0.0)) return CUTE_ERR_INVALID_ARG;
+        if (s->origin[1] < -1.0 - 1e-12 || s->origin[1] + s->size[1] > 1.0 + 1e-12) return CUTE_ERR_INVALID_ARG;
+        if (s->ncell[0] <= 0 || s->ncell[1] <= 0) return CUTE_ERR_INVALID_ARG;
+        if (s->ncell[0] > 65535) return CUTE_ERR_INVALID_ARG;
+    }
+    return CUTE_OK;
+}
+
+void wants(const cute_catalog *c, const cute_grid_spec *s, int *want_lo, int *want_f64)
+{
+    int mask = s->kind_mask;
+    if (c->coord == CUTE_COORD_XYZ) {
+        *want_lo = (mask == 0) || (mask & (1 << CUTE_RMU));
+        *want_f64 = c->dtype == CUTE_F64;
+    } else {
+        *want_lo = (mask == 0) || (mask & (1 << CUTE_ANGULAR));
+        *want_f64 = 1;   // unit vectors are computed in float64 whatever the input type
+    }
+}
+
+void cell_bounds(const cute_catalog *c, const cute_grid_spec *s, int64_t *max_cells, int64_t *max_rows)
+{
+    if (s->mode == CUTE_GRID_NONE) { *max_cells = 1; *max_rows = 1; return; }
+    if (s->mode == CUTE_GRID_SPHERE) { *max_cells = (int64_t)s->ncell[0] * s->ncell[1]; *max_rows = s->ncell[1]; return; }
+    if (s->ncell[0] > 0 && s->ncell[1] > 0 && s->ncell[2] > 0) {
+        *max_cells = (int64_t)s->ncell[0] * s->ncell[1] * s->ncell[2];
+        *max_rows = (int64_t)s->ncell[1] * s->ncell[2];
+    } else {
+        *max_cells = cell_cap(c->n);
+        *max_rows = cell_cap(c->n);
+    }
+}
+
+} // namespace
+
+extern "C" {
+
+int cute_version(void) { return CUTE_ABI_VERSION; }
+
+const char *cute_strerror(int status)
+{
+    switch (status) {
+    case CUTE_OK: return "ok";
+    case CUTE_ERR_INVALID_ARG: return "invalid argument";
+    case CUTE_ERR_UNSUPPORTED: return "unsupported combination of kind, grid and binning";
+    case CUTE_ERR_WORKSPACE_TOO_SMALL: return "device workspace too small";
+    case CUTE_ERR_CUDA: return "CUDA error";
+    case CUTE_ERR_OVERFLOW: return "counter overflow";
+    case CUTE_ERR_POINT_OUT_OF_BOX: return "a point lies outside the grid box (or is not finite)";
+    case CUTE_ERR_GRID_MISMATCH: return "the two grids of a cross-correlation carry different specs";
+    case CUTE_WARN_EMPTY_BIN: return "warning: a bin with RR = 0 got xi = 0";
+    }
+    return "unknown status";
+}
+
+int cute_catalog_bounds(const cute_catalog *cat, void *d_tmp, void *stream, double bounds[6])
+{
+    int rc = check_catalog(cat);
+    if (rc) return rc;
+    if (!d_tmp || !bounds || ((uintptr_t)d_tmp & 7)) return CUTE_ERR_INVALID_ARG;
+    for (int d = 0; d < 6; d++) bounds[d] = 0.0;
+    if (cat->n == 0) return CUTE_OK;
+    BuildPlan b;
+    memset(&b, 0, sizeof(b));
+    b.c0 = cat->c0; b.c1 = cat->c1; b.c2 = cat->coord == CUTE_COORD_RADEC ? cat->c0 : cat->c2;
+    b.n = cat->n; b.dtype = cat->dtype; b.bbox = (double *)d_tmp;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (run_bbox(b, s) != cudaSuccess) return CUTE_ERR_CUDA;
+    if (cudaMemcpyAsync(bounds, d_tmp, 48, cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
+        return CUTE_ERR_CUDA;
+    for (int d = 0; d < 6; d++) if (!isfinite(bounds[d])) return CUTE_ERR_POINT_OUT_OF_BOX;
+    return CUTE_OK;
+}
+
+int cute_grid_workspace_bytes(const cute_catalog *cat, const cute_grid_spec *spec, size_t *bytes)
+{
+    int rc = check_catalog(cat);
+    if (rc) return rc;
+    if ((rc = check_grid_spec(cat, spec))) return rc;
+    if (!bytes) return CUTE_ERR_INVALID_ARG;
+    int want_lo, want_f64;
+    int64_t mc, mr;
+    wants(cat, spec, &want_lo, &want_f64);
+    cell_bounds(cat, spec, &mc, &mr);
+    if (mc > 0x7ffffff0ll) return CUTE_ERR_INVALID_ARG;
+    *bytes = make_layout(cat->n, want_lo, want_f64, mc, mr).total;
+    return CUTE_OK;
+}
+
+int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_workspace, size_t bytes, void *stream,
+                   cute_grid **out)
+{
+    int rc = check_catalog(cat);
+    if (rc) return rc;
+    if ((rc = check_grid_spec(cat, spec))) return rc;
+    if (!out || !d_workspace || ((uintptr_t)d_workspace & 255)) return CUTE_ERR_INVALID_ARG;
+    *out = nullptr;
+    cudaStream_t s = (cudaStream_t)stream;
+    int want_lo, want_f64;
+    int64_t mc, mr;
+    wants(cat, spec, &want_lo, &want_f64);
+    cell_bounds(cat, spec, &mc, &mr);
+    const Layout L = make_layout(cat->n, want_lo, want_f64, mc, mr);
+    if (bytes < L.total) return CUTE_ERR_WORKSPACE_TOO_SMALL;
+    unsigned char *w = (unsigned char *)d_workspace;
+
+    BuildPlan b;
+    memset(&b, 0, sizeof(b));
+    b.c0 = cat->c0; b.c1 = cat->c1; b.c2 = cat->coord == CUTE_COORD_RADEC ? cat->c0 : cat->c2;
+    b.n = cat->n; b.coord = cat->coord; b.dtype = cat->dtype; b.mode = spec->mode; b.periodic = spec->periodic;
+    b.want_lo = want_lo; b.want_f64 = want_f64; b.n_pad = L.n_pad;
+    b.hi = (float4 *)(w + L.hi); b.lo = want_lo ? (float4 *)(w + L.lo) : nullptr;
+    b.p64 = want_f64 ? (double *)(w + L.p64) : nullptr;
+    b.perm = (uint32_t *)(w + L.perm); b.cid_sorted = (uint32_t *)(w + L.cid_sorted);
+    b.cell_id = (uint32_t *)(w + L.cell_id); b.rank = (uint32_t *)(w + L.rank);
+    b.count = (uint32_t *)(w + L.count); b.cell_start = (uint32_t *)(w + L.cell_start);
+    b.scan_tmp = (uint32_t *)(w + L.scan_tmp); b.row_nchunks = (uint32_t *)(w + L.row_nchunks);
+    b.row_chunk_start = (uint32_t *)(w + L.row_chunk_start); b.chunks = (Chunk *)(w + L.chunks);
+    b.row_kx = (int *)(w + L.row_kx); b.row_ylo = (int *)(w + L.row_ylo); b.row_yhi = (int *)(w + L.row_yhi);
+    b.status = (uint32_t *)(w + L.status); b.bbox = (double *)(w + L.bbox);
+    b.thetamax = spec->rmax;
+
+    // bounding box of the raw coordinates ("a box encompassing the whole catalog is
+    // first determined"); also gives the magnitude bound of the float32 error model
+    double bbox[6] = {0, 0, 0, 0, 0, 0};
+    if (cat->n > 0) {
+        if (run_bbox(b, s) != cudaSuccess) return CUTE_ERR_CUDA;
+        if (cudaMemcpyAsync(bbox, b.bbox, sizeof(bbox), cudaMemcpyDeviceToHost, s) != cudaSuccess) return CUTE_ERR_CUDA;
+        if (cudaStreamSynchronize(s) != cudaSuccess) return CUTE_ERR_CUDA;
+        for (int d = 0; d < 6; d++) if (!isfinite(bbox[d])) return CUTE_ERR_POINT_OUT_OF_BOX;
+    }
+
+    cute_grid *g = new (std::nothrow) cute_grid;
+    if (!g) return CUTE_ERR_INVALID_ARG;
+    memset(g, 0, sizeof(*g));
+    g->spec = *spec;
+    g->coord = cat->coord; g->dtype = cat->dtype; g->has_lo = want_lo; g->has_f64 = want_f64;
+    int nc[3] = {1, 1, 1};
+    if (spec->mode == CUTE_GRID_BOX3D) {
+        for (int d = 0; d < 3; d++) {
+            if (!(spec->size[d] > 0.0)) {   // bounding box, widened a little so that the maximum falls inside
+                double ext = bbox[3 + d] - bbox[d];
+                double pad = 1e-6 * (ext > 0 ? ext : 1.0) + 1e-9 * fmax(fabs(bbox[d]), fabs(bbox[3 + d]));
+                g->spec.origin[d] = bbox[d] - pad;
+                g->spec.size[d] = ext + 2 * pad;
+            }
+        }
+        int64_t cap = mc;
+        for (int d = 0; d < 3; d++) {
+            if (spec->ncell[d] > 0) nc[d] = spec->ncell[d];
+            else {   // cell side ~ rmax/2  =>  k = ceil(rmax/a) = 2 (periodic needs nc >= 2k+1)
+                double t = floor(g->spec.size[d] / (0.5 * spec->rmax) * (1.0 + 1e-12));
+                nc[d] = t < 1 ? 1 : (t > 1024 ? 1024 : (int)t);
+                if (spec->periodic) {   // nearest cell count with nc >= 2 ceil(rmax/a) + 1
+                    auto ok = [&](int n) { return n >= 1 && n >= 2 * (int)ceil(spec->rmax * n / g->spec.size[d] * (1.0 + 1e-12)) + 1; };
+                    int best = 0;
+                    for (int n = nc[d]; n >= 3 && !best; n--) if (ok(n)) best = n;
+                    for (int n = nc[d] + 1; n <= nc[d] + 64 && !best; n++) if (ok(n)) best = n;
+                    if (!best) { delete g; return CUTE_ERR_UNSUPPORTED; }
+                    nc[d] = best;
+                }
+            }
+        }
+        if (!(spec->ncell[0] > 0 && spec->ncell[1] > 0 && spec->ncell[2] > 0))
+            while ((int64_t)nc[0] * nc[1] * nc[2] > cap || (int64_t)nc[1] * nc[2] > mr) {
+                int dmax = nc[0] >= nc[1] && nc[0] >= nc[2] ? 0 : (nc[1] >= nc[2] ? 1 : 2);
+                nc[dmax] = (nc[dmax] * 3 + 3) / 4;
+            }
+        if (nc[0] > 65535) { delete g; return CUTE_ERR_INVALID_ARG; }
+        for (int d = 0; d < 3; d++) {
+            g->cell[d] = g->spec.size[d] / nc[d];
+            b.origin[d] = g->spec.origin[d]; b.size[d] = g->spec.size[d]; b.inv_cell[d] = nc[d] / g->spec.size[d];
+        }
+        if (spec->periodic)
+            for (int d = 0; d < 3; d++) {
+                int k = (int)ceil(spec->rmax / g->cell[d] * (1.0 + 1e-12));
+                if (nc[d] < 2 * k + 1) { delete g; return CUTE_ERR_UNSUPPORTED; }   // a cell would be met through two images
+            }
+    } else if (spec->mode == CUTE_GRID_SPHERE) {
+        nc[0] = spec->ncell[0]; nc[1] = spec->ncell[1];
+        for (int d = 0; d < 2; d++) {
+            g->cell[d] = spec->size[d] / nc[d];
+            b.origin[d] = spec->origin[d]; b.size[d] = spec->size[d]; b.inv_cell[d] = nc[d] / spec->size[d];
+        }
+    }
+    for (int d = 0; d < 3; d++) { b.nc[d] = nc[d]; g->spec.ncell[d] = nc[d]; }
+    b.ncells = (int64_t)nc[0] * nc[1] * nc[2];
+    b.nrows = (int64_t)nc[1] * nc[2];
+    g->ncells = b.ncells; g->nrows = b.nrows;
+    // magnitude bound
+    double m = 0.0;
+    if (cat->coord == CUTE_COORD_XYZ) for (int d = 0; d < 6; d++) m = fmax(m, fabs(bbox[d]));
+    else m = fmax(fabs(bbox[2]), fabs(bbox[5]));   // RADECZ: |z| (unit vectors are <= 1)
+    g->maxabs = m;
+
+    if (run_build(b, s) != cudaSuccess) { delete g; return CUTE_ERR_CUDA; }
+    uint32_t st[2] = {0, 0};
+    if (cudaMemcpyAsync(st, b.status, 8, cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess) {
+        delete g;
+        return CUTE_ERR_CUDA;
+    }
+    if (st[0]) { delete g; return CUTE_ERR_POINT_OUT_OF_BOX; }
+    if ((int64_t)st[1] > L.max_chunks) { delete g; return CUTE_ERR_WORKSPACE_TOO_SMALL; }
+
+    GridView &v = g->view;
+    v.hi = b.hi; v.lo = b.lo; v.p64 = b.p64; v.cell_start = b.cell_start; v.chunks = b.chunks;
+    v.row_kx = b.row_kx; v.row_ylo = b.row_ylo; v.row_yhi = b.row_yhi;
+    v.n = (uint32_t)cat->n; v.n_pad = L.n_pad; v.nchunks = st[1];
+    v.ncx = nc[0]; v.ncy = nc[1]; v.ncz = nc[2];
+    g->d_perm = b.perm;
+    // algorithmic HBM bytes of the build: read the coordinates twice (cell id,
+    // scatter), write hi (+lo, +p64), perm, cell id cache (write+read), rank (write+read), counts/scan
+    const double in_b = (cat->dtype == CUTE_F64 ? 8.0 : 4.0) * (cat->coord == CUTE_COORD_RADEC ? 2 : 3);
+    g->build_bytes = (double)cat->n * (2 * in_b + 16 + (want_lo ? 16 : 0) + (want_f64 ? 32 : 0) + 4 + 4 +
+                                       (spec->mode != CUTE_GRID_NONE ? 16 : 0)) + (double)b.ncells * 12;
+    *out = g;
+    return CUTE_OK;
+}
+
+void cute_free_grid(cute_grid *g) { delete g; }
+
+int cute_grid_get_info(const cute_grid *g, cute_grid_info *info)
+{
+    if (!g || !info || info->struct_size != sizeof(cute_grid_info)) return CUTE_ERR_INVALID_ARG;
+    info->n = g->view.n; info->mode = g->spec.mode; info->periodic = g->spec.periodic;
+    info->kind_coord = g->coord; info->dtype = g->dtype; info->has_lo = g->has_lo; info->has_f64 = g->has_f64;
+    for (int d = 0; d < 3; d++) { info->ncell[d] = g->spec.ncell[d]; info->origin[d] = g->spec.origin[d]; info->cell[d] = g->cell[d]; }
+    info->ncells = g->ncells; info->nrows = g->nrows; info->nchunks = g->view.nchunks;
+    info->d_hi = g->view.hi; info->d_lo = g->view.lo; info->d_perm = g->d_perm; info->d_cell_start = g->view.cell_start;
+    info->build_bytes = g->build_bytes;
+    return CUTE_OK;
+}
+
+} // extern "C"
+
+// =============================================================================== pair counting
+namespace {
+
+int check_bins(int kind, const cute_bin_spec *b)
+{
+    if (!b || b->struct_size != sizeof(cute_bin_spec)) return CUTE_ERR_INVALID_ARG;
+    if (kind < CUTE_ANGULAR || kind > CUTE_RADIAL) return CUTE_ERR_INVALID_ARG;
+    if (b->n1 < 1 || b->n1 > 65536 || !(b->lo1 < b->hi1) || !(b->lo1 >= 0.0)) return CUTE_ERR_INVALID_ARG;
+    if (b->log1 && !(b->lo1 > 0.0)) return CUTE_ERR_INVALID_ARG;
+    const bool two = (kind == CUTE_RMU || kind == CUTE_RADIAL);
+    if (two && (b->n2 < 1 || b->n2 > 65536 || !(b->lo2 < b->hi2) || !(b->lo2 >= 0.0))) return CUTE_ERR_INVALID_ARG;
+    if (!two && b->n2 != 0) return CUTE_ERR_INVALID_ARG;
+    if ((int64_t)b->n1 * (b->n2 > 0 ? b->n2 : 1) > (1 << 20)) return CUTE_ERR_INVALID_ARG;
+    if (kind == CUTE_RADIAL && !(b->aperture_rad > 0.0 && b->aperture_rad < kPi)) return CUTE_ERR_INVALID_ARG;
+    if (kind == CUTE_ANGULAR && b->hi1 > kPi) return CUTE_ERR_INVALID_ARG;
+    if (b->box_L != 0.0) {
+        if (kind != CUTE_MONOPOLE || !(b->box_L > 0.0)) return CUTE_ERR_UNSUPPORTED;
+        if (b->hi1 > 0.5 * b->box_L) return CUTE_ERR_INVALID_ARG;   // uniqueness of the minimum image (reading S13)
+    }
+    if (kind == CUTE_RMU && b->log1) return CUTE_ERR_UNSUPPORTED;
+    return CUTE_OK;
+}
+
+void fill_edges(const cute_bin_spec *b, int axis, double *e)
+{
+    const int n = axis == 0 ? b->n1 : b->n2;
+    const double lo = axis == 0 ? b->lo1 : b->lo2, hi = axis == 0 ? b->hi1 : b->hi2;
+    const int lg = axis == 0 ? b->log1 : 0;
+    for (int k = 0; k <= n; k++)
+        e[k] = lg ? exp(log(lo) + (double)k * (log(hi) - log(lo)) / (double)n) : lo + (hi - lo) * (double)k / (double)n;
+    e[0] = lo; e[n] = hi;
+}
+
+struct ScratchLayout { size_t queue, status, stats, edges1, edges2, total; };
+ScratchLayout scratch_layout(const cute_bin_spec *b)
+{
+    ScratchLayout S;
+    S.queue = 0; S.status = 16; S.stats = 32; S.edges1 = 64;
+    S.edges2 = S.edges1 + 8 * (size_t)(b->n1 + 1);
+    S.total = align_up(S.edges2 + 8 * (size_t)(b->n2 + 1), 256);
+    return S;
+}
+
+inline double chord_of(double theta) { return 2.0 * sin(0.5 * theta); }
+
+// theta/chord as a function of q = chord^2: theta = 2 asin(c/2)
+inline double theta_over_chord(double q)
+{
+    if (q < 1e-8) return 1.0 + q / 24.0 + q * q * (3.0 / 640.0);
+    const double c = sqrt(q);
+    return 2.0 * asin(fmin(1.0, 0.5 * c)) / c;
+}
+
+// The float32 error model.  Fills a1, a2, q_hi, dz_hi.  `tau` bounds |t_float32 - t_exact| in bins;
+// derivation in DESIGN.md "Precision".
+int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid *g2, const cute_bin_spec *b, double tau_scale)
+{
+    const double M = fmax(g1->maxabs, g2->maxabs);
+    const bool f64in = (g1->dtype == CUTE_F64) || (g2->dtype == CUTE_F64);
+    const bool minimg = (kind == CUTE_MONOPOLE && p.mode == CUTE_GRID_NONE && b->box_L > 0.0);
+    const double n1 = b->n1;
+    FastAxis &A = p.a1, &B = p.a2;
+    memset(&A, 0, sizeof(A));
+    memset(&B, 0, sizeof(B));
+    A.n = b->n1; B.n = b->n2;
+    double tau1 = 0.0, rpad = 0.0;
+    if (kind == CUTE_MONOPOLE || kind == CUTE_RMU) {
+        // error of one separation component: input rounding, subtraction rounding, periodic image
+        double e_d = (f64in ? 2.0 * kU * M : 0.0) + kU * (minimg ? b->box_L : b->hi1 * 1.01);
+        if (p.periodic && !minimg) e_d += 2.0 * kU * 2.0 * b->box_L;
+        const double e_r = sqrt(3.0) * e_d;                    // | |d+e| - |d| | <= |e|
+        const double rel = 8.0 * kU;                           // q accumulation + MUFU sqrt/lg2
+        if (b->log1) {
+            const double sc = n1 / log(b->hi1 / b->lo1);       // dt = sc * dr/r
+            A.S = (float)(0.5 * sc * log(2.0));                // t = sc*ln(r/lo) = (sc ln2 / 2) * log2(q) - sc ln(lo)
+            A.O = (float)(-sc * log(b->lo1));
+            tau1 = sc * (e_r / b->lo1 + rel) + 0.5 * sc * log(2.0) * (1.0 / 2097152.0) +
+                   4.0 * kU * (fabs((double)A.S) * 260.0 + fabs((double)A.O) + n1 + 1.0);
+            rpad = b->hi1 * (1.0 + 2.0 * tau1 / sc);
+        } else {
+            const double inv = n1 / (b->hi1 - b->lo1);
+            A.S = (float)inv;
+            A.O = (float)(-b->lo1 * inv);
+            tau1 = inv * (e_r + rel * b->hi1) + 4.0 * kU * (inv * b->hi1 + fabs((double)A.O) + n1 + 1.0);
+            rpad = b->hi1 + 2.0 * tau1 / inv;
+        }
+        tau1 *= 1.25 * tau_scale;
+        rpad = (rpad + e_r) * (1.0 + 16.0 * kU);
+        p.q_hi = (float)(rpad * rpad * (1.0 + 8.0 * kU));
+        if (kind == CUTE_RMU) {
+            const double inv2 = (double)b->n2 / (b->hi2 - b->lo2);
+            B.S = (float)inv2;
+            B.O = (float)(-b->lo2 * inv2);
+            // dmu <= mu * (sqrt3 e_d / r) + 16u ;  1/r = w * |l| <= w * 2 sqrt3 M
+            B.tau = (float)(1.25 * tau_scale * (inv2 * 16.0 * kU + 4.0 * kU * (inv2 + fabs((double)B.O) + b->n2 + 1.0)));
+            B.tau_w = (float)(1.25 * tau_scale * inv2 * e_r * 2.0 * sqrt(3.0) * M);
+        }
+    } else {
+        // unit vectors.  ANGULAR: hi/lo pairs, |dd| <= 3u|d| + sqrt3 2^-47 ; RADIAL: coarse test only.
+        const double th_hi = kind == CUTE_ANGULAR ? b->hi1 : b->aperture_rad;
+        const double c_hi = chord_of(th_hi), q_hi = c_hi * c_hi;
+        if (kind == CUTE_RADIAL) {
+            const double c = c_hi * (1.0 + 1e-6) + 8.0 * kU;
+            p.q_hi = (float)(c * c * (1.0 + 8.0 * kU));
+            p.dz_hi = (float)(b->hi2 * (1.0 + 1e-6) + 4.0 * kU * M + 1e-30);
+            p.always_refine = 1;
+            return CUTE_OK;
+        }
+        const double c_lo = chord_of(b->lo1 > 0.0 ? b->lo1 : 0.0);
+        const double e_abs = sqrt(3.0) * ldexp(1.0, -46);
+        const double stretch = 1.0 / sqrt(fmax(1e-6, 1.0 - 0.25 * q_hi));     // d theta / d chord
+        const double rel = 8.0 * kU;
+        const int NS = 4096;
+        double series_err = 0.0;
+        if (b->log1) {
+            // t = sc * ln(theta/lo) = (sc ln2/2) log2(q) + sc ln(theta/c) - sc ln(lo),
+            // sc ln(theta/c) ~ q (c1 + q (c2 + q c3)), from theta/c = 1 + q/24 + 3q^2/640 + 5q^3/7168
+            const double sc = n1 / log(b->hi1 / b->lo1);
+            A.S = (float)(0.5 * sc * log(2.0));
+            A.O = (float)(-sc * log(b->lo1));
+            const double k1 = 1.0 / 24.0, k2 = 3.0 / 640.0 - 1.0 / 1152.0, k3 = 5.0 / 7168.0 - 1.0 / 5120.0 + 1.0 / 41472.0;
+            A.c1 = (float)(sc * k1); A.c2 = (float)(sc * k2); A.c3 = (float)(sc * k3);
+            for (int i = 0; i <= NS; i++) {
+                const double q = q_hi * 1.02 * (double)i / NS;
+                const double ex = sc * log(theta_over_chord(q));
+                const double se = q * ((double)A.c1 + q * ((double)A.c2 + q * (double)A.c3));
+                series_err = fmax(series_err, fabs(ex - se));
+            }
+            const double lgmax = fabs(log2(fmax(c_lo * c_lo * 0.25, 1e-37))) + 2.0;
+            tau1 = sc * stretch * (e_abs / fmax(c_lo, 1e-18) + rel) + (double)A.S * (1.0 / 2097152.0 + 2.0 * kU * lgmax) +
+                   4.0 * kU * ((double)A.S * lgmax + fabs((double)A.O) + n1 + 1.0) + 1.5 * series_err;
+            tau1 *= 1.25 * tau_scale;
+            const double cp = chord_of(fmin(kPi, b->hi1 * (1.0 + 2.0 * tau1 / sc))) * (1.0 + 32.0 * kU) + e_abs;
+            p.q_hi = (float)(fmin(4.0, cp * cp) * (1.0 + 8.0 * kU));
+        } else {
+            // t = (theta - lo)/D,  theta = c (1 + q (c1 + q (c2 + q c3)))
+            const double inv = n1 / (b->hi1 - b->lo1);
+            A.S = (float)inv;
+            A.O = (float)(-b->lo1 * inv);
+            A.c1 = (float)(1.0 / 24.0); A.c2 = (float)(3.0 / 640.0); A.c3 = (float)(5.0 / 7168.0);
+            for (int i = 0; i <= NS; i++) {
+                const double q = fmin(4.0, q_hi * 1.02) * (double)i / NS;
+                const double c = sqrt(q);
+                const double ex = c * theta_over_chord(q);
+                const double se = c * (1.0 + q * ((double)A.c1 + q * ((double)A.c2 + q * (double)A.c3)));
+                series_err = fmax(series_err, fabs(ex - se));
+            }
+            tau1 = inv * (stretch * (e_abs + rel * c_hi) + 1.5 * series_err) + 4.0 * kU * (inv * th_hi + fabs((double)A.O) + n1 + 1.0);
+            tau1 *= 1.25 * tau_scale;
+            const double cp = chord_of(fmin(kPi, b->hi1 + 2.0 * tau1 / inv)) * (1.0 + 32.0 * kU) + e_abs;
+            p.q_hi = (float)(fmin(4.0, cp * cp) * (1.0 + 8.0 * kU));
+            p.angpoly = 1;
+        }
+        if (p.q_hi >= 4.0f) p.q_hi = 5.0f;   // whole sphere in range
+    }
+    A.tau = (float)tau1;
+    A.Oa = (float)((double)A.O - tau1);
+    A.Ob = (float)((double)A.O + tau1);
+    // Oa/Ob are rounded to float32: make sure the window did not shrink
+    A.Oa = nextafterf(A.Oa, -INFINITY);
+    A.Ob = nextafterf(A.Ob, INFINITY);
+    return CUTE_OK;
+}
+
+bool same_spec(const cute_grid *a, const cute_grid *b)
+{
+    if (a->spec.mode != b->spec.mode || a->spec.periodic != b->spec.periodic || a->coord != b->coord) {
+        // coordinates may differ only between RADEC and RADECZ
+        if (a->spec.mode != b->spec.mode || a->spec.periodic != b->spec.periodic) return false;
+        if (a->coord == CUTE_COORD_XYZ || b->coord == CUTE_COORD_XYZ) return false;
+    }
+    if (a->spec.mode == CUTE_GRID_NONE) return true;
+    for (int d = 0; d < 3; d++) {
+        if (a->spec.ncell[d] != b->spec.ncell[d]) return false;
+        if (a->spec.mode == CUTE_GRID_SPHERE && d == 2) continue;
+        if (a->spec.origin[d] != b->spec.origin[d] || a->spec.size[d] != b->spec.size[d]) return false;
+    }
+    return a->spec.rmax == b->spec.rmax;
+}
+
+} // namespace
+
+extern "C" {
+
+int cute_bin_edges(const cute_bin_spec *bins, int axis, double *edges_out)
+{
+    if (!bins || bins->struct_size != sizeof(cute_bin_spec) || !edges_out || axis < 0 || axis > 1) return CUTE_ERR_INVALID_ARG;
+    const int n = axis == 0 ? bins->n1 : bins->n2;
+    const double lo = axis == 0 ? bins->lo1 : bins->lo2, hi = axis == 0 ? bins->hi1 : bins->hi2;
+    if (n < 1 || !(lo < hi) || (axis == 0 && bins->log1 && !(lo > 0.0))) return CUTE_ERR_INVALID_ARG;
+    fill_edges(bins, axis, edges_out);
+    return CUTE_OK;
+}
+
+int cute_count_scratch_bytes(const cute_bin_spec *bins, const cute_count_opts *opts, size_t *bytes)
+{
+    (void)opts;
+    if (!bins || bins->struct_size != sizeof(cute_bin_spec) || !bytes || bins->n1 < 1 || bins->n2 < 0) return CUTE_ERR_INVALID_ARG;
+    *bytes = scratch_layout(bins).total;
+    return CUTE_OK;
+}
+
+int cute_count_pairs(int kind, const cute_grid *g1, const cute_grid *g2, const cute_bin_spec *bins, uint64_t *d_hist,
+                     void *d_scratch, size_t scratch_bytes, const cute_count_opts *opts, void *stream)
+{
+    int rc = check_bins(kind, bins);
+    if (rc) return rc;
+    if (!g1 || !d_hist || !d_scratch || ((uintptr_t)d_scratch & 15)) return CUTE_ERR_INVALID_ARG;
+    if (opts && opts->struct_size != sizeof(cute_count_opts)) return CUTE_ERR_INVALID_ARG;
+    const bool is_auto = (g2 == nullptr || g2 == g1);
+    if (is_auto) g2 = g1;
+    if (!is_auto && !same_spec(g1, g2)) return CUTE_ERR_GRID_MISMATCH;
+    const ScratchLayout SL = scratch_layout(bins);
+    if (scratch_bytes < SL.total) return CUTE_ERR_WORKSPACE_TOO_SMALL;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int mode = g1->spec.mode;
+    // kind / coordinates / grid compatibility
+    const bool xyz = g1->coord == CUTE_COORD_XYZ;
+    if ((kind == CUTE_MONOPOLE || kind == CUTE_RMU) != xyz) return CUTE_ERR_INVALID_ARG;
+    if (kind == CUTE_RADIAL && (g1->coord != CUTE_COORD_RADECZ || g2->coord != CUTE_COORD_RADECZ)) return CUTE_ERR_INVALID_ARG;
+    if ((kind == CUTE_ANGULAR || kind == CUTE_RMU) && (!g1->has_lo || !g2->has_lo)) return CUTE_ERR_INVALID_ARG;
+    if (kind == CUTE_RMU && mode == CUTE_GRID_BOX3D && g1->spec.periodic) return CUTE_ERR_UNSUPPORTED;
+    const double vmax = kind == CUTE_RADIAL ? bins->aperture_rad : bins->hi1;
+    if (mode != CUTE_GRID_NONE && vmax > g1->spec.rmax * (1.0 + 1e-12)) return CUTE_ERR_INVALID_ARG;
+    if (mode == CUTE_GRID_BOX3D && g1->spec.periodic) {
+        if (kind != CUTE_MONOPOLE || bins->box_L != g1->spec.size[0]) return CUTE_ERR_INVALID_ARG;
+    } else if (mode == CUTE_GRID_BOX3D && bins->box_L > 0.0) return CUTE_ERR_INVALID_ARG;
+
+    PairParams p;
+    memset(&p, 0, sizeof(p));
+    p.g1 = g1->view; p.g2 = g2->view;
+    p.kind = kind; p.is_auto = is_auto; p.mode = mode;
+    p.periodic = (mode == CUTE_GRID_BOX3D && g1->spec.periodic) ? 1 : 0;
+    p.logbins = bins->log1 ? 1 : 0;
+    p.n1 = bins->n1; p.n2 = bins->n2; p.n2eff = bins->n2 > 0 ? bins->n2 : 1; p.nhist = p.n1 * p.n2eff;
+    p.lo1 = bins->lo1; p.hi1 = bins->hi1; p.lo2 = bins->lo2; p.hi2 = bins->hi2;
+    p.L = kind == CUTE_MONOPOLE ? bins->box_L : 0.0; p.aperture = bins->aperture_rad;
+    p.Lf = (float)p.L;
+    p.closed_top2 = (kind == CUTE_RMU && bins->hi2 >= 1.0);
+    const double tau_scale = (opts && opts->tau_scale > 0.0) ? opts->tau_scale : 1.0;
+    if ((rc = plan_fast_path(p, kind, g1, g2, bins, tau_scale))) return rc;
+    if (opts && opts->force_refine) p.always_refine = 1;
+    if (mode == CUTE_GRID_BOX3D) {
+        const double rr = g1->spec.rmax;
+        p.kx = (int)ceil(rr / g1->cell[0] * (1.0 + 1e-12));    // k = ceil(Rmax/a), reading G3
+        p.ky = (int)ceil(rr / g1->cell[1] * (1.0 + 1e-12));
+        p.kz = (int)ceil(rr / g1->cell[2] * (1.0 + 1e-12));
+        if (!p.periodic) { p.kx = p.kx < p.g2.ncx ? p.kx : p.g2.ncx; p.ky = p.ky < p.g2.ncy ? p.ky : p.g2.ncy; p.kz = p.kz < p.g2.ncz ? p.kz : p.g2.ncz; }
+        p.ax = (float)g1->cell[0]; p.ay = (float)g1->cell[1]; p.az = (float)g1->cell[2];
+        p.rmax2 = (float)(rr * rr * 1.001);
+    }
+    if (mode == CUTE_GRID_SPHERE) p.ring = g1->spec.size[0] >= 360.0 ? 1 : 0;
+
+    unsigned char *sc = (unsigned char *)d_scratch;
+    p.queue = (uint32_t *)(sc + SL.queue); p.status = (uint32_t *)(sc + SL.status);
+    p.stats = (unsigned long long *)(sc + SL.stats);
+    p.edges1 = (const double *)(sc + SL.edges1); p.edges2 = (const double *)(sc + SL.edges2);
+    p.hist = (unsigned long long *)d_hist;
+    std::vector<double> e((size_t)bins->n1 + 1 + (size_t)bins->n2 + 1);
+    fill_edges(bins, 0, e.data());
+    if (bins->n2 > 0) fill_edges(bins, 1, e.data() + bins->n1 + 1);
+    if (cudaMemsetAsync(sc, 0, 64, s) != cudaSuccess) return CUTE_ERR_CUDA;
+    if (cudaMemcpyAsync(sc + SL.edges1, e.data(), e.size() * 8, cudaMemcpyHostToDevice, s) != cudaSuccess) return CUTE_ERR_CUDA;
+    if (cudaMemsetAsync(d_hist, 0, (size_t)p.nhist * 8, s) != cudaSuccess) return CUTE_ERR_CUDA;
+    if (p.g1.n == 0 || p.g2.n == 0 || (is_auto && p.g1.n < 2)) return CUTE_OK;   // N in {0,1}: zeros
+
+    if (plan_pair_kernel(p, opts ? opts->warps : 0, opts ? opts->hist_cols : 0) < 0) return CUTE_ERR_UNSUPPORTED;
+    const int blocks = (opts && opts->blocks > 0) ? opts->blocks : sm_count();
+    // work items: grid mode = chunks; brute force = chunks x j-splits, enough for ~16 items per warp
+    uint64_t nitems = p.g1.nchunks;
+    p.nsplit = 1; p.jsplit = p.g2.n;
+    if (mode == CUTE_GRID_NONE) {
+        const uint64_t target = 16ull * (uint64_t)blocks * p.warps;
+        uint64_t ns = (target + nitems - 1) / nitems;
+        const uint64_t max_ns = ((uint64_t)p.g2.n + kTile - 1) / kTile;
+        ns = ns < 1 ? 1 : (ns > max_ns ? max_ns : ns);
+        uint64_t js = ((uint64_t)p.g2.n + ns - 1) / ns;
+        js = (js + kTile - 1) / kTile * kTile;
+        if (js > (1u << 21)) js = 1u << 21;
+        p.jsplit = (uint32_t)js;
+        p.nsplit = (uint32_t)(((uint64_t)p.g2.n + js - 1) / js);
+        nitems *= p.nsplit;
+    }
+    if (nitems > 0xfffffff0ull) return CUTE_ERR_OVERFLOW;
+    p.item_begin = 0; p.item_end = (uint32_t)nitems;
+    if (opts && (opts->item_begin || opts->item_end)) {
+        if (opts->item_begin < 0 || opts->item_end < opts->item_begin) return CUTE_ERR_INVALID_ARG;
+        p.item_begin = (uint32_t)(opts->item_begin < (int64_t)nitems ? opts->item_begin : (int64_t)nitems);
+        p.item_end = (uint32_t)(opts->item_end < (int64_t)nitems ? opts->item_end : (int64_t)nitems);
+    }
+    p.flush_items = opts ? (uint32_t)opts->flush_items : 0u;
+    if (launch_pair_kernel(p, blocks, s) != cudaSuccess) return CUTE_ERR_CUDA;
+    return CUTE_OK;
+}
+
+int cute_count_items(int kind, const cute_grid *g1, const cute_grid *g2, const cute_bin_spec *bins, const cute_count_opts *opts,
+                     int64_t *nitems)
+{
+    // number of work items cute_count_pairs would enumerate (for sharding with item_begin/item_end)
+    if (!g1 || !nitems || !bins) return CUTE_ERR_INVALID_ARG;
+    if (!g2) g2 = g1;
+    uint64_t n = g1->view.nchunks;
+    if (g1->spec.mode == CUTE_GRID_NONE && n > 0 && g2->view.n > 0) {
+        PairParams p;
+        memset(&p, 0, sizeof(p));
+        p.kind = kind;
+        p.nhist = bins->n1 * (bins->n2 > 0 ? bins->n2 : 1);
+        if (plan_pair_kernel(p, opts ? opts->warps : 0, opts ? opts->hist_cols : 0) < 0) return CUTE_ERR_UNSUPPORTED;
+        const int blocks = (opts && opts->blocks > 0) ? opts->blocks : sm_count();
+        const uint64_t target = 16ull * (uint64_t)blocks * p.warps;
+        uint64_t ns = (target + n - 1) / n;
+        const uint64_t max_ns = ((uint64_t)g2->view.n + kTile - 1) / kTile;
+        ns = ns < 1 ? 1 : (ns > max_ns ? max_ns : ns);
+        uint64_t js = ((uint64_t)g2->view.n + ns - 1) / ns;
+        js = (js + kTile - 1) / kTile * kTile;
+        if (js > (1u << 21)) js = 1u << 21;
+        n *= ((uint64_t)g2->view.n + js - 1) / js;
+    }
+    *nitems = (int64_t)n;
+    return CUTE_OK;
+}
+
+int cute_count_status(void *d_scratch, void *stream, uint64_t stats[4])
+{
+    if (!d_scratch) return CUTE_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    unsigned char h[64];
+    if (cudaMemcpyAsync(h, d_scratch, 64, cudaMemcpyDeviceToHost, s) != cudaSuccess) return CUTE_ERR_CUDA;
+    if (cudaStreamSynchronize(s) != cudaSuccess) return CUTE_ERR_CUDA;
+    if (stats) memcpy(stats, h + 32, 32);
+    uint32_t st;
+    memcpy(&st, h + 16, 4);
+    if (st & 2u) return CUTE_ERR_OVERFLOW;
+    if (st) return CUTE_ERR_CUDA;
+    return CUTE_OK;
+}
+
+} // extern "C"
+
+// =============================================================================== end-to-end with host buffers
+namespace {
+
+size_t cat_bytes(const cute_catalog *c)
+{
+    const size_t col = align_up((size_t)(c->n > 0 ? c->n : 1) * (c->dtype == CUTE_F64 ? 8 : 4), 256);
+    return col * 3;
+}
+
+} // namespace
+
+extern "C" {
+
+int cute_host_workspace_bytes(const cute_catalog *cat1, const cute_catalog *cat2, const cute_grid_spec *spec,
+                              const cute_bin_spec *bins, size_t *bytes)
+{
+    if (!bytes || !bins || bins->struct_size != sizeof(cute_bin_spec)) return CUTE_ERR_INVALID_ARG;
+    size_t total = 0, w = 0;
+    int rc = cute_grid_workspace_bytes(cat1, spec, &w);
+    if (rc) return rc;
+    total += align_up(w, 256) + cat_bytes(cat1);
+    if (cat2) {
+        if ((rc = cute_grid_workspace_bytes(cat2, spec, &w))) return rc;
+        total += align_up(w, 256) + cat_bytes(cat2);
+    }
+    total += align_up((size_t)bins->n1 * (bins->n2 > 0 ? bins->n2 : 1) * 8, 256);
+    total += scratch_layout(bins).total;
+    *bytes = total;
+    return CUTE_OK;
+}
+
+int cute_count_pairs_host(int kind, const cute_catalog *cat1, const cute_catalog *cat2, const cute_grid_spec *spec,
+                          const cute_bin_spec *bins, uint64_t *h_hist, void *d_workspace, size_t bytes, void *stream)
+{
+    size_t need = 0;
+    int rc = cute_host_workspace_bytes(cat1, cat2, spec, bins, &need);
+    if (rc) return rc;
+    if (!h_hist || !d_workspace || ((uintptr_t)d_workspace & 255)) return CUTE_ERR_INVALID_ARG;
+    if (bytes < need) return CUTE_ERR_WORKSPACE_TOO_SMALL;
+    if ((rc = check_bins(kind, bins))) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    unsigned char *w = (unsigned char *)d_workspace;
+    const cute_catalog *cats[2] = {cat1, cat2};
+    cute_grid *grids[2] = {nullptr, nullptr};
+    for (int k = 0; k < 2 && rc == CUTE_OK; k++) {
+        const cute_catalog *c = cats[k];
+        if (!c) break;
+        cute_catalog dc = *c;
+        const size_t esz = c->dtype == CUTE_F64 ? 8 : 4;
+        const size_t col = align_up((size_t)(c->n > 0 ? c->n : 1) * esz, 256);
+        const void *src[3] = {c->c0, c->c1, c->c2};
+        const void **dst[3] = {&dc.c0, &dc.c1, &dc.c2};
+        for (int d = 0; d < 3; d++) {
+            *dst[d] = w + col * d;
+            if (src[d] && c->n > 0 && cudaMemcpyAsync(w + col * d, src[d], (size_t)c->n * esz, cudaMemcpyHostToDevice, s) != cudaSuccess)
+                rc = CUTE_ERR_CUDA;
+            if (!src[d]) *dst[d] = nullptr;
+        }
+        w += col * 3;
+        size_t gw = 0;
+        if (rc == CUTE_OK) rc = cute_grid_workspace_bytes(c, spec, &gw);
+        if (rc == CUTE_OK) rc = cute_make_grid(&dc, spec, w, gw, stream, &grids[k]);
+        w += align_up(gw, 256);
+    }
+    if (rc == CUTE_OK) {
+        const size_t nh = (size_t)bins->n1 * (bins->n2 > 0 ? bins->n2 : 1);
+        uint64_t *d_hist = (uint64_t *)w;
+        w += align_up(nh * 8, 256);
+        const size_t sb = scratch_layout(bins).total;
+        rc = cute_count_pairs(kind, grids[0], grids[1], bins, d_hist, w, sb, nullptr, stream);
+        if (rc == CUTE_OK && cudaMemcpyAsync(h_hist, d_hist, nh * 8, cudaMemcpyDeviceToHost, s) != cudaSuccess) rc = CUTE_ERR_CUDA;
+        if (rc == CUTE_OK) rc = cute_count_status(w, stream, nullptr);
+    }
+    cute_free_grid(grids[0]);
+    cute_free_grid(grids[1]);
+    return rc;
+}
+
+// =============================================================================== host-side estimators
+/* Landy-Szalay, Eq. 15: xi = [Nr(Nr-1)/(Nd(Nd-1)) DD - (Nr-1)/Nd DR + RR] / RR with DD and RR
+ * unordered pair counts and DR all Nd*Nr pairs. */
+int cute_landy_szalay(const uint64_t *dd, const uint64_t *dr, const uint64_t *rr, uint64_t nd, uint64_t nr, int nbins, double *xi)
+{
+    if (!dd || !dr || !rr || !xi || nbins < 1 || nd < 2 || nr < 2) return CUTE_ERR_INVALID_ARG;
+    const double Nd = (double)nd, Nr = (double)nr;
+    const double wdd = Nr * (Nr - 1.0) / (Nd * (Nd - 1.0)), wdr = (Nr - 1.0) / Nd;
+    int warn = CUTE_OK;
+    for (int k = 0; k < nbins; k++) {
+        if (rr[k] == 0) { xi[k] = 0.0; warn = CUTE_WARN_EMPTY_BIN; continue; }
+        xi[k] = (wdd * (double)dd[k] - wdr * (double)dr[k] + (double)rr[k]) / (double)rr[k];
+    }
+    return warn;
+}
+
+/* natural estimator, Eq. 14: xi = Nr(Nr-1)/(Nd(Nd-1)) DD/RR - 1 */
+int cute_natural_estimator(const uint64_t *dd, const uint64_t *rr, uint64_t nd, uint64_t nr, int nbins, double *xi)
+{
+    if (!dd || !rr || !xi || nbins < 1 || nd < 2 || nr < 2) return CUTE_ERR_INVALID_ARG;
+    const double Nd = (double)nd, Nr = (double)nr;
+    const double wdd = Nr * (Nr - 1.0) / (Nd * (Nd - 1.0));
+    int warn = CUTE_OK;
+    for (int k = 0; k < nbins; k++) {
+        if (rr[k] == 0) { xi[k] = 0.0; warn = CUTE_WARN_EMPTY_BIN; continue; }
+        xi[k] = wdd * (double)dd[k] / (double)rr[k] - 1.0;
+    }
+    return warn;
+}
+
+/* Periodic box (Eqs. 12-13, with the exact shell volume and N(N-1)/2 unordered pairs) */
+int cute_periodic_rr(uint64_t n, double L, const cute_bin_spec *bins, double *rr)
+{
+    if (!bins || bins->struct_size != sizeof(cute_bin_spec) || !rr || !(L > 0.0) || bins->n1 < 1 || !(bins->lo1 < bins->hi1)) return CUTE_ERR_INVALID_ARG;
+    if (bins->log1 && !(bins->lo1 > 0.0)) return CUTE_ERR_INVALID_ARG;
+    std::vector<double> e((size_t)bins->n1 + 1);
+    fill_edges(bins, 0, e.data());
+    const double np = 0.5 * (double)n * ((double)n - 1.0), v = L * L * L;
+    for (int k = 0; k < bins->n1; k++) {
+        const double a = e[k], b = e[k + 1];
+        rr[k] = np * (4.0 * kPi / 3.0) * (b * b * b - a * a * a) / v;
+    }
+    return CUTE_OK;
+}
+
+int cute_periodic_xi(const uint64_t *dd, uint64_t n, double L, const cute_bin_spec *bins, double *xi)
+{
+    if (!dd || !xi) return CUTE_ERR_INVALID_ARG;
+    int rc = cute_periodic_rr(n, L, bins, xi);
+    if (rc) return rc;
+    int warn = CUTE_OK;
+    for (int k = 0; k < bins->n1; k++) {
+        if (!(xi[k] > 0.0)) { xi[k] = 0.0; warn = CUTE_WARN_EMPTY_BIN; continue; }
+        xi[k] = (double)dd[k] / xi[k] - 1.0;
+    }
+    return warn;
+}
+
+} // extern "C"

@@ -9,18 +9,16 @@
 namespace cute {
 
 // ---- compile-time shape of the pair kernel -------------------------------------------------
-constexpr int kLanes = 32;
 constexpr int kIPerLane = 4;                      // R: i-points held in registers per lane
-constexpr int kChunk = kLanes * kIPerLane;        // 128 i-points per work item
-constexpr int kConsumerWarps = 8;
-constexpr int kConsumerThreads = kConsumerWarps * 32;
-constexpr int kThreads = kConsumerThreads + 32;   // + 1 producer warp
-constexpr int kTile = 512;                        // j-points per shared-memory tile (8 KB of float4)
-constexpr int kStages = 4;
-constexpr int kJSplit = 64 * kTile;               // brute force: j-range per work item
+constexpr int kChunk = 32 * kIPerLane;            // 128 i-points per work item (one warp)
+constexpr int kTile = 128;                        // j-points per shared-memory tile (2 KB of float4)
+constexpr int kStages = 2;                        // double buffering
+constexpr int kSegBatch = 32;                     // neighbour rows expanded per batch (one per lane)
+constexpr int kSegSlots = 3 * kSegBatch;          // <= 3 contiguous j-segments per neighbour row
+constexpr int kRefineCap = 64;                    // deferred float64 recomputations queued per warp
+constexpr int kMaxWarps = 16;
 constexpr float kSentinel = 1.0e18f;              // coordinate of a padding i-point (never in range)
-constexpr unsigned kMagicBits = 0x4B400000u;      // bits of 1.5 * 2^23
-#define CUTE_MAGIC_F 12582912.0f
+constexpr uint32_t kEpochJ = 1u << 22;            // flush a warp's uint32 histogram after this many j
 
 struct Chunk {            // one work item's i side: <=128 consecutive cell-sorted points of one cell row
     uint32_t i_begin;
@@ -59,19 +57,25 @@ struct cute_grid {
 namespace cute {
 
 // ---- pair-kernel parameters ------------------------------------------------------------------
-struct FastAxis {      // float32 bin map  t = g*S + O  (in bins), evaluated at t-tau and t+tau
-    float S, Oa, Ob;   // Oa = O - tau, Ob = O + tau
-    float c1, c2;      // ANGULAR: series correction coefficients (see pair_count.cu)
+// float32 bin map of one variable: t = S*g(q) + O + q*(c1 + q*(c2 + q*c3)) in units of bins, where
+// g = sqrt(q) (linear bins) or log2(q) (log bins).  The pair is binned by the fast path only if
+// floor(t - tau) == floor(t + tau); otherwise it is recomputed in float64.
+struct FastAxis {
+    float S, O, c1, c2, c3;
+    float tau, tau_w;      // tau_eff = tau + tau_w * w   (w: kind-specific, see pair_count.cu)
+    float Oa, Ob;          // O - tau, O + tau
     int n;
 };
 
 struct PairParams {
     GridView g1, g2;
     int kind, is_auto, mode, periodic;
-    int binmode;                 // 0: linear lo=0, 1: linear, 2: log
+    int logbins;                 // variable 1: 0 linear, 1 log
+    int angpoly;                 // ANGULAR linear bins: theta = sqrt(q) * poly(q)
     int always_refine;           // 1: every pair passing the coarse test is recomputed in float64
-    int n1, n2, n2eff, nhist;    // nhist = (n1+2)*n2eff (one guard row below and above)
-    float q_lo, q_hi;            // coarse float32 range test on q (padded by half a bin)
+    int n1, n2, n2eff, nhist;    // nhist = n1 * n2eff
+    int colshift;                // histogram columns per warp copy = 1 << colshift (32, 8 or 1)
+    float q_hi;                  // coarse float32 range test on q (padded)
     float dz_hi;                 // RADIAL: coarse test on |dz|
     FastAxis a1, a2;
     // float64 side (refine path): exact definition
@@ -82,22 +86,23 @@ struct PairParams {
     float Lf;
     int kx, ky, kz;
     float ax, ay, az;            // cell sizes
-    float rmax2;                 // pruning radius^2 (padded)
-    float rmax;
+    float rmax2;                 // row-pruning radius^2 (padded)
+    int ring;                    // SPHERE: RA axis covers 360 deg (neighbour window wraps)
     // work
     uint32_t *queue;             // [0] next item
     uint32_t *status;            // [0] error word
     unsigned long long *stats;   // [0] evaluated, [1] refined, [2] items, [3] flushes
-    unsigned long long *partial; // [blocks][nhist]
-    uint32_t item_begin, item_end, nsplit;
+    unsigned long long *hist;    // [nhist] global result
+    uint32_t item_begin, item_end, nsplit, jsplit;
     uint32_t flush_items;
+    int warps;                   // warps per CTA
+    uint32_t smem_per_warp;      // bytes
 };
 
 // host-side launchers (pair_count.cu / grid_build.cu)
 cudaError_t launch_pair_kernel(const PairParams &p, int blocks, cudaStream_t s);
-cudaError_t launch_reduce(const unsigned long long *partial, int blocks, int n1, int n2eff, unsigned long long *hist, cudaStream_t s);
-int pair_kernel_smem_bytes(const PairParams &p);
-int pair_kernel_max_blocks_per_sm(const PairParams &p);
+// fills colshift, warps, smem_per_warp; returns total dynamic shared memory or -1 if it cannot fit
+int plan_pair_kernel(PairParams &p, int want_warps, int want_cols);
 
 struct BuildPlan {
     // inputs
@@ -116,7 +121,7 @@ struct BuildPlan {
     Chunk *chunks;
     int *row_kx, *row_ylo, *row_yhi;
     uint32_t *status;  // [0] err, [1] nchunks
-    double *bbox;      // [6] min xyz, max xyz, [6] maxabs
+    double *bbox;      // [6] min xyz, max xyz
     int64_t ncells, nrows;
 };
 cudaError_t run_bbox(const BuildPlan &b, cudaStream_t s);

@@ -213,7 +213,9 @@ __global__ void k_scatter(BuildPlan b)
     uint32_t slot, id = 0;
     if (b.mode == CUTE_GRID_NONE) slot = (uint32_t)i;
     else { id = b.cell_id[i]; slot = b.cell_start[id] + b.rank[i]; }
-    double v[4] = {a, c1, c2, 0.0};
+    // XYZ: w carries |x|^2 split hi/lo, so that the (r,mu) kernel gets s.l = |x_i|^2 - |x_j|^2 without
+    // cancellation (l = x_i + x_j is the mid-point line of sight)
+    double v[4] = {a, c1, c2, a * a + c1 * c1 + c2 * c2};
     if (b.coord != CUTE_COORD_XYZ) {
         double al = a * (kPi / 180.0), de = c1 * (kPi / 180.0), sa, ca, sd, cd;
         sincos(al, &sa, &ca);

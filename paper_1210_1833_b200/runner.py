@@ -1,0 +1,84 @@
+"""Driving the C ABI for a whole workload (used by bench.py, smoke() and the GPU tests).
+
+Only plumbing lives here: host->device copies with torch, building the grids, enqueuing the pair
+counts of DD / DR / RR and reading the histograms back.  All arithmetic is in libcute_b200.so.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from . import api
+
+
+def to_device(cat, coord: int, dtype=None):
+    """numpy SoA columns -> contiguous torch CUDA tensors (one dtype)."""
+    import torch
+    need = 2 if coord == api.COORD_RADEC else 3
+    cols = []
+    for c in list(cat)[:need]:
+        a = np.ascontiguousarray(c)
+        if dtype is not None:
+            a = a.astype(dtype, copy=False)
+        elif a.dtype not in (np.float32, np.float64):
+            a = a.astype(np.float64)
+        cols.append(torch.from_numpy(a).cuda())
+    return cols
+
+
+class Job:
+    """One correlation-function job: catalogues resident on the device, grids built, counters ready."""
+
+    def __init__(self, kind: str, data, rand, bins: dict, grid: dict | None = None, opts: dict | None = None):
+        self.kind_name = kind
+        self.kind = api.KINDS[kind]
+        self.coord = api.COORD_OF_KIND[kind]
+        self.bins = dict(bins)
+        self.grid = dict(grid or {"mode": "none"})
+        self.opts = api.count_opts(**opts) if opts else None
+        self.d_data = to_device(data, self.coord)
+        self.d_rand = to_device(rand, self.coord) if rand is not None else None
+        self.nd = int(self.d_data[0].numel())
+        self.nr = int(self.d_rand[0].numel()) if self.d_rand is not None else 0
+        self.counter = api.Counter(self.bins)
+        self.g_data = self.g_rand = None
+        self.spec = None
+
+    def build(self):
+        """G0-G4 for every catalogue (cute_make_grid)."""
+        cats = [self.d_data] + ([self.d_rand] if self.d_rand is not None else [])
+        if self.spec is None:
+            self.spec = api.auto_spec(self.kind_name, self.bins, self.grid, cats, self.coord)
+        if self.g_data is not None:
+            self.g_data.free()
+        self.g_data = api.cute_make_grid(self.d_data, self.coord, self.spec, workspace=getattr(self, "_ws_d", None))
+        self._ws_d = self.g_data.workspace
+        if self.d_rand is not None:
+            if self.g_rand is not None:
+                self.g_rand.free()
+            self.g_rand = api.cute_make_grid(self.d_rand, self.coord, self.spec, workspace=getattr(self, "_ws_r", None))
+            self._ws_r = self.g_rand.workspace
+        return self
+
+    def grids(self, which: str):
+        return {"DD": (self.g_data, None), "DR": (self.g_data, self.g_rand), "RR": (self.g_rand, None)}[which]
+
+    def enqueue(self, which: str):
+        g1, g2 = self.grids(which)
+        return api.cute_count_pairs(self.kind, g1, g2, self.counter, self.opts)
+
+    def count(self, which: str = "DD"):
+        """Histogram (numpy uint64) and the kernel's statistics for one of DD / DR / RR."""
+        h = self.enqueue(which)
+        st = api.cute_count_status(self.counter)
+        return h.cpu().numpy().astype(np.uint64), st
+
+    def total_pairs(self, which: str) -> int:
+        if which == "DD":
+            return self.nd * (self.nd - 1) // 2
+        if which == "RR":
+            return self.nr * (self.nr - 1) // 2
+        return self.nd * self.nr
+
+
+def job_for_workload(w, opts: dict | None = None) -> Job:
+    return Job(w.kind, w.data, w.rand, w.bins, w.grid, opts)

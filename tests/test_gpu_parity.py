@@ -1,0 +1,253 @@
+"""GPU parity: the CUDA path (through the C ABI) against the float64 oracle, element by element.
+
+Bar (BASELINE.json north_star): histograms equal the oracle's exactly, per cell and in total,
+except for pairs the oracle flags as lying within relative 2^-20 of a bin edge -- oracle.parity_ok
+implements |gpu[c] - oracle[c]| <= amb_cell[c] and |sum gpu - sum oracle| <= amb_out.
+Integer work (cell lists, permutations) is compared bit-exactly.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from conftest import load_golden
+
+pytestmark = pytest.mark.gpu
+
+GOLDEN = ["monopole_345.txt", "monopole_periodic.txt", "monopole_cross.txt", "angular_equator.txt",
+          "angular_log.txt", "rmu_345.txt", "rmu_los.txt", "radial_ladder.txt"]
+
+
+@pytest.fixture(scope="module")
+def rt():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1210_1833_b200 import api, runner, synth
+    return api, runner, synth
+
+
+def _cat(pts, kind):
+    a = np.array(pts, dtype=np.float64).T
+    return tuple(np.ascontiguousarray(c) for c in a)
+
+
+def _run(runner, kind, data, rand, bins, grid=None, opts=None, which=("DD",)):
+    job = runner.Job(kind, data, rand, bins, grid, opts).build()
+    return {w: job.count(w) for w in which}, job
+
+
+@pytest.mark.parametrize("name", GOLDEN)
+def test_golden_fixtures(rt, name):
+    """the hand-enumerated catalogues of tests/golden (paper definitions, Eq. 11)"""
+    api, runner, synth = rt
+    kind, bins, pts, pts2, expect = load_golden(name)
+    data = _cat(pts, kind)
+    rand = _cat(pts2, kind) if pts2 else None
+    which = "DR" if rand is not None else "DD"
+    out, job = _run(runner, kind, data, rand, bins, which=(which,))
+    h, st = out[which]
+    want = np.zeros(h.size, dtype=np.uint64)
+    for k, v in expect.items():
+        want[k] = v
+    assert np.array_equal(h, want), (h.nonzero(), want.nonzero())
+
+
+def _parity(oracle, h, kind, c1, c2, bins, mode="plain"):
+    orc = oracle.count(kind, c1, c2, bins, mode=mode)
+    ok, msg = oracle.parity_ok(h, orc)
+    assert ok, msg
+    return orc
+
+
+@pytest.mark.parametrize("scale,opts", [(0.05, None), (0.1, dict(warps=4)), (0.1, dict(hist_cols=1, flush_items=3)),
+                                        (0.1, dict(force_refine=1)), (0.1, dict(tau_scale=50.0))])
+def test_c1_periodic_brute(rt, oracle, scale, opts):
+    api, runner, synth = rt
+    w = synth.workload(1, scale)
+    out, job = _run(runner, w.kind, w.data, None, w.bins, w.grid, opts)
+    h, st = out["DD"]
+    orc = _parity(oracle, h, w.kind, w.data, None, w.bins)
+    assert st["evaluated"] == job.total_pairs("DD") == orc["npairs"]
+
+
+@pytest.mark.parametrize("scale", [0.01, 0.03])
+def test_c2_angular_log(rt, oracle, scale):
+    api, runner, synth = rt
+    w = synth.workload(2, scale)
+    out, job = _run(runner, w.kind, w.data, w.rand, w.bins, w.grid, which=("DD", "DR", "RR"))
+    _parity(oracle, out["DD"][0], w.kind, w.data, None, w.bins)
+    _parity(oracle, out["DR"][0], w.kind, w.data, w.rand, w.bins)
+    _parity(oracle, out["RR"][0], w.kind, w.rand, None, w.bins)
+    assert out["DR"][1]["evaluated"] == job.nd * job.nr
+
+
+def test_c2_angular_sphere_grid_equals_brute(rt, oracle):
+    """V6: grid-assisted == brute force, log bins up to 2 deg on a pixel grid"""
+    api, runner, synth = rt
+    w = synth.workload(2, 0.03)
+    bins = dict(w.bins, hi1=math.radians(2.0), n1=52)
+    out_b, _ = _run(runner, w.kind, w.data, w.rand, bins, dict(mode="none"), which=("DD", "DR"))
+    out_g, job = _run(runner, w.kind, w.data, w.rand, bins, dict(mode="sphere", thetamax=bins["hi1"], pix=0.5), which=("DD", "DR"))
+    for k in ("DD", "DR"):
+        assert np.array_equal(out_b[k][0], out_g[k][0])
+        assert out_g[k][1]["evaluated"] < out_b[k][1]["evaluated"]
+    _parity(oracle, out_g["DD"][0], w.kind, w.data, None, bins)
+
+
+def test_angular_linear_wide(rt, oracle):
+    """the paper's own angular binning: linear in theta up to 30 deg"""
+    api, runner, synth = rt
+    w = synth.workload(2, 0.02)
+    bins = dict(n1=256, lo1=0.0, hi1=math.radians(30.0), log1=0, n2=0, lo2=0.0, hi2=0.0, aperture=0.0, box_L=0.0)
+    out, job = _run(runner, "angular", w.data, w.rand, bins, which=("DD", "DR"))
+    _parity(oracle, out["DD"][0], "angular", w.data, None, bins)
+    _parity(oracle, out["DR"][0], "angular", w.data, w.rand, bins)
+
+
+@pytest.mark.parametrize("ncell", [(0, 0, 0), (7, 9, 11)])
+def test_c3_rmu_grid(rt, oracle, ncell):
+    api, runner, synth = rt
+    w = synth.workload(3, 0.02)
+    grid = dict(w.grid, ncell=ncell)
+    out, job = _run(runner, w.kind, w.data, w.rand, w.bins, grid, which=("DD", "DR", "RR"))
+    _parity(oracle, out["DD"][0], w.kind, w.data, None, w.bins, "celled")
+    _parity(oracle, out["DR"][0], w.kind, w.data, w.rand, w.bins, "celled")
+    _parity(oracle, out["RR"][0], w.kind, w.rand, None, w.bins, "celled")
+    # and brute force gives the same integers
+    out_b, _ = _run(runner, w.kind, w.data, w.rand, w.bins, dict(mode="none"), which=("DD", "DR"))
+    assert np.array_equal(out_b["DD"][0], out["DD"][0])
+    assert np.array_equal(out_b["DR"][0], out["DR"][0])
+
+
+@pytest.mark.parametrize("pix", [2.0, 0.7])
+def test_c4_radial_sphere_grid(rt, oracle, pix):
+    api, runner, synth = rt
+    w = synth.workload(4, 0.05)
+    grid = dict(w.grid, pix=pix)
+    out, job = _run(runner, w.kind, w.data, None, w.bins, grid)
+    h, st = out["DD"]
+    orc = _parity(oracle, h, w.kind, w.data, None, w.bins, "celled")
+    assert h.sum() > 0
+    # a wider aperture on a small catalogue against the PLAIN oracle
+    w2 = synth.workload(4, 0.002)
+    bins = dict(w2.bins, aperture=math.radians(0.5))
+    out2, _ = _run(runner, w2.kind, w2.data, None, bins, dict(mode="sphere", thetamax=bins["aperture"], pix=pix))
+    _parity(oracle, out2["DD"][0], w2.kind, w2.data, None, bins, "plain")
+    out3, _ = _run(runner, w2.kind, w2.data, None, bins, dict(mode="none"))
+    assert np.array_equal(out2["DD"][0], out3["DD"][0])
+
+
+@pytest.mark.parametrize("scale,ncell", [(0.002, (0, 0, 0)), (0.002, (5, 7, 9)), (0.0005, (0, 0, 0))])
+def test_c5_periodic_grid(rt, oracle, scale, ncell):
+    api, runner, synth = rt
+    w = synth.workload(5, scale)
+    grid = dict(w.grid, ncell=ncell)
+    out, job = _run(runner, w.kind, w.data, w.rand, w.bins, grid, which=("DD", "DR"))
+    _parity(oracle, out["DD"][0], w.kind, w.data, None, w.bins, "celled")
+    _parity(oracle, out["DR"][0], w.kind, w.data, w.rand, w.bins, "celled")
+    out_b, _ = _run(runner, w.kind, w.data, w.rand, w.bins, dict(mode="none"), which=("DD", "DR"))
+    assert np.array_equal(out_b["DD"][0], out["DD"][0])
+    assert np.array_equal(out_b["DR"][0], out["DR"][0])
+    assert out["DD"][1]["evaluated"] < out_b["DD"][1]["evaluated"]
+
+
+def test_monopole_log_bins(rt, oracle):
+    """logarithmic binning of the monopole"""
+    api, runner, synth = rt
+    w = synth.workload(5, 0.001)
+    bins = dict(w.bins, lo1=0.5, log1=1, n1=48)
+    out, job = _run(runner, w.kind, w.data, w.rand, bins, w.grid, which=("DD", "DR"))
+    _parity(oracle, out["DD"][0], w.kind, w.data, None, bins, "celled")
+    _parity(oracle, out["DR"][0], w.kind, w.data, w.rand, bins, "celled")
+
+
+def test_edge_cases(rt, oracle):
+    api, runner, synth = rt
+    bins = dict(n1=8, lo1=0.0, hi1=10.0, log1=0, n2=0, lo2=0.0, hi2=0.0, aperture=0.0, box_L=0.0)
+    rng = np.random.default_rng(5)
+    for n in (0, 1, 2, 127, 128, 129, 257):
+        x = tuple(rng.random((3, n)) * 8.0)
+        out, job = _run(runner, "monopole", x, None, bins)
+        h = out["DD"][0]
+        if n > 1:
+            orc = _parity(oracle, h, "monopole", x, None, bins)
+            assert out["DD"][1]["evaluated"] == n * (n - 1) // 2
+        else:
+            assert h.sum() == 0
+    # coincident points: r = 0 is a pair in bin 0 (reading S4); cross counts everything
+    x = (np.array([1.0, 1.0, 5.0]), np.array([2.0, 2.0, 2.0]), np.array([3.0, 3.0, 3.0]))
+    out, _ = _run(runner, "monopole", x, x, bins, which=("DD", "DR"))
+    assert out["DD"][0][0] == 1 and out["DD"][0].sum() == 3
+    assert out["DR"][0][0] == 5 and out["DR"][0].sum() == 9
+
+
+def test_permutation_invariance_and_sharding(rt):
+    """V4: the histogram is invariant under a permutation of the input (an integer race detector);
+    shards of the work-item list add up exactly (the multi-GPU path of DESIGN.md)."""
+    api, runner, synth = rt
+    w = synth.workload(5, 0.002)
+    out, job = _run(runner, w.kind, w.data, w.rand, w.bins, w.grid, which=("DD", "DR"))
+    rng = np.random.default_rng(1)
+    p = rng.permutation(w.data[0].size)
+    data2 = tuple(c[p] for c in w.data)
+    out2, _ = _run(runner, w.kind, data2, w.rand, w.bins, w.grid, which=("DD", "DR"))
+    assert np.array_equal(out["DD"][0], out2["DD"][0]) and np.array_equal(out["DR"][0], out2["DR"][0])
+    g1, g2 = job.grids("DR")
+    n = api.cute_count_items(job.kind, g1, g2, job.counter)
+    acc = np.zeros_like(out["DR"][0])
+    for a, b in ((0, n // 3), (n // 3, n // 2), (n // 2, n)):
+        if a == b:
+            continue
+        job.opts = api.count_opts(item_begin=a, item_end=b)
+        acc += job.count("DR")[0]
+    assert np.array_equal(acc, out["DR"][0])
+
+
+def test_cell_list_is_a_permutation(rt):
+    """G1-G3 bit-exact: perm is a permutation, cell_start is the exclusive scan of the cell histogram,
+    and every sorted point lies in its cell."""
+    import torch
+    api, runner, synth = rt
+    w = synth.workload(5, 0.003)
+    job = runner.job_for_workload(w).build()
+    inf = job.g_data.info()
+    n, nc = inf.n, inf.ncells
+    perm = torch.empty(n, dtype=torch.int32, device="cuda")
+    cs = torch.empty(nc + 1, dtype=torch.int32, device="cuda")
+    hi = torch.empty(n * 4, dtype=torch.float32, device="cuda")
+    import ctypes
+    cudart = torch.cuda.cudart()
+    for dst, src, nb in ((perm, inf.d_perm, n * 4), (cs, inf.d_cell_start, (nc + 1) * 4), (hi, inf.d_hi, n * 16)):
+        assert int(cudart.cudaMemcpy(dst.data_ptr(), src, nb, 3)) == 0
+    perm, cs, hi = perm.cpu().numpy().astype(np.int64), cs.cpu().numpy().astype(np.int64), hi.cpu().numpy().reshape(n, 4)
+    assert np.array_equal(np.sort(perm), np.arange(n))
+    x = np.stack(w.data, axis=1)[perm]
+    assert np.array_equal(hi[:, :3], x.astype(np.float32))
+    ncx, ncy, ncz = inf.ncell[0], inf.ncell[1], inf.ncell[2]
+    cell = np.array([inf.cell[0], inf.cell[1], inf.cell[2]])
+    k = np.minimum(np.floor(x.astype(np.float64) / cell).astype(np.int64), [ncx - 1, ncy - 1, ncz - 1])
+    cid = (k[:, 2] * ncy + k[:, 1]) * ncx + k[:, 0]
+    assert np.all(np.diff(cid) >= 0)
+    want = np.concatenate([[0], np.cumsum(np.bincount(cid, minlength=nc))])
+    assert np.array_equal(cs, want)
+
+
+def test_host_entry_point_and_estimators(rt, oracle):
+    """cute_count_pairs_host (HOST buffers) == device path; Landy-Szalay on identical histograms
+    agrees with the oracle's Eq. 15 to 1e-6 absolute (north star)."""
+    api, runner, synth = rt
+    w = synth.workload(2, 0.02)
+    out, job = _run(runner, w.kind, w.data, w.rand, w.bins, w.grid, which=("DD", "DR", "RR"))
+    spec = api.grid_spec("none")
+    hh, _ = api.cute_count_pairs_host(job.kind, w.data, w.rand, job.coord, spec, w.bins)
+    assert np.array_equal(hh, out["DR"][0])
+    dd, dr, rr = out["DD"][0], out["DR"][0], out["RR"][0]
+    xi, rc = api.cute_landy_szalay(dd, dr, rr, job.nd, job.nr)
+    xo, empty = oracle.landy_szalay(dd, dr, rr, job.nd, job.nr)
+    assert np.max(np.abs(xi - xo)) <= 1e-6
+    assert (rc == api.WARN_EMPTY_BIN) == (empty > 0)
+    w1 = synth.workload(1, 0.1)
+    o1, j1 = _run(runner, w1.kind, w1.data, None, w1.bins, w1.grid)
+    rr1 = api.cute_periodic_rr(j1.nd, w1.bins["box_L"], w1.bins)
+    assert np.allclose(rr1, oracle.periodic_rr(j1.nd, w1.bins["box_L"], w1.bins), rtol=1e-13)
