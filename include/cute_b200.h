@@ -144,6 +144,8 @@ typedef struct cute_grid cute_grid; /* opaque host handle; holds pointers INTO t
 
 int cute_version(void);
 const char *cute_strerror(int status);
+/* Number of CUDA kernels this library has launched in this process so far (for reports). */
+uint64_t cute_launch_count(void);
 
 /* Bounding box of the raw coordinates ("a box encompassing the whole catalog is first
  * determined"): bounds[0..2] = minima of c0,c1,c2, bounds[3..5] = maxima (HOST, out).  cat pointers are
@@ -187,11 +189,12 @@ int cute_count_status(void *d_scratch, void *stream, uint64_t stats[4]);
 
 /* End-to-end entry point with HOST buffers: copies the catalogue(s) to the device, builds the
  * grid(s), counts, copies the histogram back.  cat2 == NULL: auto.  d_workspace: DEVICE, at least
- * cute_host_workspace_bytes().  Synchronous. */
+ * cute_host_workspace_bytes().  opts may be NULL.  Synchronous. */
 int cute_host_workspace_bytes(const cute_catalog *cat1, const cute_catalog *cat2, const cute_grid_spec *spec,
                               const cute_bin_spec *bins, size_t *bytes);
 int cute_count_pairs_host(int kind, const cute_catalog *cat1, const cute_catalog *cat2, const cute_grid_spec *spec,
-                          const cute_bin_spec *bins, uint64_t *h_hist, void *d_workspace, size_t bytes, void *stream);
+                          const cute_bin_spec *bins, const cute_count_opts *opts, uint64_t *h_hist, void *d_workspace,
+                          size_t bytes, void *stream);
 
 /* ---- host-side helpers (all pointers HOST) ---- */
 /* Bin edges, the single definition: n+1 doubles for axis 0 or 1. */

@@ -55,7 +55,7 @@ class cute_grid_info(C.Structure):
 
 
 # every symbol include/cute_b200.h declares
-SYMBOLS = ["cute_version", "cute_strerror", "cute_catalog_bounds", "cute_grid_workspace_bytes", "cute_make_grid", "cute_free_grid",
+SYMBOLS = ["cute_version", "cute_strerror", "cute_launch_count", "cute_catalog_bounds", "cute_grid_workspace_bytes", "cute_make_grid", "cute_free_grid",
            "cute_grid_get_info", "cute_count_scratch_bytes", "cute_count_pairs", "cute_count_items",
            "cute_count_status", "cute_host_workspace_bytes", "cute_count_pairs_host", "cute_bin_edges",
            "cute_landy_szalay", "cute_natural_estimator", "cute_periodic_rr", "cute_periodic_xi"]
@@ -70,6 +70,7 @@ def _load() -> C.CDLL:
     lib.cute_version.restype = C.c_int
     lib.cute_strerror.restype = C.c_char_p
     lib.cute_strerror.argtypes = [C.c_int]
+    lib.cute_launch_count.restype = C.c_uint64
     lib.cute_catalog_bounds.argtypes = [C.POINTER(cute_catalog), vp, vp, dp]
     lib.cute_grid_workspace_bytes.argtypes = [C.POINTER(cute_catalog), C.POINTER(cute_grid_spec), C.POINTER(C.c_size_t)]
     lib.cute_make_grid.argtypes = [C.POINTER(cute_catalog), C.POINTER(cute_grid_spec), vp, C.c_size_t, vp, C.POINTER(vp)]
@@ -84,7 +85,7 @@ def _load() -> C.CDLL:
     lib.cute_host_workspace_bytes.argtypes = [C.POINTER(cute_catalog), C.POINTER(cute_catalog), C.POINTER(cute_grid_spec),
                                               C.POINTER(cute_bin_spec), C.POINTER(C.c_size_t)]
     lib.cute_count_pairs_host.argtypes = [C.c_int, C.POINTER(cute_catalog), C.POINTER(cute_catalog), C.POINTER(cute_grid_spec),
-                                          C.POINTER(cute_bin_spec), up, vp, C.c_size_t, vp]
+                                          C.POINTER(cute_bin_spec), C.POINTER(cute_count_opts), up, vp, C.c_size_t, vp]
     lib.cute_bin_edges.argtypes = [C.POINTER(cute_bin_spec), C.c_int, dp]
     lib.cute_landy_szalay.argtypes = [up, up, up, C.c_uint64, C.c_uint64, C.c_int, dp]
     lib.cute_natural_estimator.argtypes = [up, up, C.c_uint64, C.c_uint64, C.c_int, dp]
@@ -110,6 +111,10 @@ def _check(rc: int, where: str) -> int:
 
 def cute_version() -> int:
     return int(lib.cute_version())
+
+
+def cute_launch_count() -> int:
+    return int(lib.cute_launch_count())
 
 
 def cute_strerror(status: int) -> str:
@@ -269,7 +274,8 @@ def cute_count_status(counter: Counter, stream=None) -> dict:
     return dict(evaluated=int(st[0]), refined=int(st[1]), items=int(st[2]), flushes=int(st[3]))
 
 
-def cute_count_pairs_host(kind: int, cat1, cat2, coord: int, spec: cute_grid_spec, bins: dict, workspace=None, stream=None):
+def cute_count_pairs_host(kind: int, cat1, cat2, coord: int, spec: cute_grid_spec, bins: dict, workspace=None, stream=None,
+                          opts: cute_count_opts | None = None):
     """End to end with HOST (numpy) buffers: H2D copies, grid build, count, D2H of the histogram."""
     torch = _torch()
     c1, k1 = _catalog([np.ascontiguousarray(c) for c in cat1], coord, False)
@@ -285,7 +291,7 @@ def cute_count_pairs_host(kind: int, cat1, cat2, coord: int, spec: cute_grid_spe
     off = (-workspace.data_ptr()) % 256
     hist = np.zeros(b.n1 * max(b.n2, 1), dtype=np.uint64)
     _check(lib.cute_count_pairs_host(int(kind), C.byref(c1), C.byref(c2) if c2 is not None else None, C.byref(spec), C.byref(b),
-                                     hist.ctypes.data_as(C.POINTER(C.c_uint64)), C.c_void_p(workspace.data_ptr() + off),
+                                     C.byref(opts) if opts is not None else None, hist.ctypes.data_as(C.POINTER(C.c_uint64)), C.c_void_p(workspace.data_ptr() + off),
                                      workspace.numel() - off, C.c_void_p(_stream_ptr(stream))), "cute_count_pairs_host")
     return hist, workspace
 

@@ -10,6 +10,10 @@
 
 using namespace cute;
 
+#include <atomic>
+static std::atomic<unsigned long long> g_launches{0};
+namespace cute { void note_launches(int n) { g_launches += (unsigned long long)n; } }
+
 namespace {
 
 constexpr double kPi = 3.14159265358979323846264338327950288;
@@ -132,6 +136,8 @@ void cell_bounds(const cute_catalog *c, const cute_grid_spec *s, int64_t *max_ce
 extern "C" {
 
 int cute_version(void) { return CUTE_ABI_VERSION; }
+
+uint64_t cute_launch_count(void) { return g_launches.load(); }
 
 const char *cute_strerror(int status)
 {
@@ -700,7 +706,8 @@ int cute_host_workspace_bytes(const cute_catalog *cat1, const cute_catalog *cat2
 }
 
 int cute_count_pairs_host(int kind, const cute_catalog *cat1, const cute_catalog *cat2, const cute_grid_spec *spec,
-                          const cute_bin_spec *bins, uint64_t *h_hist, void *d_workspace, size_t bytes, void *stream)
+                          const cute_bin_spec *bins, const cute_count_opts *opts, uint64_t *h_hist, void *d_workspace,
+                          size_t bytes, void *stream)
 {
     size_t need = 0;
     int rc = cute_host_workspace_bytes(cat1, cat2, spec, bins, &need);
@@ -737,7 +744,7 @@ int cute_count_pairs_host(int kind, const cute_catalog *cat1, const cute_catalog
         uint64_t *d_hist = (uint64_t *)w;
         w += align_up(nh * 8, 256);
         const size_t sb = scratch_layout(bins).total;
-        rc = cute_count_pairs(kind, grids[0], grids[1], bins, d_hist, w, sb, nullptr, stream);
+        rc = cute_count_pairs(kind, grids[0], grids[1], bins, d_hist, w, sb, opts, stream);
         if (rc == CUTE_OK && cudaMemcpyAsync(h_hist, d_hist, nh * 8, cudaMemcpyDeviceToHost, s) != cudaSuccess) rc = CUTE_ERR_CUDA;
         if (rc == CUTE_OK) rc = cute_count_status(w, stream, nullptr);
     }

@@ -99,6 +99,9 @@ struct PairParams {
     uint32_t smem_per_warp;      // bytes
 };
 
+// number of kernels this library has launched (reported by cute_launch_count)
+void note_launches(int n);
+
 // host-side launchers (pair_count.cu / grid_build.cu)
 cudaError_t launch_pair_kernel(const PairParams &p, int blocks, cudaStream_t s);
 // fills colshift, warps, smem_per_warp; returns total dynamic shared memory or -1 if it cannot fit

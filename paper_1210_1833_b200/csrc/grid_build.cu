@@ -79,6 +79,7 @@ cudaError_t run_bbox(const BuildPlan &b, cudaStream_t s)
         k_bbox<<<blocks, 256, 0, s>>>(b);
     }
     k_bbox_decode<<<1, 32, 0, s>>>(b.bbox);
+    note_launches(b.n > 0 ? 3 : 2);
     return cudaGetLastError();
 }
 
@@ -196,6 +197,7 @@ static cudaError_t exclusive_scan(const uint32_t *in, int64_t n, uint32_t *out, 
     k_scan_sums<<<nb, kScanBlock, 0, s>>>(in, n, tmp);
     k_scan_top<<<1, kScanBlock, 0, s>>>(tmp, nb);
     k_scan_final<<<nb, kScanBlock, 0, s>>>(in, n, tmp, out);
+    note_launches(3);
     return cudaGetLastError();
 }
 
@@ -299,15 +301,16 @@ cudaError_t run_build(const BuildPlan &b, cudaStream_t s)
     if ((e = cudaMemsetAsync(b.status, 0, 8, s)) != cudaSuccess) return e;
     if (b.mode != CUTE_GRID_NONE) {
         if ((e = cudaMemsetAsync(b.count, 0, (size_t)(b.ncells + 1) * 4, s)) != cudaSuccess) return e;
-        if (b.n > 0) k_cellid<<<blocks, T, 0, s>>>(b);
+        if (b.n > 0) { k_cellid<<<blocks, T, 0, s>>>(b); note_launches(1); }
         if ((e = exclusive_scan(b.count, b.ncells, b.cell_start, b.scan_tmp, s)) != cudaSuccess) return e;
     }
-    if (b.n > 0) k_scatter<<<blocks, T, 0, s>>>(b);
+    if (b.n > 0) { k_scatter<<<blocks, T, 0, s>>>(b); note_launches(1); }
     k_row_counts<<<(int)((b.nrows + T - 1) / T), T, 0, s>>>(b);
     if ((e = exclusive_scan(b.row_nchunks, b.nrows, b.row_chunk_start, b.scan_tmp, s)) != cudaSuccess) return e;
     uint32_t max_chunks = (uint32_t)(b.n / kChunk + b.nrows + 1);
     k_chunks<<<(max_chunks + T - 1) / T, T, 0, s>>>(b, max_chunks);
-    if (b.mode == CUTE_GRID_SPHERE) k_sphere_rows<<<(b.nc[1] + T - 1) / T, T, 0, s>>>(b);
+    if (b.mode == CUTE_GRID_SPHERE) { k_sphere_rows<<<(b.nc[1] + T - 1) / T, T, 0, s>>>(b); note_launches(1); }
+    note_launches(2);   // k_row_counts, k_chunks
     return cudaGetLastError();
 }
 

@@ -582,6 +582,7 @@ static cudaError_t launch_t(const PairParams &p, int blocks, cudaStream_t s)
     cudaError_t e = cudaFuncSetAttribute(pair_kernel<KIND, MINIMG, LOGB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     pair_kernel<KIND, MINIMG, LOGB><<<blocks, 32 * p.warps, smem, s>>>(p);
+    note_launches(1);
     return cudaGetLastError();
 }
 
