@@ -446,22 +446,21 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
         const double c_lo = chord_of(b->lo1 > 0.0 ? b->lo1 : 0.0);
         const double e_abs = sqrt(3.0) * ldexp(1.0, -46);
         const double stretch = 1.0 / sqrt(fmax(1e-6, 1.0 - 0.25 * q_hi));     // d theta / d chord
-        const double rel = 8.0 * kU;
+        const double rel = 12.0 * kU;
         const int NS = 4096;
         double series_err = 0.0;
         if (b->log1) {
-            // t = sc * ln(theta/lo) = (sc ln2/2) log2(q) + sc ln(theta/c) - sc ln(lo),
-            // sc ln(theta/c) ~ q (c1 + q (c2 + q c3)), from theta/c = 1 + q/24 + 3q^2/640 + 5q^3/7168
+            // t = sc * ln(theta/lo) = (sc ln2/2) log2(theta^2) - sc ln(lo)
             const double sc = n1 / log(b->hi1 / b->lo1);
             A.S = (float)(0.5 * sc * log(2.0));
             A.O = (float)(-sc * log(b->lo1));
-            const double k1 = 1.0 / 24.0, k2 = 3.0 / 640.0 - 1.0 / 1152.0, k3 = 5.0 / 7168.0 - 1.0 / 5120.0 + 1.0 / 41472.0;
-            A.c1 = (float)(sc * k1); A.c2 = (float)(sc * k2); A.c3 = (float)(sc * k3);
-            for (int i = 0; i <= NS; i++) {
-                const double q = q_hi * 1.02 * (double)i / NS;
-                const double ex = sc * log(theta_over_chord(q));
-                const double se = q * ((double)A.c1 + q * ((double)A.c2 + q * (double)A.c3));
-                series_err = fmax(series_err, fabs(ex - se));
+            // theta^2 = 4 asin^2(c/2) = q (1 + q/12 + q^2/90 + q^3/560 + ...): the kernel takes log2 of q*poly(q)
+            A.c1 = 1.0f; A.c2 = (float)(1.0 / 12.0); A.c3 = (float)(1.0 / 90.0);
+            for (int i = 1; i <= NS; i++) {
+                const double q = fmin(4.0, q_hi * 1.02) * (double)i / NS;
+                const double toc = theta_over_chord(q);
+                const double se = (double)A.c1 + q * ((double)A.c2 + q * (double)A.c3);
+                series_err = fmax(series_err, 0.5 * sc * fabs(log(toc * toc / se)));
             }
             const double lgmax = fabs(log2(fmax(c_lo * c_lo * 0.25, 1e-37))) + 2.0;
             tau1 = sc * stretch * (e_abs / fmax(c_lo, 1e-18) + rel) + (double)A.S * (1.0 / 2097152.0 + 2.0 * kU * lgmax) +
@@ -470,16 +469,16 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
             const double cp = chord_of(fmin(kPi, b->hi1 * (1.0 + 2.0 * tau1 / sc))) * (1.0 + 32.0 * kU) + e_abs;
             p.q_hi = (float)(fmin(4.0, cp * cp) * (1.0 + 8.0 * kU));
         } else {
-            // t = (theta - lo)/D,  theta = c (1 + q (c1 + q (c2 + q c3)))
+            // t = (theta - lo)/D,  theta = c (1 + q/24 + 3 q^2/640 + ...)
             const double inv = n1 / (b->hi1 - b->lo1);
             A.S = (float)inv;
             A.O = (float)(-b->lo1 * inv);
-            A.c1 = (float)(1.0 / 24.0); A.c2 = (float)(3.0 / 640.0); A.c3 = (float)(5.0 / 7168.0);
+            A.c1 = 1.0f; A.c2 = (float)(1.0 / 24.0); A.c3 = (float)(3.0 / 640.0);
             for (int i = 0; i <= NS; i++) {
                 const double q = fmin(4.0, q_hi * 1.02) * (double)i / NS;
                 const double c = sqrt(q);
                 const double ex = c * theta_over_chord(q);
-                const double se = c * (1.0 + q * ((double)A.c1 + q * ((double)A.c2 + q * (double)A.c3)));
+                const double se = c * ((double)A.c1 + q * ((double)A.c2 + q * (double)A.c3));
                 series_err = fmax(series_err, fabs(ex - se));
             }
             tau1 = inv * (stretch * (e_abs + rel * c_hi) + 1.5 * series_err) + 4.0 * kU * (inv * th_hi + fabs((double)A.O) + n1 + 1.0);

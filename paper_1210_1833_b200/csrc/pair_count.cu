@@ -75,6 +75,12 @@ __device__ __forceinline__ float fast_lg2(float x)
     return y;
 }
 
+// shared-memory increment without a return value
+__device__ __forceinline__ void red_shared(uint32_t addr)
+{
+    asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(addr) : "memory");
+}
+
 #define CUTE_MAGIC_F 12582912.0f        /* 1.5 * 2^23: adding it with round-down leaves floor(t) in the mantissa */
 #define CUTE_MAGIC_BITS 0x4B400000
 
@@ -190,7 +196,7 @@ __device__ __forceinline__ WarpSmem carve(unsigned char *ws)
 static inline uint32_t warp_smem_bytes(bool needlo, int nhist, int colshift)
 {
     uint32_t b = kStages * kTileBytes * (needlo ? 2 : 1) + kSegSlots * 16 + kRefineCap * 8 + 32;
-    b += (((uint32_t)nhist << colshift) * 4 + 15) & ~15u;
+    b += (((uint32_t)(nhist + 1) << colshift) * 4 + 15) & ~15u;   // + one dump row
     return (b + 127) & ~127u;
 }
 
@@ -237,17 +243,55 @@ __device__ __forceinline__ uint32_t drain_refine(const PairParams &p, const Warp
 struct IPoints {           // the R i-points of this lane (float32 fast path)
     float x[R], y[R], z[R], w[R];      // hi (x,y,z already shifted by the segment's periodic image), w
     float lx[R], ly[R], lz[R], lw[R];  // lo parts (ANGULAR) / lo of |x|^2 in lw (RMU)
-    uint32_t idx[R];                   // cell-sorted index (j>i mask, refine)
+    uint32_t idx0;                     // cell-sorted index of i-point 0 (point r is idx0 + 32 r)
 };
 
-template <int KIND, bool MINIMG, bool LOGB, bool MASK>
-__device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem &s, const IPoints &ip,
+struct Consts {            // loop constants held in registers (not re-read from the constant bank)
+    float q_hi, dz_hi, Lf;
+    float S1, Oa1, Ob1, c1, c2, c3;
+    float S2, O2, tau2, tauw2;
+    uint32_t n1, n2;
+};
+
+__device__ __forceinline__ Consts load_consts(const PairParams &p)
+{
+    Consts c;
+    c.q_hi = p.q_hi; c.dz_hi = p.dz_hi; c.Lf = p.Lf;
+    c.S1 = p.a1.S; c.Oa1 = p.a1.Oa; c.Ob1 = p.a1.Ob; c.c1 = p.a1.c1; c.c2 = p.a1.c2; c.c3 = p.a1.c3;
+    c.S2 = p.a2.S; c.O2 = p.a2.O; c.tau2 = p.a2.tau; c.tauw2 = p.a2.tau_w;
+    c.n1 = (uint32_t)p.n1; c.n2 = (uint32_t)p.n2;
+    return c;
+}
+
+// rare path: queue the pairs of this lane whose float32 bin is not certain (bit r of `need`)
+template <int KIND>
+__device__ __noinline__ void push_refine(const PairParams &p, const WarpSmem &s, uint32_t need, uint32_t idx0, uint32_t j,
+                                         uint32_t hoff, uint32_t &refined_inline)
+{
+    for (int r = 0; r < R; r++) {
+        if (!(need & (1u << r))) continue;
+        const uint32_t i = idx0 + 32u * r;
+        const uint32_t slot = atomicAdd(s.rq_count, 1u);
+        if (slot < (uint32_t)kRefineCap) s.rq[slot] = make_uint2(i, j);
+        else {
+            const int cell = refine_cell<KIND>(p, i, j);
+            refined_inline++;
+            if (cell >= 0) atomicAdd(s.hist + (((uint32_t)cell << p.colshift) + hoff), 1u);
+        }
+    }
+}
+
+// COLS32: one histogram column per lane (compile-time shift); ALWAYS: every candidate pair goes to float64
+template <int KIND, bool MINIMG, bool LOGB, bool MASK, bool COLS32, bool ALWAYS>
+__device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem &s, const Consts &c, const IPoints &ip,
                                              const float4 *th, const float4 *tl, uint32_t cnt, uint32_t j0,
                                              int lane, uint32_t &refined_inline)
 {
-    const uint32_t colmask = (1u << p.colshift) - 1u;
-    uint32_t *hcol = s.hist + (lane & colmask);
-    const float Lf = p.Lf;
+    const uint32_t cs = COLS32 ? 5u : (uint32_t)p.colshift;
+    const uint32_t hoff = (uint32_t)lane & ((1u << cs) - 1u);
+    // bin k of column hoff lives at hbase[(k << cs)]; the magic-number bits are folded into the base
+    const uint32_t dump_s = smem_u32(s.hist + (((uint32_t)p.nhist << cs) + hoff));
+    const uint32_t hbase_s = smem_u32(s.hist + hoff) - ((uint32_t)CUTE_MAGIC_BITS << (cs + 2u));   // shared-space byte address
 #pragma unroll 2
     for (uint32_t jj = 0; jj < cnt; jj++) {
         const float4 pj = th[jj];
@@ -261,70 +305,58 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
                 dx += ip.lx[r] - pl.x; dy += ip.ly[r] - pl.y; dz += ip.lz[r] - pl.z;
             }
             if (MINIMG) {                    // periodic brute force: minimum image
-                dx = fminf(fabsf(dx), Lf - fabsf(dx));
-                dy = fminf(fabsf(dy), Lf - fabsf(dy));
-                dz = fminf(fabsf(dz), Lf - fabsf(dz));
+                dx = fminf(fabsf(dx), c.Lf - fabsf(dx));
+                dy = fminf(fabsf(dy), c.Lf - fabsf(dy));
+                dz = fminf(fabsf(dz), c.Lf - fabsf(dz));
             }
             q[r] = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            if (MASK) q[r] = (j0 + jj > ip.idx[r]) ? q[r] : 3.0e38f;   // auto-correlation: j > i only
+            if (MASK) q[r] = (j0 + jj > ip.idx0 + 32u * r) ? q[r] : 3.0e38f;   // auto-correlation: j > i only
         }
         const float qm = fminf(fminf(q[0], q[1]), fminf(q[2], q[3]));
-        if (qm < p.q_hi) {
+        if (qm < c.q_hi) {
+            uint32_t need = 0;
             float nlo = 0.f;
             if (KIND == CUTE_RMU) nlo = tl[jj].w;
 #pragma unroll
             for (int r = 0; r < R; r++) {
-                if (!(q[r] < p.q_hi)) continue;
-                bool need;
-                int cell;
-                bool valid;
                 if (KIND == CUTE_RADIAL) {
-                    if (!(fabsf(ip.w[r] - pj.w) < p.dz_hi)) continue;
-                    need = true; cell = 0; valid = false;
-                } else {
-                    // variable 1
-                    float g = LOGB ? fast_lg2(q[r]) : fast_sqrt(q[r]);
-                    float ta, tb;
-                    if (KIND == CUTE_ANGULAR) {
-                        const float poly = fmaf(q[r], fmaf(q[r], p.a1.c3, p.a1.c2), p.a1.c1);
-                        if (LOGB) { const float c = q[r] * poly; ta = fmaf(g, p.a1.S, c + p.a1.Oa); tb = fmaf(g, p.a1.S, c + p.a1.Ob); }
-                        else { g = fmaf(g * q[r], poly, g); ta = fmaf(g, p.a1.S, p.a1.Oa); tb = fmaf(g, p.a1.S, p.a1.Ob); }
-                    } else {
-                        ta = fmaf(g, p.a1.S, p.a1.Oa);
-                        tb = fmaf(g, p.a1.S, p.a1.Ob);
-                    }
-                    const int ka = __float_as_int(__fadd_rd(ta, CUTE_MAGIC_F)) - CUTE_MAGIC_BITS;
-                    const int kb = __float_as_int(__fadd_rd(tb, CUTE_MAGIC_F)) - CUTE_MAGIC_BITS;
-                    need = ka != kb;
-                    valid = (uint32_t)ka < (uint32_t)p.n1;
-                    cell = ka;
-                    if (KIND == CUTE_RMU) {
-                        // mu = |s.l| / (|s||l|) with s.l = |x_i|^2 - |x_j|^2 (hi/lo) and |l|^2 = 2|x_i|^2 + 2|x_j|^2 - q
-                        const float pn = (ip.w[r] - pj.w) + (ip.lw[r] - nlo);
-                        const float m = fmaf(2.0f, ip.w[r] + pj.w, -q[r]);
-                        const float w = fast_rsqrt(q[r] * m);
-                        const float t2 = fmaf(fabsf(pn) * w, p.a2.S, p.a2.O);
-                        const float tau2 = fmaf(w, p.a2.tau_w, p.a2.tau);
-                        const int k2a = __float_as_int(__fadd_rd(t2 - tau2, CUTE_MAGIC_F)) - CUTE_MAGIC_BITS;
-                        const int k2b = __float_as_int(__fadd_rd(t2 + tau2, CUTE_MAGIC_F)) - CUTE_MAGIC_BITS;
-                        need = need || (k2a != k2b) || !(q[r] > 0.f);
-                        valid = valid && ((uint32_t)k2a < (uint32_t)p.n2);
-                        cell = ka * p.n2 + k2a;
-                    }
-                    if (p.always_refine) need = true;
+                    if (q[r] < c.q_hi && fabsf(ip.w[r] - pj.w) < c.dz_hi) need |= 1u << r;
+                    continue;
                 }
-                if (need) {
-                    const uint32_t slot = atomicAdd(s.rq_count, 1u);
-                    if (slot < (uint32_t)kRefineCap) s.rq[slot] = make_uint2(ip.idx[r], j0 + jj);
-                    else {
-                        cell = refine_cell<KIND>(p, ip.idx[r], j0 + jj);
-                        refined_inline++;
-                        if (cell >= 0) atomicAdd(hcol + ((uint32_t)cell << p.colshift), 1u);
-                    }
-                } else if (valid) {
-                    atomicAdd(hcol + ((uint32_t)cell << p.colshift), 1u);   // P4: private column, no conflict
+                // variable 1: t = S*g + O evaluated at t - tau (fa) and t + tau (fb), floored by a round-down add
+                float g;
+                if (KIND == CUTE_ANGULAR) {
+                    const float poly = fmaf(q[r], fmaf(q[r], c.c3, c.c2), c.c1);
+                    if (LOGB) g = fast_lg2(q[r] * poly);                 // log2(theta^2), theta^2 = q (1 + q/12 + ...)
+                    else { const float h = fast_sqrt(q[r]); g = h * poly; }   // theta = c (1 + q/24 + ...)
+                } else g = LOGB ? fast_lg2(q[r]) : fast_sqrt(q[r]);
+                const float fa = __fadd_rd(fmaf(g, c.S1, c.Oa1), CUTE_MAGIC_F);
+                const float fb = __fadd_rd(fmaf(g, c.S1, c.Ob1), CUTE_MAGIC_F);
+                uint32_t kb = (uint32_t)__float_as_int(fa);              // bin + MAGIC_BITS
+                bool sure = (fa == fb);
+                bool inr = (kb - (uint32_t)CUTE_MAGIC_BITS) < c.n1;
+                if (KIND == CUTE_RMU) {
+                    // mu = |s.l| / (|s||l|), s.l = |x_i|^2 - |x_j|^2 (hi/lo), |l|^2 = 2|x_i|^2 + 2|x_j|^2 - q
+                    const float pn = (ip.w[r] - pj.w) + (ip.lw[r] - nlo);
+                    const float m = fmaf(2.0f, ip.w[r] + pj.w, -q[r]);
+                    const float w = fast_rsqrt(q[r] * m);
+                    const float t2 = fmaf(fabsf(pn) * w, c.S2, c.O2);
+                    const float tau2 = fmaf(w, c.tauw2, c.tau2);
+                    const float f2a = __fadd_rd(t2 - tau2, CUTE_MAGIC_F), f2b = __fadd_rd(t2 + tau2, CUTE_MAGIC_F);
+                    const uint32_t k2 = (uint32_t)__float_as_int(f2a) - (uint32_t)CUTE_MAGIC_BITS;
+                    sure = sure && (f2a == f2b) && (q[r] > 0.f);
+                    inr = inr && (k2 < c.n2);
+                    kb = (kb - (uint32_t)CUTE_MAGIC_BITS) * c.n2 + k2 + (uint32_t)CUTE_MAGIC_BITS;
+                }
+                if (ALWAYS) { if (q[r] < c.q_hi) need |= 1u << r; }
+                else {
+                    // P4: private column, no conflict.  A pair that is out of range or queued for float64
+                    // increments the column's dump row instead: one SEL + one ATOMS, no branch.
+                    red_shared((sure && inr) ? hbase_s + (kb << (cs + 2u)) : dump_s);
+                    if (!sure && q[r] < c.q_hi) need |= 1u << r;
                 }
             }
+            if (need) push_refine<KIND>(p, s, need, ip.idx0, j0 + jj, hoff, refined_inline);
         }
     }
 }
@@ -394,15 +426,16 @@ __device__ __forceinline__ void expand_row(const PairParams &p, const Chunk &ch,
 }
 
 // ------------------------------------------------------------------------------- the kernel
-template <int KIND, bool MINIMG, bool LOGB>
+template <int KIND, bool MINIMG, bool LOGB, bool COLS32, bool ALWAYS>
 __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_constant__ PairParams p)
 {
+    const Consts cst = load_consts(p);
     constexpr bool NEEDLO = (KIND == CUTE_ANGULAR || KIND == CUTE_RMU);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const WarpSmem s = carve<NEEDLO>(smem_raw + (size_t)warp * p.smem_per_warp);
 
-    for (uint32_t k = lane; k < ((uint32_t)p.nhist << p.colshift); k += 32) s.hist[k] = 0;
+    for (uint32_t k = lane; k < ((uint32_t)(p.nhist + 1) << p.colshift); k += 32) s.hist[k] = 0;
     if (lane == 0) {
         for (int k = 0; k < kStages; k++) mbar_init(s.bar[k], 1);
         *s.rq_count = 0;
@@ -430,11 +463,11 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
 
         // ---- i-points into registers
         IPoints ip;
+        ip.idx0 = ch.i_begin + lane;
         float bx[R], by[R], bz[R];
 #pragma unroll
         for (int r = 0; r < R; r++) {
             const uint32_t k = lane + 32 * r;
-            ip.idx[r] = ch.i_begin + k;
             float4 h = make_float4(kSentinel, kSentinel, kSentinel, 0.f), l = make_float4(0.f, 0.f, 0.f, 0.f);
             if (k < ch.i_count) {
                 h = g1.hi[ch.i_begin + k];
@@ -510,16 +543,16 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
                 }
                 const float4 *th = s.thi + stage * kTile, *tl = s.tlo + stage * kTile;
                 if (seg_mask && t_j0 <= i_last) {
-                    compute_tile<KIND, MINIMG, LOGB, true>(p, s, ip, th, tl, t_cnt, t_j0, lane, refined_inline);
+                    compute_tile<KIND, MINIMG, LOGB, true, COLS32, ALWAYS>(p, s, cst, ip, th, tl, t_cnt, t_j0, lane, refined_inline);
 #pragma unroll
                     for (int r = 0; r < R; r++) {
-                        if (ip.idx[r] <= i_last) {
-                            const uint32_t b = max(t_j0, ip.idx[r] + 1), e = t_j0 + t_cnt;
+                        if (ip.idx0 + 32u * r <= i_last) {
+                            const uint32_t b = max(t_j0, ip.idx0 + 32u * r + 1), e = t_j0 + t_cnt;
                             if (b < e) evaluated += e - b;
                         }
                     }
                 } else {
-                    compute_tile<KIND, MINIMG, LOGB, false>(p, s, ip, th, tl, t_cnt, t_j0, lane, refined_inline);
+                    compute_tile<KIND, MINIMG, LOGB, false, COLS32, ALWAYS>(p, s, cst, ip, th, tl, t_cnt, t_j0, lane, refined_inline);
                     if (lane == 0) evaluated += (unsigned long long)ch.i_count * t_cnt;
                 }
                 __syncwarp();
@@ -575,15 +608,25 @@ int plan_pair_kernel(PairParams &p, int want_warps, int want_cols)
     return -1;
 }
 
+template <int KIND, bool MINIMG, bool LOGB, bool COLS32, bool ALWAYS>
+static cudaError_t launch_k(const PairParams &p, int blocks, cudaStream_t s)
+{
+    const size_t smem = (size_t)p.smem_per_warp * p.warps;
+    cudaError_t e = cudaFuncSetAttribute(pair_kernel<KIND, MINIMG, LOGB, COLS32, ALWAYS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    pair_kernel<KIND, MINIMG, LOGB, COLS32, ALWAYS><<<blocks, 32 * p.warps, smem, s>>>(p);
+    note_launches(1);
+    return cudaGetLastError();
+}
+
 template <int KIND, bool MINIMG, bool LOGB>
 static cudaError_t launch_t(const PairParams &p, int blocks, cudaStream_t s)
 {
-    const size_t smem = (size_t)p.smem_per_warp * p.warps;
-    cudaError_t e = cudaFuncSetAttribute(pair_kernel<KIND, MINIMG, LOGB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    pair_kernel<KIND, MINIMG, LOGB><<<blocks, 32 * p.warps, smem, s>>>(p);
-    note_launches(1);
-    return cudaGetLastError();
+    // the float64-everything variant (RADIAL, force_refine) is not performance critical: one column layout
+    if (p.always_refine) return launch_k<KIND, MINIMG, LOGB, false, true>(p, blocks, s);
+    if (KIND == CUTE_RADIAL) return cudaErrorInvalidValue;
+    return p.colshift == 5 ? launch_k<KIND, MINIMG, LOGB, true, false>(p, blocks, s)
+                           : launch_k<KIND, MINIMG, LOGB, false, false>(p, blocks, s);
 }
 
 cudaError_t launch_pair_kernel(const PairParams &p, int blocks, cudaStream_t s)
@@ -597,7 +640,7 @@ cudaError_t launch_pair_kernel(const PairParams &p, int blocks, cudaStream_t s)
     case CUTE_ANGULAR:
         return lg ? launch_t<CUTE_ANGULAR, false, true>(p, blocks, s) : launch_t<CUTE_ANGULAR, false, false>(p, blocks, s);
     case CUTE_RMU:
-        return lg ? launch_t<CUTE_RMU, false, true>(p, blocks, s) : launch_t<CUTE_RMU, false, false>(p, blocks, s);
+        return launch_t<CUTE_RMU, false, false>(p, blocks, s);
     case CUTE_RADIAL:
         return launch_t<CUTE_RADIAL, false, false>(p, blocks, s);
     }
