@@ -254,7 +254,7 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
                 double t = floor(g->spec.size[d] / (0.5 * spec->rmax) * (1.0 + 1e-12));
                 nc[d] = t < 1 ? 1 : (t > 1024 ? 1024 : (int)t);
                 if (spec->periodic) {   // nearest cell count with nc >= 2 ceil(rmax/a) + 1
-                    auto ok = [&](int n) { return n >= 1 && n >= 2 * (int)ceil(spec->rmax * n / g->spec.size[d] * (1.0 + 1e-12)) + 1; };
+                    auto ok = [&](int n) { return n >= 1 && n >= 2 * (int)ceil(spec->rmax * n / g->spec.size[d] * (1.0 - 1e-12)) + 1; };
                     int best = 0;
                     for (int n = nc[d]; n >= 3 && !best; n--) if (ok(n)) best = n;
                     for (int n = nc[d] + 1; n <= nc[d] + 64 && !best; n++) if (ok(n)) best = n;
@@ -275,7 +275,7 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
         }
         if (spec->periodic)
             for (int d = 0; d < 3; d++) {
-                int k = (int)ceil(spec->rmax / g->cell[d] * (1.0 + 1e-12));
+                int k = (int)ceil(spec->rmax / g->cell[d] * (1.0 - 1e-12));
                 if (nc[d] < 2 * k + 1) { delete g; return CUTE_ERR_UNSUPPORTED; }   // a cell would be met through two images
             }
     } else if (spec->mode == CUTE_GRID_SPHERE) {
@@ -578,9 +578,9 @@ int cute_count_pairs(int kind, const cute_grid *g1, const cute_grid *g2, const c
     if (opts && opts->force_refine) p.always_refine = 1;
     if (mode == CUTE_GRID_BOX3D) {
         const double rr = g1->spec.rmax;
-        p.kx = (int)ceil(rr / g1->cell[0] * (1.0 + 1e-12));    // k = ceil(Rmax/a), reading G3
-        p.ky = (int)ceil(rr / g1->cell[1] * (1.0 + 1e-12));
-        p.kz = (int)ceil(rr / g1->cell[2] * (1.0 + 1e-12));
+        p.kx = (int)ceil(rr / g1->cell[0] * (1.0 - 1e-12));    // k = ceil(Rmax/a), reading G3; a pair this rounding could miss has r within 1e-12 of Rmax
+        p.ky = (int)ceil(rr / g1->cell[1] * (1.0 - 1e-12));
+        p.kz = (int)ceil(rr / g1->cell[2] * (1.0 - 1e-12));
         if (!p.periodic) { p.kx = p.kx < p.g2.ncx ? p.kx : p.g2.ncx; p.ky = p.ky < p.g2.ncy ? p.ky : p.g2.ncy; p.kz = p.kz < p.g2.ncz ? p.kz : p.g2.ncz; }
         p.ax = (float)g1->cell[0]; p.ay = (float)g1->cell[1]; p.az = (float)g1->cell[2];
         p.rmax2 = (float)(rr * rr * 1.001);
