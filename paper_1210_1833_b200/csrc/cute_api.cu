@@ -39,6 +39,8 @@ struct Layout {
     int64_t max_cells, max_rows, max_chunks;
 };
 
+constexpr int64_t kOrderCellsMax = 65536;   // mode NONE: cells that only order the points (32^3 or 256^2)
+
 inline int64_t cell_cap(int64_t n) { return n * 2 > 4096 ? n * 2 : 4096; }
 
 Layout make_layout(int64_t n, int want_lo, int want_f64, int64_t max_cells, int64_t max_rows)
@@ -120,7 +122,7 @@ void wants(const cute_catalog *c, const cute_grid_spec *s, int *want_lo, int *wa
 
 void cell_bounds(const cute_catalog *c, const cute_grid_spec *s, int64_t *max_cells, int64_t *max_rows)
 {
-    if (s->mode == CUTE_GRID_NONE) { *max_cells = 1; *max_rows = 1; return; }
+    if (s->mode == CUTE_GRID_NONE) { *max_cells = kOrderCellsMax; *max_rows = 1; return; }   // ordering cells
     if (s->mode == CUTE_GRID_SPHERE) { *max_cells = (int64_t)s->ncell[0] * s->ncell[1]; *max_rows = s->ncell[1]; return; }
     if (s->ncell[0] > 0 && s->ncell[1] > 0 && s->ncell[2] > 0) {
         *max_cells = (int64_t)s->ncell[0] * s->ncell[1] * s->ncell[2];
@@ -289,6 +291,38 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     b.ncells = (int64_t)nc[0] * nc[1] * nc[2];
     b.nrows = (int64_t)nc[1] * nc[2];
     g->ncells = b.ncells; g->nrows = b.nrows;
+    if (spec->mode == CUTE_GRID_NONE && cat->n > 0) {
+        // Brute force evaluates every pair, in any order: sort the points by the cells of a coarse box (or
+        // pixel map) over the bounding box, ~48 points per cell, so that the 128 i-points of a warp and the
+        // j-points of a tile are neighbours in space and the in-range test is (nearly) uniform over the warp.
+        b.order_only = 1;
+        b.periodic = 0;
+        int m;
+        if (cat->coord == CUTE_COORD_XYZ) {
+            b.mode = CUTE_GRID_BOX3D;
+            m = (int)lround(cbrt((double)cat->n / 48.0));
+            m = m < 1 ? 1 : (m > 32 ? 32 : m);
+            for (int d = 0; d < 3; d++) {
+                const double ext = bbox[3 + d] - bbox[d];
+                const double pad = 1e-6 * (ext > 0 ? ext : 1.0) + 1e-9 * fmax(fabs(bbox[d]), fabs(bbox[3 + d]));
+                b.origin[d] = bbox[d] - pad; b.size[d] = ext + 2 * pad; b.nc[d] = m; b.inv_cell[d] = m / b.size[d];
+            }
+        } else {
+            b.mode = CUTE_GRID_SPHERE;
+            m = (int)lround(sqrt((double)cat->n / 48.0));
+            m = m < 1 ? 1 : (m > 256 ? 256 : m);
+            const double ext = fmin(360.0, (bbox[3] - bbox[0]) * (1.0 + 1e-9) + 1e-9);
+            b.origin[0] = ext < 360.0 ? bbox[0] - 0.5 * (ext - (bbox[3] - bbox[0])) : 0.0;
+            b.size[0] = ext;
+            const double u0 = fmax(-1.0, sin(fmax(-90.0, bbox[1]) * (kPi / 180.0)) - 1e-9);
+            const double u1 = fmin(1.0, sin(fmin(90.0, bbox[4]) * (kPi / 180.0)) + 1e-9);
+            b.origin[1] = u0; b.size[1] = fmax(u1 - u0, 1e-9);
+            b.nc[0] = m; b.nc[1] = m; b.nc[2] = 1;
+            b.inv_cell[0] = m / b.size[0]; b.inv_cell[1] = m / b.size[1];
+        }
+        b.ncells = (int64_t)b.nc[0] * b.nc[1] * b.nc[2];
+        b.nrows = 1;
+    }
     // magnitude bound
     double m = 0.0;
     if (cat->coord == CUTE_COORD_XYZ) for (int d = 0; d < 6; d++) m = fmax(m, fabs(bbox[d]));

@@ -112,6 +112,7 @@ struct BuildPlan {
     const void *c0, *c1, *c2;
     int64_t n;
     int coord, dtype, mode, periodic;
+    int order_only;    // mode NONE: the cells only ORDER the points (spatially coherent warps); one row, all pairs
     double origin[3], inv_cell[3], size[3];
     int nc[3];
     double thetamax;

@@ -238,7 +238,7 @@ __global__ void k_row_counts(BuildPlan b)
 {
     int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (r >= b.nrows) return;
-    uint32_t n = (b.mode == CUTE_GRID_NONE) ? (uint32_t)b.n
+    uint32_t n = (b.mode == CUTE_GRID_NONE || b.order_only) ? (uint32_t)b.n
                                               : b.cell_start[(r + 1) * b.nc[0]] - b.cell_start[r * b.nc[0]];
     b.row_nchunks[r] = (n + kChunk - 1) / kChunk;
 }
@@ -253,14 +253,15 @@ __global__ void k_chunks(BuildPlan b, uint32_t max_chunks)
     int64_t lo = 0, hi = b.nrows - 1;
     while (lo < hi) { int64_t m = (lo + hi + 1) >> 1; if (b.row_chunk_start[m] <= c) lo = m; else hi = m - 1; }
     uint32_t row = (uint32_t)lo, k = c - b.row_chunk_start[row];
-    uint32_t r0 = (b.mode == CUTE_GRID_NONE) ? 0u : b.cell_start[(int64_t)row * b.nc[0]];
-    uint32_t r1 = (b.mode == CUTE_GRID_NONE) ? (uint32_t)b.n : b.cell_start[((int64_t)row + 1) * b.nc[0]];
+    const bool one_row = (b.mode == CUTE_GRID_NONE || b.order_only);
+    uint32_t r0 = one_row ? 0u : b.cell_start[(int64_t)row * b.nc[0]];
+    uint32_t r1 = one_row ? (uint32_t)b.n : b.cell_start[((int64_t)row + 1) * b.nc[0]];
     Chunk ch;
     ch.i_begin = r0 + k * kChunk;
     ch.i_count = min((uint32_t)kChunk, r1 - ch.i_begin);
     ch.row = row;
     uint32_t cx0 = 0, cx1 = 0;
-    if (b.mode != CUTE_GRID_NONE) {
+    if (!one_row) {
         cx0 = b.cid_sorted[ch.i_begin] % (uint32_t)b.nc[0];
         cx1 = b.cid_sorted[ch.i_begin + ch.i_count - 1] % (uint32_t)b.nc[0];
     }
@@ -309,7 +310,7 @@ cudaError_t run_build(const BuildPlan &b, cudaStream_t s)
     if ((e = exclusive_scan(b.row_nchunks, b.nrows, b.row_chunk_start, b.scan_tmp, s)) != cudaSuccess) return e;
     uint32_t max_chunks = (uint32_t)(b.n / kChunk + b.nrows + 1);
     k_chunks<<<(max_chunks + T - 1) / T, T, 0, s>>>(b, max_chunks);
-    if (b.mode == CUTE_GRID_SPHERE) { k_sphere_rows<<<(b.nc[1] + T - 1) / T, T, 0, s>>>(b); note_launches(1); }
+    if (b.mode == CUTE_GRID_SPHERE && !b.order_only) { k_sphere_rows<<<(b.nc[1] + T - 1) / T, T, 0, s>>>(b); note_launches(1); }
     note_launches(2);   // k_row_counts, k_chunks
     return cudaGetLastError();
 }
