@@ -132,6 +132,7 @@ typedef struct cute_grid_info {
     int mode, periodic, kind_coord, dtype, has_lo, has_f64;
     int ncell[3];
     double origin[3], cell[3];
+    double size[3];           /* resolved box: pass origin, size, ncell to the second grid of a cross-correlation */
     int64_t ncells, nrows, nchunks;
     const void *d_hi;         /* float4[n]   cell-sorted (x,y,z,w)                */
     const void *d_lo;         /* float4[n]   low parts (or NULL)                  */

@@ -48,7 +48,7 @@ class cute_count_opts(C.Structure):
 class cute_grid_info(C.Structure):
     _fields_ = [("struct_size", C.c_size_t), ("n", C.c_int64), ("mode", C.c_int), ("periodic", C.c_int),
                 ("kind_coord", C.c_int), ("dtype", C.c_int), ("has_lo", C.c_int), ("has_f64", C.c_int),
-                ("ncell", C.c_int * 3), ("origin", C.c_double * 3), ("cell", C.c_double * 3),
+                ("ncell", C.c_int * 3), ("origin", C.c_double * 3), ("cell", C.c_double * 3), ("size", C.c_double * 3),
                 ("ncells", C.c_int64), ("nrows", C.c_int64), ("nchunks", C.c_int64),
                 ("d_hi", C.c_void_p), ("d_lo", C.c_void_p), ("d_perm", C.c_void_p),
                 ("d_cell_start", C.c_void_p), ("build_bytes", C.c_double)]

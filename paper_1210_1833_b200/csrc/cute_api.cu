@@ -252,8 +252,14 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
         int64_t cap = mc;
         for (int d = 0; d < 3; d++) {
             if (spec->ncell[d] > 0) nc[d] = spec->ncell[d];
-            else {   // cell side ~ rmax/2  =>  k = ceil(rmax/a) = 2 (periodic needs nc >= 2k+1)
-                double t = floor(g->spec.size[d] / (0.5 * spec->rmax) * (1.0 + 1e-12));
+            else {   // cell side ~ rmax/4  =>  k = ceil(rmax/a) = 4: with the corners of the 9^3 cube trimmed, ~45 % of
+                     // the evaluated pairs are in range (measured on C5: 1.35x faster than rmax/2); periodic needs nc >= 2k+1
+                // ... but not so small that a cell holds fewer than ~160 points on average: a 128-point work item
+                // should come from one or two cells, else its j-ranges widen again (measured on C3)
+                const double vol = g->spec.size[0] * g->spec.size[1] * g->spec.size[2];
+                const double a_dens = cat->n > 0 ? cbrt(160.0 * vol / (double)cat->n) : 0.0;
+                const double a_want = fmax(0.25 * spec->rmax, fmin(a_dens, 0.5 * spec->rmax));
+                double t = floor(g->spec.size[d] / a_want * (1.0 + 1e-12));
                 nc[d] = t < 1 ? 1 : (t > 1024 ? 1024 : (int)t);
                 if (spec->periodic) {   // nearest cell count with nc >= 2 ceil(rmax/a) + 1
                     auto ok = [&](int n) { return n >= 1 && n >= 2 * (int)ceil(spec->rmax * n / g->spec.size[d] * (1.0 - 1e-12)) + 1; };
@@ -360,7 +366,7 @@ int cute_grid_get_info(const cute_grid *g, cute_grid_info *info)
     if (!g || !info || info->struct_size != sizeof(cute_grid_info)) return CUTE_ERR_INVALID_ARG;
     info->n = g->view.n; info->mode = g->spec.mode; info->periodic = g->spec.periodic;
     info->kind_coord = g->coord; info->dtype = g->dtype; info->has_lo = g->has_lo; info->has_f64 = g->has_f64;
-    for (int d = 0; d < 3; d++) { info->ncell[d] = g->spec.ncell[d]; info->origin[d] = g->spec.origin[d]; info->cell[d] = g->cell[d]; }
+    for (int d = 0; d < 3; d++) { info->ncell[d] = g->spec.ncell[d]; info->origin[d] = g->spec.origin[d]; info->cell[d] = g->cell[d]; info->size[d] = g->spec.size[d]; }
     info->ncells = g->ncells; info->nrows = g->nrows; info->nchunks = g->view.nchunks;
     info->d_hi = g->view.hi; info->d_lo = g->view.lo; info->d_perm = g->d_perm; info->d_cell_start = g->view.cell_start;
     info->build_bytes = g->build_bytes;
@@ -618,6 +624,7 @@ int cute_count_pairs(int kind, const cute_grid *g1, const cute_grid *g2, const c
         if (!p.periodic) { p.kx = p.kx < p.g2.ncx ? p.kx : p.g2.ncx; p.ky = p.ky < p.g2.ncy ? p.ky : p.g2.ncy; p.kz = p.kz < p.g2.ncz ? p.kz : p.g2.ncz; }
         p.ax = (float)g1->cell[0]; p.ay = (float)g1->cell[1]; p.az = (float)g1->cell[2];
         p.rmax2 = (float)(rr * rr * 1.001);
+        p.ox = (float)g1->spec.origin[0]; p.inv_ax = (float)(1.0 / g1->cell[0]);
     }
     if (mode == CUTE_GRID_SPHERE) p.ring = g1->spec.size[0] >= 360.0 ? 1 : 0;
 

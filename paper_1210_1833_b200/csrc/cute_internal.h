@@ -86,6 +86,7 @@ struct PairParams {
     float Lf;
     int kx, ky, kz;
     float ax, ay, az;            // cell sizes
+    float ox, inv_ax;            // BOX3D: origin and 1/cell along x
     float rmax2;                 // row-pruning radius^2 (padded)
     int ring;                    // SPHERE: RA axis covers 360 deg (neighbour window wraps)
     // work

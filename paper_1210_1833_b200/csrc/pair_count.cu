@@ -281,6 +281,42 @@ __device__ __noinline__ void push_refine(const PairParams &p, const WarpSmem &s,
     }
 }
 
+struct BinOut { uint32_t kb; uint32_t unsure; bool inr; };   // kb = cell + MAGIC_BITS
+
+// P3: the float32 bin map of one pair.  t = S*g + O is evaluated at t - tau and t + tau and floored by a
+// round-down add of 1.5*2^23; `unsure` = floor(t+tau) - floor(t-tau) (+ the same for mu), 0 when the bin is certain.
+template <int KIND, bool LOGB>
+__device__ __forceinline__ BinOut bin_of(const Consts &c, float q, float wi, float lwi, float wj, float lwj)
+{
+    BinOut o;
+    float g;
+    if (KIND == CUTE_ANGULAR) {
+        const float poly = fmaf(q, fmaf(q, c.c3, c.c2), c.c1);
+        if (LOGB) g = fast_lg2(q * poly);                      // log2(theta^2), theta^2 = q (1 + q/12 + ...)
+        else { const float h = fast_sqrt(q); g = h * poly; }   // theta = c (1 + q/24 + ...)
+    } else g = LOGB ? fast_lg2(q) : fast_sqrt(q);
+    const float fa = __fadd_rd(fmaf(g, c.S1, c.Oa1), CUTE_MAGIC_F);
+    const float fb = __fadd_rd(fmaf(g, c.S1, c.Ob1), CUTE_MAGIC_F);
+    o.kb = __float_as_uint(fa);
+    o.unsure = __float_as_uint(fb) - __float_as_uint(fa);
+    o.inr = (o.kb - (uint32_t)CUTE_MAGIC_BITS) < c.n1;
+    if (KIND == CUTE_RMU) {
+        // mu = |s.l| / (|s||l|), s.l = |x_i|^2 - |x_j|^2 (hi/lo), |l|^2 = 2|x_i|^2 + 2|x_j|^2 - q
+        const float pn = (wi - wj) + (lwi - lwj);
+        const float m = fmaf(2.0f, wi + wj, -q);
+        const float w = fast_rsqrt(q * m);
+        const float t2 = fmaf(fabsf(pn) * w, c.S2, c.O2);
+        const float tau2 = fmaf(w, c.tauw2, c.tau2);
+        const float f2a = __fadd_rd(t2 - tau2, CUTE_MAGIC_F), f2b = __fadd_rd(t2 + tau2, CUTE_MAGIC_F);
+        const uint32_t k2 = __float_as_uint(f2a) - (uint32_t)CUTE_MAGIC_BITS;
+        // q = 0 or NaN/inf from the reciprocal square root: f2a == f2b cannot be trusted
+        o.unsure += (__float_as_uint(f2b) - __float_as_uint(f2a)) + ((q > 0.f && f2a == f2a && f2b == f2b) ? 0u : 1u);
+        o.inr = o.inr && (k2 < c.n2);
+        o.kb = (o.kb - (uint32_t)CUTE_MAGIC_BITS) * c.n2 + k2 + (uint32_t)CUTE_MAGIC_BITS;
+    }
+    return o;
+}
+
 // COLS32: one histogram column per lane (compile-time shift); ALWAYS: every candidate pair goes to float64
 template <int KIND, bool MINIMG, bool LOGB, bool MASK, bool COLS32, bool ALWAYS>
 __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem &s, const Consts &c, const IPoints &ip,
@@ -314,49 +350,38 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
         }
         const float qm = fminf(fminf(q[0], q[1]), fminf(q[2], q[3]));
         if (qm < c.q_hi) {
-            uint32_t need = 0;
             float nlo = 0.f;
             if (KIND == CUTE_RMU) nlo = tl[jj].w;
+            if (ALWAYS || KIND == CUTE_RADIAL) {
+                uint32_t need = 0;
 #pragma unroll
-            for (int r = 0; r < R; r++) {
-                if (KIND == CUTE_RADIAL) {
-                    if (q[r] < c.q_hi && fabsf(ip.w[r] - pj.w) < c.dz_hi) need |= 1u << r;
-                    continue;
+                for (int r = 0; r < R; r++) {
+                    bool in = q[r] < c.q_hi;
+                    if (KIND == CUTE_RADIAL) in = in && (fabsf(ip.w[r] - pj.w) < c.dz_hi);
+                    if (in) need |= 1u << r;
                 }
-                // variable 1: t = S*g + O evaluated at t - tau (fa) and t + tau (fb), floored by a round-down add
-                float g;
-                if (KIND == CUTE_ANGULAR) {
-                    const float poly = fmaf(q[r], fmaf(q[r], c.c3, c.c2), c.c1);
-                    if (LOGB) g = fast_lg2(q[r] * poly);                 // log2(theta^2), theta^2 = q (1 + q/12 + ...)
-                    else { const float h = fast_sqrt(q[r]); g = h * poly; }   // theta = c (1 + q/24 + ...)
-                } else g = LOGB ? fast_lg2(q[r]) : fast_sqrt(q[r]);
-                const float fa = __fadd_rd(fmaf(g, c.S1, c.Oa1), CUTE_MAGIC_F);
-                const float fb = __fadd_rd(fmaf(g, c.S1, c.Ob1), CUTE_MAGIC_F);
-                uint32_t kb = (uint32_t)__float_as_int(fa);              // bin + MAGIC_BITS
-                bool sure = (fa == fb);
-                bool inr = (kb - (uint32_t)CUTE_MAGIC_BITS) < c.n1;
-                if (KIND == CUTE_RMU) {
-                    // mu = |s.l| / (|s||l|), s.l = |x_i|^2 - |x_j|^2 (hi/lo), |l|^2 = 2|x_i|^2 + 2|x_j|^2 - q
-                    const float pn = (ip.w[r] - pj.w) + (ip.lw[r] - nlo);
-                    const float m = fmaf(2.0f, ip.w[r] + pj.w, -q[r]);
-                    const float w = fast_rsqrt(q[r] * m);
-                    const float t2 = fmaf(fabsf(pn) * w, c.S2, c.O2);
-                    const float tau2 = fmaf(w, c.tauw2, c.tau2);
-                    const float f2a = __fadd_rd(t2 - tau2, CUTE_MAGIC_F), f2b = __fadd_rd(t2 + tau2, CUTE_MAGIC_F);
-                    const uint32_t k2 = (uint32_t)__float_as_int(f2a) - (uint32_t)CUTE_MAGIC_BITS;
-                    sure = sure && (f2a == f2b) && (q[r] > 0.f);
-                    inr = inr && (k2 < c.n2);
-                    kb = (kb - (uint32_t)CUTE_MAGIC_BITS) * c.n2 + k2 + (uint32_t)CUTE_MAGIC_BITS;
+                if (need) push_refine<KIND>(p, s, need, ip.idx0, j0 + jj, hoff, refined_inline);
+            } else {
+                // acc = sum over the 4 pairs of floor(t+tau) - floor(t-tau) (>= 0): non-zero <=> some bin is not certain
+                uint32_t acc = 0;
+#pragma unroll
+                for (int r = 0; r < R; r++) {
+                    BinOut o = bin_of<KIND, LOGB>(c, q[r], ip.w[r], ip.lw[r], pj.w, nlo);
+                    acc += o.unsure;
+                    // P4: private column, no conflict.  A pair that is out of range or uncertain increments the
+                    // column's dump row instead: one SEL + one ATOMS, no branch.
+                    red_shared((o.unsure == 0u && o.inr) ? hbase_s + (o.kb << (cs + 2u)) : dump_s);
                 }
-                if (ALWAYS) { if (q[r] < c.q_hi) need |= 1u << r; }
-                else {
-                    // P4: private column, no conflict.  A pair that is out of range or queued for float64
-                    // increments the column's dump row instead: one SEL + one ATOMS, no branch.
-                    red_shared((sure && inr) ? hbase_s + (kb << (cs + 2u)) : dump_s);
-                    if (!sure && q[r] < c.q_hi) need |= 1u << r;
+                if (acc) {   // rare: find the uncertain pairs again and queue them for float64
+                    uint32_t need = 0;
+#pragma unroll
+                    for (int r = 0; r < R; r++) {
+                        BinOut o = bin_of<KIND, LOGB>(c, q[r], ip.w[r], ip.lw[r], pj.w, nlo);
+                        if (o.unsure && q[r] < c.q_hi) need |= 1u << r;
+                    }
+                    if (need) push_refine<KIND>(p, s, need, ip.idx0, j0 + jj, hoff, refined_inline);
                 }
             }
-            if (need) push_refine<KIND>(p, s, need, ip.idx0, j0 + jj, hoff, refined_inline);
         }
     }
 }
@@ -374,7 +399,8 @@ __device__ __forceinline__ float image_shift(uint32_t code, int axis, float L)
 // cell-sorted j array ("we only correlate C_i with the cells inside a cube of 2k+1 cells per side
 // around it", with k = ceil(Rmax/a) -- DESIGN.md reading G3; on the sphere the rows
 // and the RA window of the repaired Eq. 16).
-__device__ __forceinline__ void expand_row(const PairParams &p, const Chunk &ch, int nb, int nrows_nb, uint4 *out)
+__device__ __forceinline__ void expand_row(const PairParams &p, const Chunk &ch, float xmin, float xmax, int nb, int nrows_nb,
+                                           uint4 *out)
 {
     uint4 none = make_uint4(0u, 0u, 0u, 0u);
     out[0] = out[1] = out[2] = none;
@@ -386,6 +412,7 @@ __device__ __forceinline__ void expand_row(const PairParams &p, const Chunk &ch,
     int y, z = cz, kx = p.kx;
     uint32_t code = 0;
     bool same_row, wrapx;
+    int lo_x = -0x40000000, hi_x = 0x40000000;   // cells reached by [xmin - w, xmax + w] (BOX3D)
     if (p.mode == CUTE_GRID_SPHERE) {
         y = p.g1.row_ylo[cy] + nb;
         if (p.is_auto && y < cy) return;
@@ -399,6 +426,11 @@ __device__ __forceinline__ void expand_row(const PairParams &p, const Chunk &ch,
         // prune rows that cannot hold a pair within rmax
         const float my = (float)max(0, abs(dy) - 1) * p.ay, mz = (float)max(0, abs(dz) - 1) * p.az;
         if (my * my + mz * mz > p.rmax2) return;
+        // ... and trim the row's cells the same way: only x within w = sqrt(rmax^2 - my^2 - mz^2) of the chunk's
+        // own x-extent can hold a pair (rmax2 is padded by 0.1 %, far above the float32 rounding here)
+        const float w = sqrtf(p.rmax2 - (my * my + mz * mz));
+        lo_x = (int)floorf((xmin - w - p.ox) * p.inv_ax);
+        hi_x = (int)floorf((xmax + w - p.ox) * p.inv_ax);
         y = cy + dy; z = cz + dz;
         if (p.periodic) {
             if (y >= ncy) { y -= ncy; code |= 2u << 2; } else if (y < 0) { y += ncy; code |= 1u << 2; }
@@ -409,7 +441,7 @@ __device__ __forceinline__ void expand_row(const PairParams &p, const Chunk &ch,
     }
     const uint32_t rb = (uint32_t)(z * ncy + y) * (uint32_t)ncx;
     const uint32_t *cs = g.cell_start + rb;
-    int lo = cx0 - kx, hi = cx1 + kx;
+    int lo = max(cx0 - kx, lo_x), hi = min(cx1 + kx, hi_x);
     const bool self = p.is_auto && same_row;
     if (p.mode == CUTE_GRID_SPHERE && wrapx && hi - lo + 1 >= ncx) { lo = 0; hi = ncx - 1; wrapx = false; }
     const int a0 = max(lo, 0), a1 = min(hi, ncx - 1);
@@ -477,6 +509,16 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
             ip.lx[r] = l.x; ip.ly[r] = l.y; ip.lz[r] = l.z; ip.lw[r] = l.w;
         }
 
+        // x-extent of the chunk (the j-ranges are trimmed to it)
+        float xmin = 3.0e38f, xmax = -3.0e38f;
+#pragma unroll
+        for (int r = 0; r < R; r++)
+            if ((uint32_t)(lane + 32 * r) < ch.i_count) { xmin = fminf(xmin, bx[r]); xmax = fmaxf(xmax, bx[r]); }
+        for (int o = 16; o; o >>= 1) {
+            xmin = fminf(xmin, __shfl_xor_sync(0xffffffffu, xmin, o));
+            xmax = fmaxf(xmax, __shfl_xor_sync(0xffffffffu, xmax, o));
+        }
+
         // ---- neighbour rows, 32 at a time
         int nrows_nb = 1;
         if (p.mode == CUTE_GRID_BOX3D) nrows_nb = (2 * p.ky + 1) * (2 * p.kz + 1);
@@ -494,7 +536,7 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
                 if (lane == 0) s.segs[0] = make_uint4(jb, max(jb, je), code, 0u);
                 nslots = 1;
             } else {
-                expand_row(p, ch, nb0 + lane, nrows_nb, s.segs + 3 * lane);
+                expand_row(p, ch, xmin, xmax, nb0 + lane, nrows_nb, s.segs + 3 * lane);
                 nslots = 3 * min(kSegBatch, nrows_nb - nb0);
             }
             __syncwarp();

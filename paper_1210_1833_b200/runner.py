@@ -52,6 +52,13 @@ class Job:
             self.g_data.free()
         self.g_data = api.cute_make_grid(self.d_data, self.coord, self.spec, workspace=getattr(self, "_ws_d", None))
         self._ws_d = self.g_data.workspace
+        if self.d_rand is not None and self.spec.mode == api.GRID_BOX3D:
+            # the two grids of a cross-correlation must carry one spec: hand the second build the cell counts
+            # (and box) the library resolved for the first
+            inf = self.g_data.info()
+            self.spec = api.grid_spec("box3d", periodic=bool(self.spec.periodic), origin=tuple(inf.origin),
+                                      size=tuple(inf.size), ncell=tuple(inf.ncell),
+                                      rmax=self.spec.rmax, kind_mask=self.spec.kind_mask)
         if self.d_rand is not None:
             if self.g_rand is not None:
                 self.g_rand.free()
