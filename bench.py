@@ -35,6 +35,9 @@ if ROOT not in sys.path:
 METRIC = "pairs/sec (1e9) counted into bins on 1 B200; % of pair-kernel roofline"
 UNIT = "1e9 pairs/s"
 SM_COUNT, LANES_PER_SM, SM_MAX_MHZ = 148, 128, 1965.0
+# dram__bytes_read.sum + dram__bytes_write.sum per pair-kernel launch from the committed `ncu --set full` capture
+# (profiles/r01_pair_kernel_c2.md: 11.3 MB DD, 33.8 MB DR; RR as DR), averaged over the 3 launches of a C2 step
+NCU_TRAFFIC_BYTES = {2: (11.29e6 + 33.82e6 + 33.82e6) / 3.0}
 
 
 # ------------------------------------------------------------------------------- sharding (host logic)
@@ -173,6 +176,21 @@ ALG_INSTR = {
 }
 
 
+def build_report(job, build_ms):
+    """The cell-list build (G0-G4) against the HBM roofline: algorithmic bytes / CUDA-event time of
+    cute_make_grid for all catalogues of the step (includes its host read-backs)."""
+    peak, src = 6650.0, "fallback (B200_PROFILING.md)"
+    try:
+        peak, src = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        pass
+    nbytes = job.g_data.info().build_bytes + (job.g_rand.info().build_bytes if job.g_rand is not None else 0.0)
+    ms = float(np.mean(build_ms)) if build_ms else 0.0
+    gbs = nbytes / (ms * 1e-3) / 1e9 if ms > 0 else 0.0
+    return {"bound": "hbm", "ms": ms, "algorithmic_bytes": nbytes, "achieved": gbs, "peak": peak, "unit": "GB/s",
+            "frac": gbs / peak, "peak_source": src}
+
+
 def run_ours(args, w, cfg):
     import torch
     rank = int(os.environ.get("RANK", "0"))
@@ -198,8 +216,13 @@ def run_ours(args, w, cfg):
             dist.barrier()
         torch.cuda.synchronize()
 
+    build_ms = []
+
     def one_step(record):
+        b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        b0.record()
         job.build()                                           # G0-G4 for both catalogues
+        b1.record()
         evs = []
         for which in whichs:
             g1, g2 = job.grids(which)
@@ -213,7 +236,8 @@ def run_ours(args, w, cfg):
             else:
                 job.counter.hist.zero_()
             e1.record()
-            st = api.cute_count_status(job.counter)
+            skipped = world > 1 and e <= b
+            st = api.cute_count_status(job.counter) if not skipped else {"evaluated": 0}
             acc[which].copy_(job.counter.hist)
             evs.append((e0, e1, st["evaluated"]))
         if dist is not None:                                  # the one exchange step: sum of partial histograms
@@ -229,6 +253,8 @@ def run_ours(args, w, cfg):
             xi, _ = api.cute_periodic_xi(hs["DD"], job.nd, w.bins["box_L"], w.bins)
         torch.cuda.synchronize()
         ev_pairs = 0
+        if record:
+            build_ms.append(b0.elapsed_time(b1))
         for (e0, e1, npairs), k in zip(evs, whichs):
             ev_pairs += npairs
             if record:
@@ -331,11 +357,14 @@ def run_ours(args, w, cfg):
            "dtype": "f32", "data": "synthetic", "config": cfg, "clocks": clocks, "gpu_launches": int(launches),
            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
            "roofline": {"bound": "alu", "kernel": "pair_kernel", "achieved": achieved, "peak": peak, "unit": "T lane-instr/s",
-                        "frac": achieved / peak, "traffic": None,
+                        "frac": achieved / peak,
+                        "traffic": NCU_TRAFFIC_BYTES.get(args.config) if args.scale == 1.0 and world == 1 else None,
+                        "traffic_unit": "bytes of DRAM per pair-kernel launch (ncu, profiles/r01_pair_kernel_c2.md)",
                         "peak_source": "148 SMs x 128 FP32 lanes x 1965 MHz (guide unit counts and max clock; DESIGN.md)",
                         "pair_kernel_share_of_step": kern_s / (total_ms * 1e-3),
                         "pairs_per_s_in_kernel": sum(pair_pairs) / kern_s if kern_s > 0 else 0.0,
                         "alg_instr_per_pair": [i_all, i_bin]},
+           "build": build_report(job, build_ms),
            "rates": {"evaluated_pairs_per_step": total_pairs / args.steps,
                      "binned_pairs_per_step": (sum(b for b in pair_binned if b is not None) / args.steps) if world == 1 else None}}
     if world == 1 and not args.no_cpu_baseline:

@@ -33,7 +33,7 @@ inline int sm_count()
 
 // ---- workspace layout of one grid -------------------------------------------------------------
 struct Layout {
-    size_t hi, lo, p64, perm, cid_sorted, cell_id, rank, count, cell_start, scan_tmp, row_nchunks, row_chunk_start, chunks,
+    size_t hi, lo, p64, perm, cell_id, rank, count, cell_start, scan_tmp, row_nchunks, row_chunk_start, chunks,
         row_kx, row_ylo, row_yhi, status, bbox, total;
     uint32_t n_pad;
     int64_t max_cells, max_rows, max_chunks;
@@ -58,7 +58,6 @@ Layout make_layout(int64_t n, int want_lo, int want_f64, int64_t max_cells, int6
     L.lo = want_lo ? take((size_t)L.n_pad * 16) : 0;
     L.p64 = want_f64 ? take((size_t)L.n_pad * 32) : 0;
     L.perm = take((size_t)L.n_pad * 4);
-    L.cid_sorted = take((size_t)L.n_pad * 4);
     L.cell_id = take((size_t)L.n_pad * 4);
     L.rank = take((size_t)L.n_pad * 4);
     L.count = take((size_t)(max_cells + 2) * 4);
@@ -170,8 +169,10 @@ int cute_catalog_bounds(const cute_catalog *cat, void *d_tmp, void *stream, doub
     b.n = cat->n; b.dtype = cat->dtype; b.bbox = (double *)d_tmp;
     cudaStream_t s = (cudaStream_t)stream;
     if (run_bbox(b, s) != cudaSuccess) return CUTE_ERR_CUDA;
-    if (cudaMemcpyAsync(bounds, d_tmp, 48, cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
+    long long raw[6];
+    if (cudaMemcpyAsync(raw, d_tmp, 48, cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
         return CUTE_ERR_CUDA;
+    decode_bbox(raw, bounds);
     for (int d = 0; d < 6; d++) if (!isfinite(bounds[d])) return CUTE_ERR_POINT_OUT_OF_BOX;
     return CUTE_OK;
 }
@@ -215,7 +216,7 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     b.want_lo = want_lo; b.want_f64 = want_f64; b.n_pad = L.n_pad;
     b.hi = (float4 *)(w + L.hi); b.lo = want_lo ? (float4 *)(w + L.lo) : nullptr;
     b.p64 = want_f64 ? (double *)(w + L.p64) : nullptr;
-    b.perm = (uint32_t *)(w + L.perm); b.cid_sorted = (uint32_t *)(w + L.cid_sorted);
+    b.perm = (uint32_t *)(w + L.perm);
     b.cell_id = (uint32_t *)(w + L.cell_id); b.rank = (uint32_t *)(w + L.rank);
     b.count = (uint32_t *)(w + L.count); b.cell_start = (uint32_t *)(w + L.cell_start);
     b.scan_tmp = (uint32_t *)(w + L.scan_tmp); b.row_nchunks = (uint32_t *)(w + L.row_nchunks);
@@ -226,12 +227,19 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
 
     // bounding box of the raw coordinates ("a box encompassing the whole catalog is
     // first determined"); also gives the magnitude bound of the float32 error model
+    // It is skipped when the caller gave the box (BOX3D with explicit sizes) or nothing needs it (RA/Dec pixels).
     double bbox[6] = {0, 0, 0, 0, 0, 0};
-    if (cat->n > 0) {
+    const bool box_given = spec->mode == CUTE_GRID_BOX3D && spec->size[0] > 0.0 && spec->size[1] > 0.0 && spec->size[2] > 0.0;
+    const bool need_bbox = cat->n > 0 && !box_given && !(spec->mode == CUTE_GRID_SPHERE && cat->coord == CUTE_COORD_RADEC);
+    if (need_bbox) {
+        long long raw[6];
         if (run_bbox(b, s) != cudaSuccess) return CUTE_ERR_CUDA;
-        if (cudaMemcpyAsync(bbox, b.bbox, sizeof(bbox), cudaMemcpyDeviceToHost, s) != cudaSuccess) return CUTE_ERR_CUDA;
+        if (cudaMemcpyAsync(raw, b.bbox, sizeof(raw), cudaMemcpyDeviceToHost, s) != cudaSuccess) return CUTE_ERR_CUDA;
         if (cudaStreamSynchronize(s) != cudaSuccess) return CUTE_ERR_CUDA;
+        decode_bbox(raw, bbox);
         for (int d = 0; d < 6; d++) if (!isfinite(bbox[d])) return CUTE_ERR_POINT_OUT_OF_BOX;
+    } else if (box_given) {
+        for (int d = 0; d < 3; d++) { bbox[d] = spec->origin[d]; bbox[3 + d] = spec->origin[d] + spec->size[d]; }
     }
 
     cute_grid *g = new (std::nothrow) cute_grid;
@@ -351,10 +359,10 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     v.ncx = nc[0]; v.ncy = nc[1]; v.ncz = nc[2];
     g->d_perm = b.perm;
     // algorithmic HBM bytes of the build: read the coordinates twice (cell id,
-    // scatter), write hi (+lo, +p64), perm, cell id cache (write+read), rank (write+read), counts/scan
+    // scatter), write hi (+lo, +p64) and perm, cell id cache and rank (write + read: 16 B), counts/scan
     const double in_b = (cat->dtype == CUTE_F64 ? 8.0 : 4.0) * (cat->coord == CUTE_COORD_RADEC ? 2 : 3);
-    g->build_bytes = (double)cat->n * (2 * in_b + 16 + (want_lo ? 16 : 0) + (want_f64 ? 32 : 0) + 4 + 4 +
-                                       (spec->mode != CUTE_GRID_NONE ? 16 : 0)) + (double)b.ncells * 12;
+    g->build_bytes = (double)cat->n * (2 * in_b + 16 + (want_lo ? 16 : 0) + (want_f64 ? 32 : 0) + 4 +
+                                       16) + (double)b.ncells * 12;
     *out = g;
     return CUTE_OK;
 }

@@ -122,14 +122,15 @@ struct BuildPlan {
     float4 *hi, *lo;
     double *p64;
     uint32_t n_pad;
-    uint32_t *perm, *cid_sorted, *cell_id, *rank, *count, *cell_start, *scan_tmp, *row_nchunks, *row_chunk_start;
+    uint32_t *perm, *cell_id, *rank, *count, *cell_start, *scan_tmp, *row_nchunks, *row_chunk_start;
     Chunk *chunks;
     int *row_kx, *row_ylo, *row_yhi;
     uint32_t *status;  // [0] err, [1] nchunks
     double *bbox;      // [6] min xyz, max xyz
     int64_t ncells, nrows;
 };
-cudaError_t run_bbox(const BuildPlan &b, cudaStream_t s);
+cudaError_t run_bbox(const BuildPlan &b, cudaStream_t s);       // leaves 6 order-preserving int64 images in b.bbox
+void decode_bbox(const long long raw[6], double out[6]);
 cudaError_t run_build(const BuildPlan &b, cudaStream_t s);
 
 } // namespace cute

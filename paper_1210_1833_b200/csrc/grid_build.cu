@@ -6,6 +6,7 @@
 // HBM-bound, O(N).
 #include "cute_internal.h"
 #include <math.h>
+#include <string.h>
 
 namespace cute {
 
@@ -53,33 +54,28 @@ __global__ void k_bbox(BuildPlan b)
     }
 }
 
-__global__ void k_bbox_init(double *bbox)
+// The device holds the box as order-preserving int64 images of the doubles; decode on the host.
+void decode_bbox(const long long raw[6], double out[6])
 {
-    long long *p = reinterpret_cast<long long *>(bbox);
-    if (threadIdx.x < 3) p[threadIdx.x] = 0x7fffffffffffffffll;
-    else if (threadIdx.x < 6) p[threadIdx.x] = (long long)0x8000000000000000ull + 1;
-}
-
-__global__ void k_bbox_decode(double *bbox)
-{
-    long long *p = reinterpret_cast<long long *>(bbox);
-    if (threadIdx.x < 6) {
-        long long v = p[threadIdx.x];
+    for (int d = 0; d < 6; d++) {
+        long long v = raw[d];
         v = v < 0 ? (long long)(0x8000000000000000ull) - v : v;
-        bbox[threadIdx.x] = __longlong_as_double(v);
+        memcpy(&out[d], &v, 8);
     }
 }
 
 cudaError_t run_bbox(const BuildPlan &b, cudaStream_t s)
 {
-    k_bbox_init<<<1, 32, 0, s>>>(b.bbox);
+    // minima start at 0x7f7f... (a huge positive image), maxima at 0x8080... (a huge negative one)
+    cudaError_t e;
+    if ((e = cudaMemsetAsync(b.bbox, 0x7f, 24, s)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(reinterpret_cast<char *>(b.bbox) + 24, 0x80, 24, s)) != cudaSuccess) return e;
     if (b.n > 0) {
         int blocks = (int)((b.n + 255) / 256);
         if (blocks > 148 * 8) blocks = 148 * 8;
         k_bbox<<<blocks, 256, 0, s>>>(b);
+        note_launches(1);
     }
-    k_bbox_decode<<<1, 32, 0, s>>>(b.bbox);
-    note_launches(b.n > 0 ? 3 : 2);
     return cudaGetLastError();
 }
 
@@ -230,7 +226,6 @@ __global__ void k_scatter(BuildPlan b)
     if (b.want_lo) b.lo[slot] = make_float4(l[0], l[1], l[2], l[3]);
     if (b.want_f64) for (int d = 0; d < 4; d++) b.p64[(size_t)d * b.n_pad + slot] = v[d];
     b.perm[slot] = (uint32_t)i;
-    b.cid_sorted[slot] = id;
 }
 
 // ---- G4: chunk table ---------------------------------------------------------------------------
@@ -262,8 +257,15 @@ __global__ void k_chunks(BuildPlan b, uint32_t max_chunks)
     ch.row = row;
     uint32_t cx0 = 0, cx1 = 0;
     if (!one_row) {
-        cx0 = b.cid_sorted[ch.i_begin] % (uint32_t)b.nc[0];
-        cx1 = b.cid_sorted[ch.i_begin + ch.i_count - 1] % (uint32_t)b.nc[0];
+        // cell (along x) of a sorted index = last cell of the row whose start is <= the index
+        const uint32_t *cs = b.cell_start + (int64_t)row * b.nc[0];
+        auto cell_of_index = [&](uint32_t idx) {
+            uint32_t lo = 0, hi = (uint32_t)b.nc[0] - 1;
+            while (lo < hi) { uint32_t m = (lo + hi + 1) >> 1; if (cs[m] <= idx) lo = m; else hi = m - 1; }
+            return lo;
+        };
+        cx0 = cell_of_index(ch.i_begin);
+        cx1 = cell_of_index(ch.i_begin + ch.i_count - 1);
     }
     ch.cx01 = cx0 | (cx1 << 16);
     b.chunks[c] = ch;
