@@ -262,10 +262,10 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
             if (spec->ncell[d] > 0) nc[d] = spec->ncell[d];
             else {   // cell side ~ rmax/4  =>  k = ceil(rmax/a) = 4: with the corners of the 9^3 cube trimmed, ~45 % of
                      // the evaluated pairs are in range (measured on C5: 1.35x faster than rmax/2); periodic needs nc >= 2k+1
-                // ... but not so small that a cell holds fewer than ~160 points on average: a 128-point work item
+                // ... but not so small that a cell holds fewer than ~150 points on average: a 128-point work item
                 // should come from one or two cells, else its j-ranges widen again (measured on C3)
                 const double vol = g->spec.size[0] * g->spec.size[1] * g->spec.size[2];
-                const double a_dens = cat->n > 0 ? cbrt(160.0 * vol / (double)cat->n) : 0.0;
+                const double a_dens = cat->n > 0 ? cbrt(150.0 * vol / (double)cat->n) : 0.0;
                 const double a_want = fmax(0.25 * spec->rmax, fmin(a_dens, 0.5 * spec->rmax));
                 double t = floor(g->spec.size[d] / a_want * (1.0 + 1e-12));
                 nc[d] = t < 1 ? 1 : (t > 1024 ? 1024 : (int)t);

@@ -310,7 +310,8 @@ __device__ __forceinline__ BinOut bin_of(const Consts &c, float q, float wi, flo
         const float f2a = __fadd_rd(t2 - tau2, CUTE_MAGIC_F), f2b = __fadd_rd(t2 + tau2, CUTE_MAGIC_F);
         const uint32_t k2 = __float_as_uint(f2a) - (uint32_t)CUTE_MAGIC_BITS;
         // q = 0 or NaN/inf from the reciprocal square root: f2a == f2b cannot be trusted
-        o.unsure += (__float_as_uint(f2b) - __float_as_uint(f2a)) + ((q > 0.f && f2a == f2a && f2b == f2b) ? 0u : 1u);
+        // (clamped: tau2 grows without bound as r -> 0, and the caller keeps one byte per pair)
+        o.unsure += min((__float_as_uint(f2b) - __float_as_uint(f2a)) | ((q > 0.f && f2a == f2a && f2b == f2b) ? 0u : 1u), 15u);
         o.inr = o.inr && (k2 < c.n2);
         o.kb = (o.kb - (uint32_t)CUTE_MAGIC_BITS) * c.n2 + k2 + (uint32_t)CUTE_MAGIC_BITS;
     }
@@ -328,7 +329,7 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
     // bin k of column hoff lives at hbase[(k << cs)]; the magic-number bits are folded into the base
     const uint32_t dump_s = smem_u32(s.hist + (((uint32_t)p.nhist << cs) + hoff));
     const uint32_t hbase_s = smem_u32(s.hist + hoff) - ((uint32_t)CUTE_MAGIC_BITS << (cs + 2u));   // shared-space byte address
-#pragma unroll 2
+#pragma unroll (KIND == 2 ? 2 : 4)   /* 2 = CUTE_RMU: its bin path is long, 4 copies cost more than they hide */
     for (uint32_t jj = 0; jj < cnt; jj++) {
         const float4 pj = th[jj];
         float4 pl = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -362,23 +363,21 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
                 }
                 if (need) push_refine<KIND>(p, s, need, ip.idx0, j0 + jj, hoff, refined_inline);
             } else {
-                // acc = sum over the 4 pairs of floor(t+tau) - floor(t-tau) (>= 0): non-zero <=> some bin is not certain
+                // acc packs, one byte per pair, floor(t+tau) - floor(t-tau) (>= 0): non-zero <=> some bin is not certain
                 uint32_t acc = 0;
 #pragma unroll
                 for (int r = 0; r < R; r++) {
                     BinOut o = bin_of<KIND, LOGB>(c, q[r], ip.w[r], ip.lw[r], pj.w, nlo);
-                    acc += o.unsure;
+                    acc += o.unsure << (8 * r);   // one byte per pair (unsure <= 5)
                     // P4: private column, no conflict.  A pair that is out of range or uncertain increments the
                     // column's dump row instead: one SEL + one ATOMS, no branch.
                     red_shared((o.unsure == 0u && o.inr) ? hbase_s + (o.kb << (cs + 2u)) : dump_s);
                 }
-                if (acc) {   // rare: find the uncertain pairs again and queue them for float64
+                if (acc) {   // rare: queue the uncertain pairs for float64
                     uint32_t need = 0;
 #pragma unroll
-                    for (int r = 0; r < R; r++) {
-                        BinOut o = bin_of<KIND, LOGB>(c, q[r], ip.w[r], ip.lw[r], pj.w, nlo);
-                        if (o.unsure && q[r] < c.q_hi) need |= 1u << r;
-                    }
+                    for (int r = 0; r < R; r++)
+                        if (((acc >> (8 * r)) & 0xffu) && q[r] < c.q_hi) need |= 1u << r;
                     if (need) push_refine<KIND>(p, s, need, ip.idx0, j0 + jj, hoff, refined_inline);
                 }
             }
