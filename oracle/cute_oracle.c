@@ -25,6 +25,8 @@
  *   S4  self pairs skipped; distinct coincident points are a pair with r = 0;
  *   S5  mu uses the mid-point line of sight l = x_i + x_j (pinned by Eq. 9);
  *   S6  mu = |cos|;  mu >= 1 goes to the last mu bin when hi2 >= 1; r = 0 => mu := 0;
+ *   N1  (pi,sigma): pi = r mu with the mu of S5/S6, sigma = sqrt(max(0, r^2 - pi^2)) (Eq. 2); first
+ *       variable pi (major index), second sigma;
  *   S7  radial: zbar = (z_i+z_j)/2 (major index), dz = |z_i - z_j|;
  *   S8  radial aperture test is strict: theta < aperture;
  *   S12 the angular distance measure is theta itself, computed as
@@ -53,6 +55,7 @@
 #define ORC_MONOPOLE 1
 #define ORC_RMU 2
 #define ORC_RADIAL 3
+#define ORC_PISIGMA 4 /* xi(pi,sigma): v = (pi, sigma), pi = r mu, sigma = sqrt(r^2 - pi^2), Eq. 2 */
 
 #define ORC_OK 0
 #define ORC_EINVAL (-1)
@@ -204,6 +207,16 @@ static inline void pair_eval(acc_t *A, const cat_t *c1, int64_t i, const cat_t *
         if (mu > 1.0) mu = 1.0;
         v1 = r; v2 = mu;
     } break;
+    case ORC_PISIGMA: { /* Eq. 2: pi = r mu (along the mid-point line of sight), sigma = sqrt(r^2 - pi^2) */
+        double sx = c1->a[i] - c2->a[j], sy = c1->b[i] - c2->b[j], sz = c1->c[i] - c2->c[j];
+        double lx = c1->a[i] + c2->a[j], ly = c1->b[i] + c2->b[j], lz = c1->c[i] + c2->c[j];
+        double r = sqrt(sx * sx + sy * sy + sz * sz), l = sqrt(lx * lx + ly * ly + lz * lz);
+        double mu = 0.0;
+        if (r > 0.0 && l > 0.0) mu = fabs(sx * lx + sy * ly + sz * lz) / (r * l);
+        if (mu > 1.0) mu = 1.0;
+        double pi = r * mu, s2 = r * r - pi * pi;
+        v1 = pi; v2 = s2 > 0.0 ? sqrt(s2) : 0.0;
+    } break;
     default: { /* ORC_RADIAL */
         double th = theta_of(c1, i, c2, j);
         in_ap = th < A->aperture;
@@ -264,9 +277,9 @@ static void acc_free(acc_t *A) { free(A->hist); free(A->amb_cell); free(A->amb_e
 
 static int check_args(int kind, const orc_bins *b, int auto_)
 {
-    if (kind < 0 || kind > 3 || b->n1 < 1 || !(b->lo1 < b->hi1)) return ORC_EINVAL;
+    if (kind < 0 || kind > 4 || b->n1 < 1 || !(b->lo1 < b->hi1)) return ORC_EINVAL;
     if (b->log1 && !(b->lo1 > 0.0)) return ORC_EINVAL;
-    if ((kind == ORC_RMU || kind == ORC_RADIAL) && (b->n2 < 1 || !(b->lo2 < b->hi2))) return ORC_EINVAL;
+    if ((kind == ORC_RMU || kind == ORC_RADIAL || kind == ORC_PISIGMA) && (b->n2 < 1 || !(b->lo2 < b->hi2))) return ORC_EINVAL;
     if ((kind == ORC_ANGULAR || kind == ORC_MONOPOLE) && b->n2 != 0) return ORC_EINVAL;
     if (kind == ORC_RADIAL && !(b->aperture > 0.0)) return ORC_EINVAL;
     if (kind == ORC_MONOPOLE && b->box_L > 0.0 && b->hi1 > 0.5 * b->box_L) return ORC_EINVAL; /* S13 */
@@ -415,8 +428,9 @@ int orc_count(int kind, int mode,
     cells_t cells; int have_cells = 0;
     double rmax = 0.0;
     if (mode == 1) {
-        if (kind == ORC_MONOPOLE || kind == ORC_RMU) {
+        if (kind == ORC_MONOPOLE || kind == ORC_RMU || kind == ORC_PISIGMA) {
             rmax = bins->hi1 * (1.0 + 4.0 * ORC_BAND);
+            if (kind == ORC_PISIGMA) rmax = sqrt(bins->hi1 * bins->hi1 + bins->hi2 * bins->hi2) * (1.0 + 4.0 * ORC_BAND);
             if ((rc = build_cells3d(&cells, C2, rmax, G.L))) return rc;
             have_cells = 1;
             /* a periodic grid with fewer than 3 cells per side would meet a cell through two images */
@@ -575,6 +589,27 @@ int orc_periodic_rr(uint64_t n, double L, const orc_bins *b, double *rr)
     }
     free(e);
     return rc;
+}
+
+/* Multipoles of xi(r,mu), Eq. 3-4: xi(r,mu) = sum_l xi_l(r) P_l(mu), so
+ * xi_l(r) = (2l+1)/2 int_{-1}^{1} xi(r,mu) P_l(mu) dmu = (2l+1) int_0^1 ... for the even l of a pair-symmetric xi;
+ * the monopole is Eq. 4.  The integral over the mu bins is the mid-point rule (reading M1 in DESIGN.md).
+ * xi: [n_r][n_mu] over mu in [0,1]; out: [3][n_r] for l = 0, 2, 4. */
+int orc_multipoles(const double *xi, int n_r, int n_mu, double *out)
+{
+    if (n_r < 1 || n_mu < 1) return ORC_EINVAL;
+    for (int k = 0; k < n_r; k++) {
+        double a0 = 0.0, a2 = 0.0, a4 = 0.0;
+        for (int m = 0; m < n_mu; m++) {
+            double mu = ((double)m + 0.5) / (double)n_mu, x = xi[(size_t)k * n_mu + m];
+            double p2 = 0.5 * (3.0 * mu * mu - 1.0), p4 = (35.0 * mu * mu * mu * mu - 30.0 * mu * mu + 3.0) / 8.0;
+            a0 += x; a2 += x * p2; a4 += x * p4;
+        }
+        out[k] = a0 / (double)n_mu;
+        out[n_r + k] = 5.0 * a2 / (double)n_mu;
+        out[2 * n_r + k] = 9.0 * a4 / (double)n_mu;
+    }
+    return ORC_OK;
 }
 
 int orc_max_threads(void) { return omp_get_max_threads(); }

@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "cute_oracle.c")
 _LIB = os.path.join(_HERE, "libcute_oracle.so")
 
-KINDS = {"angular": 0, "monopole": 1, "rmu": 2, "radial": 3}
+KINDS = {"angular": 0, "monopole": 1, "rmu": 2, "radial": 3, "pisigma": 4}
 
 # float64, no FMA contraction, no fast-math: the arithmetic is the definition's
 CFLAGS = ["-O2", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC", "-std=c11"]
@@ -50,6 +50,7 @@ def _load():
         _lib.orc_landy_szalay.argtypes = [up, up, up, C.c_uint64, C.c_uint64, C.c_int, dp]
         _lib.orc_natural.argtypes = [up, up, C.c_uint64, C.c_uint64, C.c_int, dp]
         _lib.orc_periodic_rr.argtypes = [C.c_uint64, C.c_double, C.POINTER(_Bins), dp]
+        _lib.orc_multipoles.argtypes = [dp, C.c_int, C.c_int, dp]
     return _lib
 
 
@@ -143,6 +144,16 @@ def periodic_rr(n: int, L: float, bins: dict) -> np.ndarray:
     if rc:
         raise ValueError(f"orc_periodic_rr failed ({rc})")
     return rr
+
+
+def multipoles(xi_rmu, n_r: int, n_mu: int) -> np.ndarray:
+    """xi_0, xi_2, xi_4 of xi(r, mu) ([n_r][n_mu], mu in [0,1]); returns shape (3, n_r)."""
+    xi = np.ascontiguousarray(np.asarray(xi_rmu, dtype=np.float64)).ravel()
+    out = np.zeros((3, n_r))
+    rc = _load().orc_multipoles(_dp(xi), int(n_r), int(n_mu), _dp(out))
+    if rc:
+        raise ValueError(f"orc_multipoles failed ({rc})")
+    return out
 
 
 def parity_ok(gpu_hist, orc: dict):

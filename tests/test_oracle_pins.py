@@ -328,3 +328,63 @@ def test_radial_aperture_is_strict_and_flagged(oracle):
     assert pair(ap * 1.001)["hist"].sum() == 0
     r = pair(ap * (1 + 2.0 ** -22))
     assert r["amb_cell"][0] == 1 and r["amb_cell"][-1] == 1 and r["amb_e2"][-1] == 1
+
+
+# ------------------------------------------------------------------------------- N1: (pi, sigma) and multipoles
+def test_pisigma_fixture(oracle):
+    kind, bins, pts, pts2, expect = load_golden("pisigma_los.txt")
+    cat = tuple(np.array(c) for c in zip(*pts))
+    r = oracle.count(kind, cat, None, bins)
+    want = np.zeros(r["hist"].size, dtype=np.uint64)
+    for k, v in expect.items():
+        want[k] = v
+    assert np.array_equal(r["hist"], want)
+
+
+def test_pisigma_is_the_geometric_decomposition(oracle):
+    """V11: Eq. 2, pi = r mu and sigma = sqrt(r^2 - pi^2), must equal the geometric definition:
+    pi = |s . l^| (component of the separation along the unit mid-point vector) and sigma = |s - (s.l^) l^|
+    (the perpendicular component), computed here with numpy from scratch."""
+    rng = np.random.default_rng(11)
+    n = 400
+    x = rng.normal(size=(n, 3)) * 30.0 + np.array([0.0, 200.0, 900.0])
+    bins = dict(n1=13, lo1=0.0, hi1=60.0, n2=11, lo2=0.0, hi2=70.0)
+    r = oracle.count("pisigma", tuple(x.T.copy()), None, bins)
+    i, j = np.triu_indices(n, 1)
+    s = x[i] - x[j]
+    lv = x[i] + x[j]
+    lhat = lv / np.linalg.norm(lv, axis=1)[:, None]
+    par = np.einsum("ij,ij->i", s, lhat)
+    perp = np.linalg.norm(s - par[:, None] * lhat, axis=1)
+    h, _, _ = np.histogram2d(np.abs(par), perp, bins=[oracle.edges(bins, 0), oracle.edges(bins, 1)])
+    ok, msg = oracle.parity_ok(h.astype(np.int64).ravel(), r)
+    assert ok, msg
+    assert r["hist"].sum() > 1000
+    # bins that cover every separation: total = N(N-1)/2 (V4)
+    big = dict(n1=3, lo1=0.0, hi1=1e4, n2=3, lo2=0.0, hi2=1e4)
+    assert oracle.count("pisigma", tuple(x.T.copy()), None, big)["hist"].sum() == n * (n - 1) // 2
+
+
+def test_pisigma_celled_equals_plain(oracle):
+    rng = np.random.default_rng(12)
+    x = rng.random((3, 3000)) * 300.0 + 500.0
+    y = rng.random((3, 2000)) * 300.0 + 500.0
+    bins = dict(n1=8, lo1=0.0, hi1=40.0, n2=8, lo2=0.0, hi2=30.0)
+    for c2 in (None, tuple(y)):
+        a = oracle.count("pisigma", tuple(x), c2, bins, mode="plain")
+        b = oracle.count("pisigma", tuple(x), c2, bins, mode="celled")
+        assert np.array_equal(a["hist"], b["hist"]) and b["npairs"] < a["npairs"]
+
+
+def test_multipoles_closed_form(oracle):
+    """Eq. 3-4: xi(r,mu) = xi_0 + xi_2 P_2(mu) + xi_4 P_4(mu) must give back xi_0, xi_2, xi_4
+    (mid-point rule over 50 mu bins: error O(1/n_mu^2)); a mu-independent xi has only a monopole, exactly."""
+    n_r, n_mu = 7, 50
+    mu = (np.arange(n_mu) + 0.5) / n_mu
+    p2, p4 = 0.5 * (3 * mu**2 - 1), (35 * mu**4 - 30 * mu**2 + 3) / 8
+    a, b, c = np.linspace(1, 2, n_r), np.linspace(-0.5, 0.5, n_r), np.linspace(0.1, 0.3, n_r)
+    xi = a[:, None] + b[:, None] * p2[None, :] + c[:, None] * p4[None, :]
+    m = oracle.multipoles(xi, n_r, n_mu)
+    assert np.allclose(m[0], a, atol=2e-3) and np.allclose(m[1], b, atol=5e-3) and np.allclose(m[2], c, atol=1e-2)
+    m = oracle.multipoles(np.full((n_r, n_mu), 0.7), n_r, n_mu)
+    assert np.allclose(m[0], 0.7, atol=1e-14) and np.allclose(m[1], 0, atol=2e-3) and np.allclose(m[2], 0, atol=2e-3)
