@@ -171,6 +171,8 @@ ALG_INSTR = {
     ("monopole", "box3d"): (7.0, 9.0),    # 3 FADD + FMUL + 2 FFMA + range test
     ("rmu", "box3d"): (7.0, 21.0),        # + 3 FADD (s.l) + 2 (|l|^2) + FMUL + RSQ + FMUL + 2 FFMA + 2 FADD + 2 floor + cmp + range + IMAD
     ("rmu", "none"): (7.0, 21.0),
+    ("pisigma", "box3d"): (7.0, 24.0),
+    ("pisigma", "none"): (7.0, 24.0),
     ("radial", "sphere"): (8.0, 0.0),
     ("radial", "none"): (8.0, 0.0),
 }

@@ -50,9 +50,10 @@ extern "C" {
 #define CUTE_MONOPOLE 1 /* xi_0(r): v = r; periodic box: PAPER.md:245-249       */
 #define CUTE_RMU 2      /* xi(r,mu): v = (r, mu), mid-point line of sight */
 #define CUTE_RADIAL 3   /* xi_r(zbar,dz): pairs with theta < aperture, v = (zbar, dz) */
+#define CUTE_PISIGMA 4  /* xi(pi,sigma): v = (pi, sigma), pi = r mu, sigma = sqrt(r^2 - pi^2), Eq. 2 */
 
 /* catalogue coordinates */
-#define CUTE_COORD_XYZ 0     /* c0,c1,c2 = x,y,z (Mpc/h)              -> MONOPOLE, RMU */
+#define CUTE_COORD_XYZ 0     /* c0,c1,c2 = x,y,z (Mpc/h)              -> MONOPOLE, RMU, PISIGMA */
 #define CUTE_COORD_RADEC 1   /* c0,c1 = RA,Dec in degrees; c2 ignored -> ANGULAR       */
 #define CUTE_COORD_RADECZ 2  /* c0,c1 = RA,Dec in degrees; c2 = z     -> RADIAL (and ANGULAR) */
 #define CUTE_F32 0
@@ -97,10 +98,10 @@ typedef struct cute_grid_spec {
                    /* coordinates allow.  Lets the build skip arrays a kind does not read (the low parts). */
 } cute_grid_spec;
 
-/* Binning.  Variable 1: theta [rad] (ANGULAR), r (MONOPOLE, RMU), zbar (RADIAL); linear or, if
+/* Binning.  Variable 1: theta [rad] (ANGULAR), r (MONOPOLE, RMU), zbar (RADIAL), pi (PISIGMA); linear or, if
  * log1 != 0, logarithmic: e_k = lo1 (hi1/lo1)^(k/n1) ("logarithmic binning").
  * Variable 2 (n2 = 0 for 1-D kinds): mu in [lo2,hi2] (RMU; mu = 1 belongs to the last bin when
- * hi2 >= 1), dz (RADIAL); always linear.  aperture_rad: RADIAL only, strict theta < aperture.
+ * hi2 >= 1), dz (RADIAL), sigma (PISIGMA; a grid must then have rmax >= sqrt(hi1^2 + hi2^2)); always linear.  aperture_rad: RADIAL only, strict theta < aperture.
  * box_L > 0: periodic box of side L, minimum-image separations (MONOPOLE only; needs hi1 <= L/2). */
 typedef struct cute_bin_spec {
     size_t struct_size;
@@ -205,6 +206,9 @@ int cute_landy_szalay(const uint64_t *dd, const uint64_t *dr, const uint64_t *rr
                       int nbins, double *xi);
 /* Natural estimator, Eq. 14. */
 int cute_natural_estimator(const uint64_t *dd, const uint64_t *rr, uint64_t nd, uint64_t nr, int nbins, double *xi);
+/* Multipoles of xi(r,mu), Eqs. 3-4: xi_l(r) = (2l+1) int_0^1 xi(r,mu) P_l(mu) dmu for l = 0, 2, 4
+ * (mid-point rule over the mu bins, which must span [0,1]).  xi: HOST [n_r][n_mu]; out: HOST [3][n_r]. */
+int cute_multipoles(const double *xi, int n_r, int n_mu, double *out);
 /* Expected unordered pairs of a uniform periodic box, N(N-1)/2 * (4pi/3)(e_{k+1}^3-e_k^3)/L^3
  * (Eqs. 12-13, exact shell volume), and xi = DD/RR - 1. */
 int cute_periodic_rr(uint64_t n, double L, const cute_bin_spec *bins, double *rr);

@@ -14,8 +14,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcute_b200.so")
 
-ANGULAR, MONOPOLE, RMU, RADIAL = 0, 1, 2, 3
-KINDS = {"angular": ANGULAR, "monopole": MONOPOLE, "rmu": RMU, "radial": RADIAL}
+ANGULAR, MONOPOLE, RMU, RADIAL, PISIGMA = 0, 1, 2, 3, 4
+KINDS = {"angular": ANGULAR, "monopole": MONOPOLE, "rmu": RMU, "radial": RADIAL, "pisigma": PISIGMA}
 COORD_XYZ, COORD_RADEC, COORD_RADECZ = 0, 1, 2
 F32, F64 = 0, 1
 GRID_NONE, GRID_BOX3D, GRID_SPHERE = 0, 1, 2
@@ -58,7 +58,7 @@ class cute_grid_info(C.Structure):
 SYMBOLS = ["cute_version", "cute_strerror", "cute_launch_count", "cute_catalog_bounds", "cute_grid_workspace_bytes", "cute_make_grid", "cute_free_grid",
            "cute_grid_get_info", "cute_count_scratch_bytes", "cute_count_pairs", "cute_count_items",
            "cute_count_status", "cute_host_workspace_bytes", "cute_count_pairs_host", "cute_bin_edges",
-           "cute_landy_szalay", "cute_natural_estimator", "cute_periodic_rr", "cute_periodic_xi"]
+           "cute_landy_szalay", "cute_natural_estimator", "cute_multipoles", "cute_periodic_rr", "cute_periodic_xi"]
 
 
 def _load() -> C.CDLL:
@@ -89,6 +89,7 @@ def _load() -> C.CDLL:
     lib.cute_bin_edges.argtypes = [C.POINTER(cute_bin_spec), C.c_int, dp]
     lib.cute_landy_szalay.argtypes = [up, up, up, C.c_uint64, C.c_uint64, C.c_int, dp]
     lib.cute_natural_estimator.argtypes = [up, up, C.c_uint64, C.c_uint64, C.c_int, dp]
+    lib.cute_multipoles.argtypes = [dp, C.c_int, C.c_int, dp]
     lib.cute_periodic_rr.argtypes = [C.c_uint64, C.c_double, C.POINTER(cute_bin_spec), dp]
     lib.cute_periodic_xi.argtypes = [up, C.c_uint64, C.c_double, C.POINTER(cute_bin_spec), dp]
     return lib
@@ -326,6 +327,14 @@ def cute_natural_estimator(dd, rr, nd: int, nr: int):
     return xi, rc
 
 
+def cute_multipoles(xi_rmu, n_r: int, n_mu: int) -> np.ndarray:
+    """xi_0, xi_2, xi_4 (shape (3, n_r)) of xi(r, mu) given as [n_r][n_mu] over mu in [0,1] (Eqs. 3-4)."""
+    xi = np.ascontiguousarray(np.asarray(xi_rmu, dtype=np.float64)).ravel()
+    out = np.zeros((3, n_r))
+    _check(lib.cute_multipoles(_dp(xi), int(n_r), int(n_mu), _dp(out)), "cute_multipoles")
+    return out
+
+
 def cute_periodic_rr(n: int, L: float, bins: dict) -> np.ndarray:
     b = bin_spec(bins)
     rr = np.zeros(b.n1)
@@ -342,7 +351,7 @@ def cute_periodic_xi(dd, n: int, L: float, bins: dict):
 
 
 # ------------------------------------------------------------------------------- workload convenience
-COORD_OF_KIND = {"monopole": COORD_XYZ, "rmu": COORD_XYZ, "angular": COORD_RADEC, "radial": COORD_RADECZ}
+COORD_OF_KIND = {"monopole": COORD_XYZ, "rmu": COORD_XYZ, "pisigma": COORD_XYZ, "angular": COORD_RADEC, "radial": COORD_RADECZ}
 
 
 def auto_spec(kind: str, bins: dict, grid: dict, cats_dev, coord: int) -> cute_grid_spec:

@@ -111,7 +111,7 @@ void wants(const cute_catalog *c, const cute_grid_spec *s, int *want_lo, int *wa
 {
     int mask = s->kind_mask;
     if (c->coord == CUTE_COORD_XYZ) {
-        *want_lo = (mask == 0) || (mask & (1 << CUTE_RMU));
+        *want_lo = (mask == 0) || (mask & ((1 << CUTE_RMU) | (1 << CUTE_PISIGMA)));
         *want_f64 = c->dtype == CUTE_F64;
     } else {
         *want_lo = (mask == 0) || (mask & (1 << CUTE_ANGULAR));
@@ -389,10 +389,10 @@ namespace {
 int check_bins(int kind, const cute_bin_spec *b)
 {
     if (!b || b->struct_size != sizeof(cute_bin_spec)) return CUTE_ERR_INVALID_ARG;
-    if (kind < CUTE_ANGULAR || kind > CUTE_RADIAL) return CUTE_ERR_INVALID_ARG;
+    if (kind < CUTE_ANGULAR || kind > CUTE_PISIGMA) return CUTE_ERR_INVALID_ARG;
     if (b->n1 < 1 || b->n1 > 65536 || !(b->lo1 < b->hi1) || !(b->lo1 >= 0.0)) return CUTE_ERR_INVALID_ARG;
     if (b->log1 && !(b->lo1 > 0.0)) return CUTE_ERR_INVALID_ARG;
-    const bool two = (kind == CUTE_RMU || kind == CUTE_RADIAL);
+    const bool two = (kind == CUTE_RMU || kind == CUTE_RADIAL || kind == CUTE_PISIGMA);
     if (two && (b->n2 < 1 || b->n2 > 65536 || !(b->lo2 < b->hi2) || !(b->lo2 >= 0.0))) return CUTE_ERR_INVALID_ARG;
     if (!two && b->n2 != 0) return CUTE_ERR_INVALID_ARG;
     if ((int64_t)b->n1 * (b->n2 > 0 ? b->n2 : 1) > (1 << 20)) return CUTE_ERR_INVALID_ARG;
@@ -402,7 +402,7 @@ int check_bins(int kind, const cute_bin_spec *b)
         if (kind != CUTE_MONOPOLE || !(b->box_L > 0.0)) return CUTE_ERR_UNSUPPORTED;
         if (b->hi1 > 0.5 * b->box_L) return CUTE_ERR_INVALID_ARG;   // uniqueness of the minimum image (reading S13)
     }
-    if (kind == CUTE_RMU && b->log1) return CUTE_ERR_UNSUPPORTED;
+    if ((kind == CUTE_RMU || kind == CUTE_PISIGMA) && b->log1) return CUTE_ERR_UNSUPPORTED;
     return CUTE_OK;
 }
 
@@ -449,7 +449,31 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
     memset(&B, 0, sizeof(B));
     A.n = b->n1; B.n = b->n2;
     double tau1 = 0.0, rpad = 0.0;
-    if (kind == CUTE_MONOPOLE || kind == CUTE_RMU) {
+    if (kind == CUTE_PISIGMA) {
+        // pi = |s.l| / |l| with s.l = |x_i|^2 - |x_j|^2 from the hi/lo squares (no cancellation) and
+        // |l|^2 = 2|x_i|^2 + 2|x_j|^2 - q;  sigma = sqrt(q - pi^2).  Errors: q carries the float32 input rounding
+        // (e_r on r), pi only relative rounding, sigma inherits both divided by sigma: tau_2 = a + b / sigma.
+        const double e_d = (f64in ? 2.0 * kU * M : 0.0) + kU * (sqrt(b->hi1 * b->hi1 + b->hi2 * b->hi2) * 1.01);
+        const double e_r = sqrt(3.0) * e_d;
+        const double rmaxp = sqrt(b->hi1 * b->hi1 + b->hi2 * b->hi2);
+        const double inv1 = n1 / (b->hi1 - b->lo1), inv2 = (double)b->n2 / (b->hi2 - b->lo2);
+        A.S = (float)inv1; A.O = (float)(-b->lo1 * inv1);
+        B.S = (float)inv2; B.O = (float)(-b->lo2 * inv2);
+        // e_pi, the absolute error of pi, depends on the pair: |l|^2 = 2(|x_i|^2 + |x_j|^2) - q cancels when |l| << |x|
+        // (error 8u M^2 on |l|^2, i.e. pi * 4u M^2 / |l|^2 on pi), and s.l carries 2^-40 M^2 absolute (generous):
+        //   e_pi = Ep0 + Kp w1^2,  w1 = 1/|l|   (kernel: A.c2 + A.c1 w1^2, scaled by 1.25 tau_scale here)
+        const double sc = 1.25 * tau_scale;
+        const double Ep0 = sc * (16.0 * kU * rmaxp + ldexp(1.0, -40) * (M * M + 1.0));
+        const double Kp = sc * (4.0 * kU * (3.0 * M * M + 1.0) * rmaxp + ldexp(1.0, -40) * (M * M + 1.0));
+        A.c1 = (float)Kp; A.c2 = (float)Ep0;
+        tau1 = 4.0 * kU * (inv1 * b->hi1 + fabs((double)A.O) + n1 + 1.0);          // constant part; + S1 e_pi in the kernel
+        // d(sigma) = (r e_r + pi e_pi) / sigma:  tau_2 = B.tau + w2 (B.tau_w + A.c3 e_pi),  w2 = 1/sigma
+        B.tau = (float)(sc * (inv2 * 16.0 * kU * rmaxp + 4.0 * kU * (inv2 * b->hi2 + fabs((double)B.O) + b->n2 + 1.0)));
+        B.tau_w = (float)(sc * inv2 * rmaxp * e_r * 1.01);
+        A.c3 = (float)(inv2 * rmaxp * 1.01);
+        const double rpad = (rmaxp * (1.0 + 1e-4) + e_r) * (1.0 + 16.0 * kU);
+        p.q_hi = (float)(rpad * rpad * (1.0 + 8.0 * kU));
+    } else if (kind == CUTE_MONOPOLE || kind == CUTE_RMU) {
         // error of one separation component: input rounding, subtraction rounding, periodic image
         double e_d = (f64in ? 2.0 * kU * M : 0.0) + kU * (minimg ? b->box_L : b->hi1 * 1.01);
         if (p.periodic && !minimg) e_d += 2.0 * kU * 2.0 * b->box_L;
@@ -479,6 +503,9 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
             // dmu <= mu * (sqrt3 e_d / r) + 16u ;  1/r = w * |l| <= w * 2 sqrt3 M
             B.tau = (float)(1.25 * tau_scale * (inv2 * 16.0 * kU + 4.0 * kU * (inv2 + fabs((double)B.O) + b->n2 + 1.0)));
             B.tau_w = (float)(1.25 * tau_scale * inv2 * e_r * 2.0 * sqrt(3.0) * M);
+            // |l|^2 = 2(|x_i|^2 + |x_j|^2) - q cancels when |l| << |x| (a catalogue around the origin): its
+            // error 8u 3M^2 enters mu as mu * 4u 3M^2 / |l|^2, and 1/|l|^2 = w^2 q in the kernel
+            A.c1 = (float)(1.25 * tau_scale * inv2 * 4.0 * kU * (3.0 * M * M + 1.0));
         }
     } else {
         // unit vectors.  ANGULAR: hi/lo pairs, |dd| <= 3u|d| + sqrt3 2^-47 ; RADIAL: coarse test only.
@@ -600,11 +627,12 @@ int cute_count_pairs(int kind, const cute_grid *g1, const cute_grid *g2, const c
     const int mode = g1->spec.mode;
     // kind / coordinates / grid compatibility
     const bool xyz = g1->coord == CUTE_COORD_XYZ;
-    if ((kind == CUTE_MONOPOLE || kind == CUTE_RMU) != xyz) return CUTE_ERR_INVALID_ARG;
+    if ((kind == CUTE_MONOPOLE || kind == CUTE_RMU || kind == CUTE_PISIGMA) != xyz) return CUTE_ERR_INVALID_ARG;
     if (kind == CUTE_RADIAL && (g1->coord != CUTE_COORD_RADECZ || g2->coord != CUTE_COORD_RADECZ)) return CUTE_ERR_INVALID_ARG;
-    if ((kind == CUTE_ANGULAR || kind == CUTE_RMU) && (!g1->has_lo || !g2->has_lo)) return CUTE_ERR_INVALID_ARG;
-    if (kind == CUTE_RMU && mode == CUTE_GRID_BOX3D && g1->spec.periodic) return CUTE_ERR_UNSUPPORTED;
-    const double vmax = kind == CUTE_RADIAL ? bins->aperture_rad : bins->hi1;
+    if ((kind == CUTE_ANGULAR || kind == CUTE_RMU || kind == CUTE_PISIGMA) && (!g1->has_lo || !g2->has_lo)) return CUTE_ERR_INVALID_ARG;
+    if ((kind == CUTE_RMU || kind == CUTE_PISIGMA) && mode == CUTE_GRID_BOX3D && g1->spec.periodic) return CUTE_ERR_UNSUPPORTED;
+    const double vmax = kind == CUTE_RADIAL ? bins->aperture_rad
+                                           : (kind == CUTE_PISIGMA ? sqrt(bins->hi1 * bins->hi1 + bins->hi2 * bins->hi2) : bins->hi1);
     if (mode != CUTE_GRID_NONE && vmax > g1->spec.rmax * (1.0 + 1e-12)) return CUTE_ERR_INVALID_ARG;
     if (mode == CUTE_GRID_BOX3D && g1->spec.periodic) {
         if (kind != CUTE_MONOPOLE || bins->box_L != g1->spec.size[0]) return CUTE_ERR_INVALID_ARG;
@@ -829,6 +857,24 @@ int cute_natural_estimator(const uint64_t *dd, const uint64_t *rr, uint64_t nd, 
         xi[k] = wdd * (double)dd[k] / (double)rr[k] - 1.0;
     }
     return warn;
+}
+
+/* Multipoles, Eqs. 3-4; mid-point rule over the mu bins (reading M1) */
+int cute_multipoles(const double *xi, int n_r, int n_mu, double *out)
+{
+    if (!xi || !out || n_r < 1 || n_mu < 1) return CUTE_ERR_INVALID_ARG;
+    const double dmu = 1.0 / (double)n_mu;
+    for (int k = 0; k < n_r; k++) {
+        double s0 = 0.0, s2 = 0.0, s4 = 0.0;
+        for (int m = 0; m < n_mu; m++) {
+            const double mu = ((double)m + 0.5) * dmu, m2 = mu * mu, x = xi[(size_t)k * n_mu + m];
+            s0 += x;
+            s2 += x * (1.5 * m2 - 0.5);
+            s4 += x * (4.375 * m2 * m2 - 3.75 * m2 + 0.375);
+        }
+        out[k] = s0 * dmu; out[n_r + k] = 5.0 * s2 * dmu; out[2 * n_r + k] = 9.0 * s4 * dmu;
+    }
+    return CUTE_OK;
 }
 
 /* Periodic box (Eqs. 12-13, with the exact shell volume and N(N-1)/2 unordered pairs) */

@@ -140,7 +140,7 @@ __device__ __noinline__ int refine_cell(const PairParams &p, uint32_t i_idx, uin
             v1 = __dmul_rn(0.5, __dadd_rn(a[3], b[3]));
             v2 = fabs(__dsub_rn(a[3], b[3]));
         }
-    } else {   // RMU: mid-point line of sight l = x_i + x_j (Eq. 9)
+    } else {   // RMU, PISIGMA: mid-point line of sight l = x_i + x_j (Eq. 9)
         double lx = __dadd_rn(a[0], b[0]), ly = __dadd_rn(a[1], b[1]), lz = __dadd_rn(a[2], b[2]);
         double r = __dsqrt_rn(norm2_64(dx, dy, dz)), l = __dsqrt_rn(norm2_64(lx, ly, lz));
         double mu = 0.0;
@@ -150,6 +150,10 @@ __device__ __noinline__ int refine_cell(const PairParams &p, uint32_t i_idx, uin
         }
         if (mu > 1.0) mu = 1.0;
         v1 = r; v2 = mu;
+        if (KIND == CUTE_PISIGMA) {   // Eq. 2: pi = r mu, sigma = sqrt(r^2 - pi^2)
+            const double pi = __dmul_rn(r, mu), s2 = __dsub_rn(__dmul_rn(r, r), __dmul_rn(pi, pi));
+            v1 = pi; v2 = s2 > 0.0 ? __dsqrt_rn(s2) : 0.0;
+        }
     }
     int k1 = find_bin64(p.edges1, p.n1, p.lo1, p.hi1, p.logbins, 0, v1);
     if (k1 < 0) return -1;
@@ -249,6 +253,7 @@ struct IPoints {           // the R i-points of this lane (float32 fast path)
 struct Consts {            // loop constants held in registers (not re-read from the constant bank)
     float q_hi, dz_hi, Lf;
     float S1, Oa1, Ob1, c1, c2, c3;
+    float O1, tau1, tauw1;     // PISIGMA: the pi axis has a pair-dependent tau too
     float S2, O2, tau2, tauw2;
     uint32_t n1, n2;
 };
@@ -258,6 +263,7 @@ __device__ __forceinline__ Consts load_consts(const PairParams &p)
     Consts c;
     c.q_hi = p.q_hi; c.dz_hi = p.dz_hi; c.Lf = p.Lf;
     c.S1 = p.a1.S; c.Oa1 = p.a1.Oa; c.Ob1 = p.a1.Ob; c.c1 = p.a1.c1; c.c2 = p.a1.c2; c.c3 = p.a1.c3;
+    c.O1 = p.a1.O; c.tau1 = p.a1.tau; c.tauw1 = p.a1.tau_w;
     c.S2 = p.a2.S; c.O2 = p.a2.O; c.tau2 = p.a2.tau; c.tauw2 = p.a2.tau_w;
     c.n1 = (uint32_t)p.n1; c.n2 = (uint32_t)p.n2;
     return c;
@@ -289,6 +295,27 @@ template <int KIND, bool LOGB>
 __device__ __forceinline__ BinOut bin_of(const Consts &c, float q, float wi, float lwi, float wj, float lwj)
 {
     BinOut o;
+    if (KIND == CUTE_PISIGMA) {
+        // pi = |s.l| / |l| (s.l = |x_i|^2 - |x_j|^2 from the hi/lo squares, |l|^2 = 2|x_i|^2 + 2|x_j|^2 - q),
+        // sigma = sqrt(q - pi^2)  (Eq. 2); both taus depend on the pair (1/|l| and 1/sigma)
+        const float pn = (wi - wj) + (lwi - lwj);
+        const float m = fmaf(2.0f, wi + wj, -q);
+        const float w1 = fast_rsqrt(m);
+        const float pi = fabsf(pn) * w1;
+        const float epi = fmaf(w1 * w1, c.c1, c.c2);                   // absolute error bound of pi for this pair
+        const float t1 = fmaf(pi, c.S1, c.O1), tau1 = fmaf(epi, c.S1, c.tau1);
+        const float fa = __fadd_rd(t1 - tau1, CUTE_MAGIC_F), fb = __fadd_rd(t1 + tau1, CUTE_MAGIC_F);
+        const float s2 = fmaf(-pi, pi, q);
+        const float w2 = fast_rsqrt(s2);
+        const float t2 = fmaf(s2 * w2, c.S2, c.O2), tau2 = fmaf(w2, fmaf(epi, c.c3, c.tauw2), c.tau2);
+        const float f2a = __fadd_rd(t2 - tau2, CUTE_MAGIC_F), f2b = __fadd_rd(t2 + tau2, CUTE_MAGIC_F);
+        const uint32_t k1 = __float_as_uint(fa) - (uint32_t)CUTE_MAGIC_BITS, k2 = __float_as_uint(f2a) - (uint32_t)CUTE_MAGIC_BITS;
+        const bool finite = (fa == fa) && (fb == fb) && (f2a == f2a) && (f2b == f2b);   // sigma^2 <= 0, |l| = 0: NaN
+        o.unsure = min((__float_as_uint(fb) - __float_as_uint(fa)) | (__float_as_uint(f2b) - __float_as_uint(f2a)) | (finite ? 0u : 1u), 15u);
+        o.inr = (k1 < c.n1) && (k2 < c.n2);
+        o.kb = k1 * c.n2 + k2 + (uint32_t)CUTE_MAGIC_BITS;
+        return o;
+    }
     float g;
     if (KIND == CUTE_ANGULAR) {
         const float poly = fmaf(q, fmaf(q, c.c3, c.c2), c.c1);
@@ -306,7 +333,7 @@ __device__ __forceinline__ BinOut bin_of(const Consts &c, float q, float wi, flo
         const float m = fmaf(2.0f, wi + wj, -q);
         const float w = fast_rsqrt(q * m);
         const float t2 = fmaf(fabsf(pn) * w, c.S2, c.O2);
-        const float tau2 = fmaf(w, c.tauw2, c.tau2);
+        const float tau2 = fmaf(w * w * q, c.c1, fmaf(w, c.tauw2, c.tau2));   // a + b/(r|l|) + c/|l|^2
         const float f2a = __fadd_rd(t2 - tau2, CUTE_MAGIC_F), f2b = __fadd_rd(t2 + tau2, CUTE_MAGIC_F);
         const uint32_t k2 = __float_as_uint(f2a) - (uint32_t)CUTE_MAGIC_BITS;
         // q = 0 or NaN/inf from the reciprocal square root: f2a == f2b cannot be trusted
@@ -329,7 +356,7 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
     // bin k of column hoff lives at hbase[(k << cs)]; the magic-number bits are folded into the base
     const uint32_t dump_s = smem_u32(s.hist + (((uint32_t)p.nhist << cs) + hoff));
     const uint32_t hbase_s = smem_u32(s.hist + hoff) - ((uint32_t)CUTE_MAGIC_BITS << (cs + 2u));   // shared-space byte address
-#pragma unroll (KIND == 2 ? 2 : 4)   /* 2 = CUTE_RMU: its bin path is long, 4 copies cost more than they hide */
+#pragma unroll ((KIND == 2 || KIND == 4) ? 2 : 4)   /* RMU, PISIGMA: the bin path is long, 4 copies cost more than they hide */
     for (uint32_t jj = 0; jj < cnt; jj++) {
         const float4 pj = th[jj];
         float4 pl = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -352,7 +379,7 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
         const float qm = fminf(fminf(q[0], q[1]), fminf(q[2], q[3]));
         if (qm < c.q_hi) {
             float nlo = 0.f;
-            if (KIND == CUTE_RMU) nlo = tl[jj].w;
+            if (KIND == CUTE_RMU || KIND == CUTE_PISIGMA) nlo = tl[jj].w;
             if (ALWAYS || KIND == CUTE_RADIAL) {
                 uint32_t need = 0;
 #pragma unroll
@@ -461,7 +488,7 @@ template <int KIND, bool MINIMG, bool LOGB, bool COLS32, bool ALWAYS>
 __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_constant__ PairParams p)
 {
     const Consts cst = load_consts(p);
-    constexpr bool NEEDLO = (KIND == CUTE_ANGULAR || KIND == CUTE_RMU);
+    constexpr bool NEEDLO = (KIND == CUTE_ANGULAR || KIND == CUTE_RMU || KIND == CUTE_PISIGMA);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const WarpSmem s = carve<NEEDLO>(smem_raw + (size_t)warp * p.smem_per_warp);
@@ -634,7 +661,7 @@ int plan_pair_kernel(PairParams &p, int want_warps, int want_cols)
     // Warps hide the latency of the dependent MUFU/FFMA chains and ncu shows throughput growing with the warp
     // count up to 16, while the number of private histogram columns (32, 8, 1) makes no measurable difference
     // (ATOMS.POPC.INC merges lanes that hit one address): default = 8 columns, as many warps as fit.
-    const bool needlo = (p.kind == CUTE_ANGULAR || p.kind == CUTE_RMU);
+    const bool needlo = (p.kind == CUTE_ANGULAR || p.kind == CUTE_RMU || p.kind == CUTE_PISIGMA);
     const int clist[] = {3, 0, 5};
     for (int ci = 0; ci < 3; ci++) {
         if (want_cols > 0 && (1 << clist[ci]) != want_cols) continue;
@@ -685,6 +712,8 @@ cudaError_t launch_pair_kernel(const PairParams &p, int blocks, cudaStream_t s)
         return launch_t<CUTE_RMU, false, false>(p, blocks, s);
     case CUTE_RADIAL:
         return launch_t<CUTE_RADIAL, false, false>(p, blocks, s);
+    case CUTE_PISIGMA:
+        return launch_t<CUTE_PISIGMA, false, false>(p, blocks, s);
     }
     return cudaErrorInvalidValue;
 }

@@ -15,7 +15,7 @@ from conftest import load_golden
 pytestmark = pytest.mark.gpu
 
 GOLDEN = ["monopole_345.txt", "monopole_periodic.txt", "monopole_cross.txt", "angular_equator.txt",
-          "angular_log.txt", "rmu_345.txt", "rmu_los.txt", "radial_ladder.txt"]
+          "angular_log.txt", "rmu_345.txt", "rmu_los.txt", "radial_ladder.txt", "pisigma_los.txt"]
 
 
 @pytest.fixture(scope="module")
@@ -118,6 +118,31 @@ def test_c3_rmu_grid(rt, oracle, ncell):
     out_b, _ = _run(runner, w.kind, w.data, w.rand, w.bins, dict(mode="none"), which=("DD", "DR"))
     assert np.array_equal(out_b["DD"][0], out["DD"][0])
     assert np.array_equal(out_b["DR"][0], out["DR"][0])
+
+
+@pytest.mark.parametrize("grid", ["box3d", "none"])
+def test_pisigma_on_c3(rt, oracle, grid):
+    """xi(pi,sigma), Eq. 2 -- the variant the paper times (Table II) and plots (Fig. 6) -- on the C3 catalogues"""
+    api, runner, synth = rt
+    w = synth.workload(3, 0.02)
+    bins = dict(n1=32, lo1=0.0, hi1=80.0, log1=0, n2=32, lo2=0.0, hi2=80.0, aperture=0.0, box_L=0.0)
+    g = dict(mode="box3d", rmax=math.hypot(80.0, 80.0)) if grid == "box3d" else dict(mode="none")
+    out, job = _run(runner, "pisigma", w.data, w.rand, bins, g, which=("DD", "DR", "RR"))
+    _parity(oracle, out["DD"][0], "pisigma", w.data, None, bins, "celled")
+    _parity(oracle, out["DR"][0], "pisigma", w.data, w.rand, bins, "celled")
+    _parity(oracle, out["RR"][0], "pisigma", w.rand, None, bins, "celled")
+    out2, _ = _run(runner, "pisigma", w.data, w.rand, bins, g, dict(force_refine=1), which=("DR",))
+    assert np.array_equal(out2["DR"][0], out["DR"][0])
+    # pairs along the line of sight (sigma -> 0) and a catalogue through the origin (|l| -> 0) go through float64
+    rng = np.random.default_rng(4)
+    x = rng.normal(size=(3, 300)) * 20.0
+    x = np.concatenate([x, -x[:, :50], x[:, :50] * 1.01], axis=1)
+    b2 = dict(bins, hi1=30.0, hi2=30.0, n1=15, n2=15)
+    out3, _ = _run(runner, "pisigma", tuple(x), None, b2, dict(mode="none"))
+    _parity(oracle, out3["DD"][0], "pisigma", tuple(x), None, b2)
+    b3 = dict(n1=15, lo1=0.0, hi1=30.0, log1=0, n2=20, lo2=0.0, hi2=1.0, aperture=0.0, box_L=0.0)
+    out4, _ = _run(runner, "rmu", tuple(x), None, b3, dict(mode="none"))
+    _parity(oracle, out4["DD"][0], "rmu", tuple(x), None, b3)
 
 
 @pytest.mark.parametrize("pix", [2.0, 0.7])

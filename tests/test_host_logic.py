@@ -77,6 +77,16 @@ def test_estimators_equal_oracle(api, oracle):
     assert np.max(np.abs(xp)) < 0.03
 
 
+def test_multipoles_equal_oracle(api, oracle):
+    """Eqs. 3-4 on the host: library == oracle, and a pure quadrupole comes back"""
+    rng = np.random.default_rng(8)
+    xi = rng.normal(size=(40, 50))
+    assert np.allclose(api.cute_multipoles(xi, 40, 50), oracle.multipoles(xi, 40, 50), rtol=1e-12, atol=1e-14)
+    mu = (np.arange(50) + 0.5) / 50
+    m = api.cute_multipoles(np.tile(0.5 * (3 * mu**2 - 1), (3, 1)), 3, 50)
+    assert np.allclose(m[0], 0, atol=1e-3) and np.allclose(m[1], 1, atol=5e-3)
+
+
 def test_validation_without_gpu(api):
     """host-side argument checks return error codes (no exceptions, no abort) before anything touches the device"""
     lib = api.lib
