@@ -377,6 +377,8 @@ def auto_spec(kind: str, bins: dict, grid: dict, cats_dev, coord: int) -> cute_g
     ra_lo, ra_hi = bb[:, 0].min(), bb[:, 3].max()
     de_lo, de_hi = bb[:, 1].min(), bb[:, 4].max()
     dra = min(360.0, (ra_hi - ra_lo) * (1 + 1e-9) + 1e-9)
+    if dra > 180.0:                      # wide or seam-straddling footprint: pixels over the full ring (RA wraps)
+        dra = 360.0
     ra0 = ra_lo - 0.5 * (dra - (ra_hi - ra_lo)) if dra < 360.0 else 0.0
     u_lo = max(-1.0, np.sin(np.radians(de_lo)) - 1e-12)
     u_hi = min(1.0, np.sin(np.radians(de_hi)) + 1e-12)

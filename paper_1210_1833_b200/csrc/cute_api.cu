@@ -103,6 +103,15 @@ int check_grid_spec(const cute_catalog *c, const cute_grid_spec *s)
         if (s->origin[1] < -1.0 - 1e-12 || s->origin[1] + s->size[1] > 1.0 + 1e-12) return CUTE_ERR_INVALID_ARG;
         if (s->ncell[0] <= 0 || s->ncell[1] <= 0) return CUTE_ERR_INVALID_ARG;
         if (s->ncell[0] > 65535) return CUTE_ERR_INVALID_ARG;
+        if (s->size[0] < 360.0) {
+            // an RA span short of the full ring has no wrap-around neighbours: refuse spans so wide that two
+            // points could be within rmax of each other THROUGH the gap (the caller must use size[0] = 360)
+            const double umax = fmax(fabs(s->origin[1]), fabs(s->origin[1] + s->size[1]));
+            const double cosd = sqrt(fmax(0.0, 1.0 - umax * umax));
+            if (!(sin(fmin(s->rmax, 0.5 * kPi)) < cosd)) return CUTE_ERR_INVALID_ARG;   // cap reaches a pole
+            const double win = asin(sin(s->rmax) / cosd) * (180.0 / kPi);
+            if (360.0 - s->size[0] < win) return CUTE_ERR_INVALID_ARG;
+        }
     }
     return CUTE_OK;
 }

@@ -95,6 +95,42 @@ def test_c2_angular_sphere_grid_equals_brute(rt, oracle):
     _parity(oracle, out_g["DD"][0], w.kind, w.data, None, bins)
 
 
+def test_sphere_grid_full_sky_poles_and_seam(rt, oracle):
+    """Eq. 16 (repaired, G2) at its hard places: a full-sky catalogue (both poles, the RA = 0/360 seam) on
+    a ring of pixels, and a footprint that straddles the seam; grid == brute force == oracle"""
+    api, runner, synth = rt
+    rng = np.random.default_rng(21)
+    n = 20000
+    ra = rng.random(n) * 360.0
+    dec = np.degrees(np.arcsin(rng.random(n) * 2 - 1))
+    dec[:40] = 90.0 - rng.random(40) * 0.5          # a knot at the north pole
+    dec[40:80] = -90.0 + rng.random(40) * 0.5       # and one at the south pole
+    ra[80:200] = (359.7 + rng.random(120) * 0.6) % 360.0   # and one across the seam
+    bins = dict(n1=20, lo1=math.radians(0.05), hi1=math.radians(3.0), log1=1, n2=0, lo2=0.0, hi2=0.0, aperture=0.0, box_L=0.0)
+    for pix in (1.0, 0.4):
+        out_g, job = _run(runner, "angular", (ra, dec), None, bins, dict(mode="sphere", thetamax=bins["hi1"], pix=pix))
+        assert job.spec.size[0] == 360.0
+        out_b, _ = _run(runner, "angular", (ra, dec), None, bins, dict(mode="none"))
+        assert np.array_equal(out_g["DD"][0], out_b["DD"][0])
+        assert out_g["DD"][1]["evaluated"] < out_b["DD"][1]["evaluated"]
+    _parity(oracle, out_g["DD"][0], "angular", (ra, dec), None, bins)
+    # a narrow footprint across RA = 0 (given as 350..360 and 0..10), cross-correlated with randoms
+    m = 6000
+    ra1 = (350.0 + rng.random(m) * 20.0) % 360.0
+    dec1 = rng.random(m) * 10.0 - 60.0
+    ra2 = (350.0 + rng.random(m) * 20.0) % 360.0
+    dec2 = rng.random(m) * 10.0 - 60.0
+    out_g, job = _run(runner, "angular", (ra1, dec1), (ra2, dec2), bins, dict(mode="sphere", thetamax=bins["hi1"], pix=1.0), which=("DD", "DR"))
+    out_b, _ = _run(runner, "angular", (ra1, dec1), (ra2, dec2), bins, dict(mode="none"), which=("DD", "DR"))
+    assert np.array_equal(out_g["DD"][0], out_b["DD"][0]) and np.array_equal(out_g["DR"][0], out_b["DR"][0])
+    _parity(oracle, out_g["DR"][0], "angular", (ra1, dec1), (ra2, dec2), bins)
+    # a span just short of the ring is refused (points could be neighbours through the gap)
+    with pytest.raises(api.CuteError):
+        spec = api.grid_spec("sphere", origin=(0.0, -0.9, 0), size=(359.0, 0.2, 0), ncell=(100, 10, 1), rmax=bins["hi1"])
+        import torch
+        api.cute_make_grid([torch.from_numpy(ra1).cuda(), torch.from_numpy(dec1).cuda()], api.COORD_RADEC, spec)
+
+
 def test_angular_linear_wide(rt, oracle):
     """the paper's own angular binning: linear in theta up to 30 deg"""
     api, runner, synth = rt
@@ -291,3 +327,44 @@ def test_host_entry_point_and_estimators(rt, oracle):
     o1, j1 = _run(runner, w1.kind, w1.data, None, w1.bins, w1.grid)
     rr1 = api.cute_periodic_rr(j1.nd, w1.bins["box_L"], w1.bins)
     assert np.allclose(rr1, oracle.periodic_rr(j1.nd, w1.bins["box_L"], w1.bins), rtol=1e-13)
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_fuzz_box_grids(rt, oracle, seed):
+    """random small catalogues, boxes, cell counts, bins: periodic and open cell lists against the PLAIN oracle
+    (exercises wrap segments, chunks wider than a cell, empty cells, 1..3 cells per axis, ragged tiles)"""
+    api, runner, synth = rt
+    rng = np.random.default_rng(1000 + seed)
+    periodic = bool(seed % 2)
+    n1, n2 = int(rng.integers(1, 2500)), int(rng.integers(1, 2500))
+    L = float(rng.uniform(50.0, 200.0))
+    if periodic:
+        rmax = float(rng.uniform(0.03, 0.45)) * L
+        a = tuple(rng.random((3, n1)) * L)
+        b = tuple(rng.random((3, n2)) * L)
+        kind = "monopole"
+    else:
+        rmax = float(rng.uniform(0.05, 0.8)) * L
+        ext = rng.uniform(0.2, 1.0, 3) * L
+        off = rng.uniform(-500.0, 500.0, 3)
+        a = tuple((rng.random((3, n1)) * ext[:, None]) + off[:, None])
+        b = tuple((rng.random((3, n2)) * ext[:, None] * rng.uniform(0.5, 1.2)) + off[:, None])
+        kind = ("monopole", "rmu", "pisigma")[seed // 2 % 3]
+    log1 = int(kind == "monopole" and rng.random() < 0.4)
+    bins = dict(n1=int(rng.integers(3, 40)), lo1=(rmax * 0.01 if log1 else 0.0), hi1=rmax, log1=log1, n2=0, lo2=0.0, hi2=0.0,
+                aperture=0.0, box_L=L if periodic else 0.0)
+    grmax = rmax
+    if kind == "rmu":
+        bins.update(n2=int(rng.integers(2, 30)), hi2=1.0)
+    if kind == "pisigma":
+        bins.update(n2=int(rng.integers(2, 30)), hi2=rmax * float(rng.uniform(0.3, 1.0)))
+        grmax = math.hypot(bins["hi1"], bins["hi2"])
+    ncell = (0, 0, 0) if rng.random() < 0.4 else tuple(int(v) for v in rng.integers(1 if not periodic else 3, 14, 3))
+    grid = dict(mode="box3d", rmax=grmax, ncell=ncell)
+    try:
+        out, job = _run(runner, kind, a, b, bins, grid, which=("DD", "DR"))
+    except api.CuteError as e:
+        assert periodic and e.status == -2      # too few cells for this rmax: refused, never silently wrong
+        out, job = _run(runner, kind, a, b, bins, dict(mode="none"), which=("DD", "DR"))
+    _parity(oracle, out["DD"][0], kind, a, None, bins)
+    _parity(oracle, out["DR"][0], kind, a, b, bins)
