@@ -300,18 +300,17 @@ __device__ __forceinline__ BinOut bin_of(const Consts &c, float q, float wi, flo
         // sigma = sqrt(q - pi^2)  (Eq. 2); both taus depend on the pair (1/|l| and 1/sigma)
         const float pn = (wi - wj) + (lwi - lwj);
         const float m = fmaf(2.0f, wi + wj, -q);
-        const float w1 = fast_rsqrt(m);
+        const float w1 = fast_rsqrt(fmaxf(m, 1.0e-30f));               // clamps: no NaN/inf, a huge tau instead
         const float pi = fabsf(pn) * w1;
         const float epi = fmaf(w1 * w1, c.c1, c.c2);                   // absolute error bound of pi for this pair
         const float t1 = fmaf(pi, c.S1, c.O1), tau1 = fmaf(epi, c.S1, c.tau1);
         const float fa = __fadd_rd(t1 - tau1, CUTE_MAGIC_F), fb = __fadd_rd(t1 + tau1, CUTE_MAGIC_F);
-        const float s2 = fmaf(-pi, pi, q);
+        const float s2 = fmaxf(fmaf(-pi, pi, q), 1.0e-30f);
         const float w2 = fast_rsqrt(s2);
         const float t2 = fmaf(s2 * w2, c.S2, c.O2), tau2 = fmaf(w2, fmaf(epi, c.c3, c.tauw2), c.tau2);
         const float f2a = __fadd_rd(t2 - tau2, CUTE_MAGIC_F), f2b = __fadd_rd(t2 + tau2, CUTE_MAGIC_F);
         const uint32_t k1 = __float_as_uint(fa) - (uint32_t)CUTE_MAGIC_BITS, k2 = __float_as_uint(f2a) - (uint32_t)CUTE_MAGIC_BITS;
-        const bool finite = (fa == fa) && (fb == fb) && (f2a == f2a) && (f2b == f2b);   // sigma^2 <= 0, |l| = 0: NaN
-        o.unsure = min((__float_as_uint(fb) - __float_as_uint(fa)) | (__float_as_uint(f2b) - __float_as_uint(f2a)) | (finite ? 0u : 1u), 15u);
+        o.unsure = min((__float_as_uint(fb) - __float_as_uint(fa)) | (__float_as_uint(f2b) - __float_as_uint(f2a)), 15u);
         o.inr = (k1 < c.n1) && (k2 < c.n2);
         o.kb = k1 * c.n2 + k2 + (uint32_t)CUTE_MAGIC_BITS;
         return o;
@@ -331,14 +330,14 @@ __device__ __forceinline__ BinOut bin_of(const Consts &c, float q, float wi, flo
         // mu = |s.l| / (|s||l|), s.l = |x_i|^2 - |x_j|^2 (hi/lo), |l|^2 = 2|x_i|^2 + 2|x_j|^2 - q
         const float pn = (wi - wj) + (lwi - lwj);
         const float m = fmaf(2.0f, wi + wj, -q);
-        const float w = fast_rsqrt(q * m);
+        // clamped away from 0: q = 0 or |l| = 0 then give a huge but finite w, hence a huge tau2 and an uncertain pair
+        const float w = fast_rsqrt(fmaxf(q * m, 1.0e-30f));
         const float t2 = fmaf(fabsf(pn) * w, c.S2, c.O2);
         const float tau2 = fmaf(w * w * q, c.c1, fmaf(w, c.tauw2, c.tau2));   // a + b/(r|l|) + c/|l|^2
         const float f2a = __fadd_rd(t2 - tau2, CUTE_MAGIC_F), f2b = __fadd_rd(t2 + tau2, CUTE_MAGIC_F);
         const uint32_t k2 = __float_as_uint(f2a) - (uint32_t)CUTE_MAGIC_BITS;
-        // q = 0 or NaN/inf from the reciprocal square root: f2a == f2b cannot be trusted
         // (clamped: tau2 grows without bound as r -> 0, and the caller keeps one byte per pair)
-        o.unsure += min((__float_as_uint(f2b) - __float_as_uint(f2a)) | ((q > 0.f && f2a == f2a && f2b == f2b) ? 0u : 1u), 15u);
+        o.unsure += min(__float_as_uint(f2b) - __float_as_uint(f2a), 15u);
         o.inr = o.inr && (k2 < c.n2);
         o.kb = (o.kb - (uint32_t)CUTE_MAGIC_BITS) * c.n2 + k2 + (uint32_t)CUTE_MAGIC_BITS;
     }
