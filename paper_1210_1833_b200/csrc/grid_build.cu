@@ -110,17 +110,39 @@ __device__ __forceinline__ bool cell_of(const BuildPlan &b, double a, double c1,
     return ok;
 }
 
-__global__ void k_cellid(BuildPlan b)
+// kPts points per thread, loads issued before their uses: these kernels are bound by the latency of dependent
+// scattered accesses (ncu: long_scoreboard), so memory-level parallelism per thread is what buys bandwidth.
+constexpr int kPts = 4;
+
+__global__ void __launch_bounds__(256) k_cellid(BuildPlan b)
 {
-    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (i >= b.n) return;
-    double a = load_coord(b.c0, b.dtype, i), c1 = load_coord(b.c1, b.dtype, i);
-    double c2 = (b.coord == CUTE_COORD_RADEC) ? 0.0 : load_coord(b.c2, b.dtype, i);
-    uint32_t id;
-    bool ok = cell_of(b, a, c1, c2, id);
-    if (!ok || !isfinite(a) || !isfinite(c1) || !isfinite(c2)) atomicExch(&b.status[0], 1u);
-    b.cell_id[i] = id;
-    b.rank[i] = atomicAdd(&b.count[id], 1u);   // rank inside the cell (order arbitrary, pin V4)
+    const int64_t base = (int64_t)blockIdx.x * (blockDim.x * kPts) + threadIdx.x;
+    double a[kPts], c1[kPts], c2[kPts];
+#pragma unroll
+    for (int k = 0; k < kPts; k++) {
+        const int64_t i = base + (int64_t)k * blockDim.x;
+        a[k] = c1[k] = c2[k] = 0.0;
+        if (i < b.n) {
+            a[k] = load_coord(b.c0, b.dtype, i); c1[k] = load_coord(b.c1, b.dtype, i);
+            if (b.coord != CUTE_COORD_RADEC) c2[k] = load_coord(b.c2, b.dtype, i);
+        }
+    }
+    uint32_t id[kPts], rk[kPts];
+    bool bad = false;
+#pragma unroll
+    for (int k = 0; k < kPts; k++) {
+        const bool ok = cell_of(b, a[k], c1[k], c2[k], id[k]);
+        bad = bad || ((base + (int64_t)k * blockDim.x < b.n) && (!ok || !isfinite(a[k]) || !isfinite(c1[k]) || !isfinite(c2[k])));
+    }
+#pragma unroll
+    for (int k = 0; k < kPts; k++)
+        rk[k] = (base + (int64_t)k * blockDim.x < b.n) ? atomicAdd(&b.count[id[k]], 1u) : 0u;   // rank inside the cell (order arbitrary, pin V4)
+#pragma unroll
+    for (int k = 0; k < kPts; k++) {
+        const int64_t i = base + (int64_t)k * blockDim.x;
+        if (i < b.n) { b.cell_id[i] = id[k]; b.rank[i] = rk[k]; }
+    }
+    if (bad) atomicExch(&b.status[0], 1u);
 }
 
 // ---- G2: exclusive scan (three launches; n <= 2^27 elements) ---------------------------------
@@ -202,30 +224,53 @@ static cudaError_t exclusive_scan(const uint32_t *in, int64_t n, uint32_t *out, 
 // sin d) in float64 ("projects all objects in the catalog into the unit sphere"),
 // then the same hi/lo split; w carries float32(z) for RADECZ.  p64 keeps the float64 values for
 // the refine path.
-__global__ void k_scatter(BuildPlan b)
+__global__ void __launch_bounds__(256) k_scatter(BuildPlan b)
 {
-    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (i >= b.n) return;
-    double a = load_coord(b.c0, b.dtype, i), c1 = load_coord(b.c1, b.dtype, i);
-    double c2 = (b.coord == CUTE_COORD_RADEC) ? 0.0 : load_coord(b.c2, b.dtype, i);
-    uint32_t slot, id = 0;
-    if (b.mode == CUTE_GRID_NONE) slot = (uint32_t)i;
-    else { id = b.cell_id[i]; slot = b.cell_start[id] + b.rank[i]; }
-    // XYZ: w carries |x|^2 split hi/lo, so that the (r,mu) kernel gets s.l = |x_i|^2 - |x_j|^2 without
-    // cancellation (l = x_i + x_j is the mid-point line of sight)
-    double v[4] = {a, c1, c2, a * a + c1 * c1 + c2 * c2};
-    if (b.coord != CUTE_COORD_XYZ) {
-        double al = a * (kPi / 180.0), de = c1 * (kPi / 180.0), sa, ca, sd, cd;
-        sincos(al, &sa, &ca);
-        sincos(de, &sd, &cd);
-        v[0] = cd * ca; v[1] = cd * sa; v[2] = sd; v[3] = c2;
+    const int64_t base = (int64_t)blockIdx.x * (blockDim.x * kPts) + threadIdx.x;
+    double a[kPts], c1[kPts], c2[kPts];
+    uint32_t slot[kPts];
+#pragma unroll
+    for (int k = 0; k < kPts; k++) {
+        const int64_t i = base + (int64_t)k * blockDim.x;
+        a[k] = c1[k] = c2[k] = 0.0;
+        slot[k] = 0;
+        if (i < b.n) {
+            a[k] = load_coord(b.c0, b.dtype, i); c1[k] = load_coord(b.c1, b.dtype, i);
+            if (b.coord != CUTE_COORD_RADEC) c2[k] = load_coord(b.c2, b.dtype, i);
+            slot[k] = (b.mode == CUTE_GRID_NONE) ? (uint32_t)i : b.cell_id[i];
+        }
     }
-    float h[4], l[4];
-    for (int d = 0; d < 4; d++) { h[d] = (float)v[d]; l[d] = (float)(v[d] - (double)h[d]); }
-    b.hi[slot] = make_float4(h[0], h[1], h[2], h[3]);
-    if (b.want_lo) b.lo[slot] = make_float4(l[0], l[1], l[2], l[3]);
-    if (b.want_f64) for (int d = 0; d < 4; d++) b.p64[(size_t)d * b.n_pad + slot] = v[d];
-    b.perm[slot] = (uint32_t)i;
+    if (b.mode != CUTE_GRID_NONE) {
+        uint32_t rk[kPts];
+#pragma unroll
+        for (int k = 0; k < kPts; k++) {
+            const int64_t i = base + (int64_t)k * blockDim.x;
+            rk[k] = (i < b.n) ? b.rank[i] : 0u;
+            slot[k] = (i < b.n) ? b.cell_start[slot[k]] : 0u;
+        }
+#pragma unroll
+        for (int k = 0; k < kPts; k++) slot[k] += rk[k];
+    }
+#pragma unroll
+    for (int k = 0; k < kPts; k++) {
+        const int64_t i = base + (int64_t)k * blockDim.x;
+        if (i >= b.n) continue;
+        // XYZ: w carries |x|^2 split hi/lo, so that the (r,mu) kernel gets s.l = |x_i|^2 - |x_j|^2 without
+        // cancellation (l = x_i + x_j is the mid-point line of sight)
+        double v[4] = {a[k], c1[k], c2[k], a[k] * a[k] + c1[k] * c1[k] + c2[k] * c2[k]};
+        if (b.coord != CUTE_COORD_XYZ) {
+            double al = a[k] * (kPi / 180.0), de = c1[k] * (kPi / 180.0), sa, ca, sd, cd;
+            sincos(al, &sa, &ca);
+            sincos(de, &sd, &cd);
+            v[0] = cd * ca; v[1] = cd * sa; v[2] = sd; v[3] = c2[k];
+        }
+        float h[4], l[4];
+        for (int d = 0; d < 4; d++) { h[d] = (float)v[d]; l[d] = (float)(v[d] - (double)h[d]); }
+        b.hi[slot[k]] = make_float4(h[0], h[1], h[2], h[3]);
+        if (b.want_lo) b.lo[slot[k]] = make_float4(l[0], l[1], l[2], l[3]);
+        if (b.want_f64) for (int d = 0; d < 4; d++) b.p64[(size_t)d * b.n_pad + slot[k]] = v[d];
+        b.perm[slot[k]] = (uint32_t)i;
+    }
 }
 
 // ---- G4: chunk table ---------------------------------------------------------------------------
@@ -300,14 +345,14 @@ cudaError_t run_build(const BuildPlan &b, cudaStream_t s)
 {
     cudaError_t e;
     const int T = 256;
-    int blocks = (int)((b.n + T - 1) / T);
+    const int pblocks = (int)((b.n + (int64_t)T * kPts - 1) / ((int64_t)T * kPts));
     if ((e = cudaMemsetAsync(b.status, 0, 8, s)) != cudaSuccess) return e;
     if (b.mode != CUTE_GRID_NONE) {
         if ((e = cudaMemsetAsync(b.count, 0, (size_t)(b.ncells + 1) * 4, s)) != cudaSuccess) return e;
-        if (b.n > 0) { k_cellid<<<blocks, T, 0, s>>>(b); note_launches(1); }
+        if (b.n > 0) { k_cellid<<<pblocks, T, 0, s>>>(b); note_launches(1); }
         if ((e = exclusive_scan(b.count, b.ncells, b.cell_start, b.scan_tmp, s)) != cudaSuccess) return e;
     }
-    if (b.n > 0) { k_scatter<<<blocks, T, 0, s>>>(b); note_launches(1); }
+    if (b.n > 0) { k_scatter<<<pblocks, T, 0, s>>>(b); note_launches(1); }
     k_row_counts<<<(int)((b.nrows + T - 1) / T), T, 0, s>>>(b);
     if ((e = exclusive_scan(b.row_nchunks, b.nrows, b.row_chunk_start, b.scan_tmp, s)) != cudaSuccess) return e;
     uint32_t max_chunks = (uint32_t)(b.n / kChunk + b.nrows + 1);
