@@ -386,9 +386,18 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config 1..5 (default 2: the metric's workload)")
     ap.add_argument("--scale", type=float, default=1.0, help="shrink the catalogues (debugging only; 1.0 = the named config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--grid", default="default", choices=["default", "none", "sphere", "box3d"],
+                    help="override the workload's neighbour search (default: the one BASELINE.json names)")
+    ap.add_argument("--pix", type=float, default=0.1, help="--grid sphere: pixel side in units of theta_max")
     args = ap.parse_args()
     from paper_1210_1833_b200 import synth
     w = synth.workload(args.config, args.scale)
+    if args.grid == "none":
+        w.grid = dict(mode="none")
+    elif args.grid == "sphere":
+        w.grid = dict(mode="sphere", thetamax=w.bins["aperture"] if w.kind == "radial" else w.bins["hi1"], pix=args.pix)
+    elif args.grid == "box3d":
+        w.grid = dict(mode="box3d", rmax=w.bins["hi1"])
     cfg = {"workload": f"BASELINE.json configs[{args.config - 1}] ({w.name}: {w.kind}, {'+'.join(w.pairs)}, "
                        f"nd={len(w.data[0])}, nr={len(w.rand[0]) if w.rand is not None else 0}, bins={w.bins['n1']}x{max(w.bins.get('n2', 0), 1)}, "
                        f"grid={w.grid.get('mode', 'none')})",

@@ -25,6 +25,10 @@
  *   S4  self pairs skipped; distinct coincident points are a pair with r = 0;
  *   S5  mu uses the mid-point line of sight l = x_i + x_j (pinned by Eq. 9);
  *   S6  mu = |cos|;  mu >= 1 goes to the last mu bin when hi2 >= 1; r = 0 => mu := 0;
+ *   P1  pixelised catalogues: pixels with constant limits in (sin dec, RA); a pixel is
+ *       represented by its centre in those coordinates and weighted by its number of objects;
+ *   P2  weighted pairs: pair (i,j) counts w_i w_j; in an auto-correlation the w_i objects of one pixel count as
+ *       w_i (w_i - 1)/2 pairs at zero separation, so that weights are exactly equivalent to repeated objects;
  *   N1  (pi,sigma): pi = r mu with the mu of S5/S6, sigma = sqrt(max(0, r^2 - pi^2)) (Eq. 2); first
  *       variable pi (major index), second sigma;
  *   S7  radial: zbar = (z_i+z_j)/2 (major index), dz = |z_i - z_j|;
@@ -131,6 +135,7 @@ static int edge_flag(const axis_t *a, double v, int k, int *edge, int *other)
 typedef struct {
     int64_t n;
     const double *a, *b, *c; /* inputs: xyz | ra,dec[,z] */
+    const uint32_t *w;       /* optional integer weights (NULL = 1): objects per pixel */
     double *ux, *uy, *uz;    /* unit vectors (ANGULAR/RADIAL), owned */
 } cat_t;
 
@@ -180,7 +185,9 @@ static inline double theta_of(const cat_t *c1, int64_t i, const cat_t *c2, int64
     return 2.0 * asin(h);
 }
 
-static inline void pair_eval(acc_t *A, const cat_t *c1, int64_t i, const cat_t *c2, int64_t j)
+/* wp = weight of the pair: w_i * w_j ("weighting each of them by the number of objects that fall inside it",
+ * PAPER.md:233), or w_i (w_i - 1) / 2 for the objects of one pixel among themselves (j == i, zero separation) */
+static inline void pair_eval(acc_t *A, const cat_t *c1, int64_t i, const cat_t *c2, int64_t j, uint64_t wp)
 {
     double v1, v2 = 0.0;
     int in_ap = 1, ap_flag = 0;
@@ -230,15 +237,15 @@ static inline void pair_eval(acc_t *A, const cat_t *c1, int64_t i, const cat_t *
     int two = A->ax2.n > 0;
     if (two) k2 = find_bin(&A->ax2, v2);
     int cell = (in_ap && k1 >= 0 && k2 >= 0) ? k1 * A->n2eff + k2 : -1;
-    if (cell >= 0) A->hist[cell]++;
+    if (cell >= 0) A->hist[cell] += wp;
     /* ambiguity flags */
     int e1, o1 = 0, e2 = 0, o2 = 0;
     int f1 = edge_flag(&A->ax1, v1, k1, &e1, &o1);
     int f2 = two ? edge_flag(&A->ax2, v2, k2, &e2, &o2) : 0;
     if (!(f1 || f2 || ap_flag)) return;
-    if (f1) A->amb_e1[e1]++;
-    if (f2) A->amb_e2[e2]++;
-    if (ap_flag) A->amb_e2[A->ax2.n + 1]++;
+    if (f1) A->amb_e1[e1] += wp;
+    if (f2) A->amb_e2[e2] += wp;
+    if (ap_flag) A->amb_e2[A->ax2.n + 1] += wp;
     /* every cell the pair could land in: product of candidate bins, "out" -> virtual cell */
     int c1s[2] = {k1, o1}, c2s[2] = {k2, o2};
     int n1c = f1 ? 2 : 1, n2c = f2 ? 2 : 1, nap = ap_flag ? 2 : 1;
@@ -251,7 +258,7 @@ static inline void pair_eval(acc_t *A, const cat_t *c1, int64_t i, const cat_t *
                 int c = (inap && kk1 >= 0 && kk2 >= 0) ? kk1 * A->n2eff + kk2 : A->ncell;
                 int dup = 0;
                 for (int s = 0; s < ns; s++) if (seen[s] == c) dup = 1;
-                if (!dup) { seen[ns++] = c; A->amb_cell[c]++; }
+                if (!dup) { seen[ns++] = c; A->amb_cell[c] += wp; }
             }
 }
 
@@ -402,11 +409,11 @@ static int64_t lower_bound_d(const double *a, int64_t lo, int64_t hi, double v)
  * amb_e2[n2+2] (may be NULL), *npairs = separations evaluated.
  * Angles: coordinates RA/Dec in DEGREES; bin limits and aperture in RADIANS.
  */
-int orc_count(int kind, int mode,
-              int64_t n1, const double *a1, const double *b1, const double *c1,
-              int64_t n2, const double *a2, const double *b2, const double *c2,
-              const orc_bins *bins, int64_t i_begin, int64_t i_end, int nthreads,
-              uint64_t *hist, uint64_t *amb_cell, uint64_t *amb_e1, uint64_t *amb_e2, uint64_t *npairs)
+int orc_count_w(int kind, int mode,
+                int64_t n1, const double *a1, const double *b1, const double *c1, const uint32_t *w1,
+                int64_t n2, const double *a2, const double *b2, const double *c2, const uint32_t *w2,
+                const orc_bins *bins, int64_t i_begin, int64_t i_end, int nthreads,
+                uint64_t *hist, uint64_t *amb_cell, uint64_t *amb_e1, uint64_t *amb_e2, uint64_t *npairs)
 {
     int auto_ = (a2 == NULL);
     int rc = check_args(kind, bins, auto_);
@@ -417,7 +424,8 @@ int orc_count(int kind, int mode,
     if (!e1 || !e2) return ORC_ENOMEM;
     orc_edges(bins, 0, e1);
     if (bins->n2 > 0) orc_edges(bins, 1, e2);
-    cat_t C1 = {n1, a1, b1, c1, 0, 0, 0}, C2s = {n2, a2, b2, c2, 0, 0, 0};
+    cat_t C1 = {n1, a1, b1, c1, w1, 0, 0, 0}, C2s = {n2, a2, b2, c2, w2, 0, 0, 0};
+#define WPROD(i, j) ((uint64_t)(C1.w ? C1.w[i] : 1u) * (uint64_t)(C2->w ? C2->w[j] : 1u))
     if ((rc = prep_cat(kind, &C1))) return rc;
     cat_t *C2 = &C1;
     if (!auto_) { if ((rc = prep_cat(kind, &C2s))) return rc; C2 = &C2s; }
@@ -455,8 +463,11 @@ int orc_count(int kind, int mode,
         if (!failed) {
 #pragma omp for schedule(dynamic, 16)
             for (int64_t i = i_begin; i < i_end; i++) {
+                /* the w_i objects of one pixel are w_i (w_i - 1) / 2 pairs at zero separation (reading P2) */
+                if (auto_ && C1.w && C1.w[i] > 1)
+                    pair_eval(&T, &C1, i, C2, i, (uint64_t)C1.w[i] * (uint64_t)(C1.w[i] - 1) / 2);
                 if (mode == 0) {
-                    for (int64_t j = auto_ ? i + 1 : 0; j < C2->n; j++) pair_eval(&T, &C1, i, C2, j);
+                    for (int64_t j = auto_ ? i + 1 : 0; j < C2->n; j++) pair_eval(&T, &C1, i, C2, j, WPROD(i, j));
                 } else if (cells.kind3d) {
                     const double *X[3] = {C1.a, C1.b, C1.c};
                     int k[3], lo[3], hi[3];
@@ -484,7 +495,7 @@ int orc_count(int kind, int mode,
                                 for (int64_t s = cells.start[cidx]; s < cells.start[cidx + 1]; s++) {
                                     int64_t j = cells.idx[s];
                                     if (auto_ && j <= i) continue;
-                                    pair_eval(&T, &C1, i, C2, j);
+                                    pair_eval(&T, &C1, i, C2, j, WPROD(i, j));
                                 }
                             }
                 } else {
@@ -514,7 +525,7 @@ int orc_count(int kind, int mode,
                             for (int64_t s = p0; s < s1 && cells.ra_sorted[s] <= wins[q][1]; s++) {
                                 int64_t j = cells.idx[s];
                                 if (auto_ && j <= i) continue;
-                                pair_eval(&T, &C1, i, C2, j);
+                                pair_eval(&T, &C1, i, C2, j, WPROD(i, j));
                             }
                         }
                     }
@@ -544,6 +555,57 @@ int orc_count(int kind, int mode,
     if (!auto_) free_cat(&C2s);
     free(e1); free(e2);
     return failed ? ORC_ENOMEM : ORC_OK;
+}
+
+int orc_count(int kind, int mode,
+              int64_t n1, const double *a1, const double *b1, const double *c1,
+              int64_t n2, const double *a2, const double *b2, const double *c2,
+              const orc_bins *bins, int64_t i_begin, int64_t i_end, int nthreads,
+              uint64_t *hist, uint64_t *amb_cell, uint64_t *amb_e1, uint64_t *amb_e2, uint64_t *npairs)
+{
+    return orc_count_w(kind, mode, n1, a1, b1, c1, NULL, n2, a2, b2, c2, NULL, bins, i_begin, i_end, nthreads,
+                       hist, amb_cell, amb_e1, amb_e2, npairs);
+}
+
+/* Pixel map of an angular catalogue ("create a pixel map from the catalog and then correlate the
+ * pixels (weighting each of them by the number of objects that fall inside it)"), on pixels "with constant limits
+ * in (cos theta, phi)": n_ra x n_u pixels over RA in [ra0, ra0+dra) (degrees, taken modulo 360
+ * relative to ra0) and u = sin(dec) in [u0, u0+du).  Reading P1: a pixel is represented by its centre in (RA, u).
+ * Outputs (caller-allocated, n_ra*n_u entries, only the first *npix used): centre RA, centre Dec [deg], count.
+ * Non-empty pixels only, in pixel-index order (u-major).  Returns ORC_EINVAL if a point falls outside the map. */
+int orc_pixelize(int64_t n, const double *ra, const double *dec, double ra0, double dra, double u0, double du,
+                 int n_ra, int n_u, double *pra, double *pdec, uint32_t *pw, int64_t *npix)
+{
+    if (n < 0 || n_ra < 1 || n_u < 1 || !(dra > 0.0) || !(du > 0.0)) return ORC_EINVAL;
+    int64_t np = (int64_t)n_ra * n_u;
+    uint32_t *cnt = (uint32_t *)calloc((size_t)np, sizeof(uint32_t));
+    if (!cnt) return ORC_ENOMEM;
+    for (int64_t i = 0; i < n; i++) {
+        double al = fmod(ra[i] - ra0, 360.0);
+        if (al < 0.0) al += 360.0;
+        double u = sin(dec[i] * (ORC_PI / 180.0)) - u0;
+        if (al > dra || u < -1e-15 || u > du + 1e-15) { free(cnt); return ORC_EINVAL; }
+        int kx = (int)floor(al * ((double)n_ra / dra)), ky = (int)floor(u * ((double)n_u / du));
+        if (kx > n_ra - 1) kx = n_ra - 1;
+        if (ky > n_u - 1) ky = n_u - 1;
+        if (kx < 0) kx = 0;
+        if (ky < 0) ky = 0;
+        cnt[(int64_t)ky * n_ra + kx]++;
+    }
+    int64_t m = 0;
+    for (int64_t p = 0; p < np; p++) {
+        if (!cnt[p]) continue;
+        int kx = (int)(p % n_ra), ky = (int)(p / n_ra);
+        double r = ra0 + ((double)kx + 0.5) * (dra / (double)n_ra);
+        double uc = u0 + ((double)ky + 0.5) * (du / (double)n_u);
+        if (uc > 1.0) uc = 1.0;
+        if (uc < -1.0) uc = -1.0;
+        pra[m] = fmod(r, 360.0); pdec[m] = asin(uc) * (180.0 / ORC_PI); pw[m] = cnt[p];
+        m++;
+    }
+    *npix = m;
+    free(cnt);
+    return ORC_OK;
 }
 
 /* ------------------------------------------------------------------ estimators (host arithmetic) */

@@ -46,6 +46,11 @@ def _load():
         up = C.POINTER(C.c_uint64)
         _lib.orc_count.argtypes = [C.c_int, C.c_int, C.c_int64, dp, dp, dp, C.c_int64, dp, dp, dp,
                                    C.POINTER(_Bins), C.c_int64, C.c_int64, C.c_int, up, up, up, up, up]
+        wp = C.POINTER(C.c_uint32)
+        _lib.orc_count_w.argtypes = [C.c_int, C.c_int, C.c_int64, dp, dp, dp, wp, C.c_int64, dp, dp, dp, wp,
+                                     C.POINTER(_Bins), C.c_int64, C.c_int64, C.c_int, up, up, up, up, up]
+        _lib.orc_pixelize.argtypes = [C.c_int64, dp, dp, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int,
+                                      dp, dp, wp, C.POINTER(C.c_int64)]
         _lib.orc_edges.argtypes = [C.POINTER(_Bins), C.c_int, dp]
         _lib.orc_landy_szalay.argtypes = [up, up, up, C.c_uint64, C.c_uint64, C.c_int, dp]
         _lib.orc_natural.argtypes = [up, up, C.c_uint64, C.c_uint64, C.c_int, dp]
@@ -90,7 +95,7 @@ def edges(bins: dict, axis: int = 0) -> np.ndarray:
     return e
 
 
-def count(kind: str, cat1, cat2, bins: dict, mode: str = "plain", i_range=None, nthreads: int = 0):
+def count(kind: str, cat1, cat2, bins: dict, mode: str = "plain", i_range=None, nthreads: int = 0, w1=None, w2=None):
     """Histogram of the pairs of cat1 x cat2 (cat2 None: unordered pairs of cat1).
 
     Returns dict(hist, amb_cell, amb_e1, amb_e2, npairs); hist has n1*max(n2,1) uint64 entries
@@ -113,14 +118,32 @@ def count(kind: str, cat1, cat2, bins: dict, mode: str = "plain", i_range=None, 
     npairs = np.zeros(1, dtype=np.uint64)
     i0, i1 = (0, n1) if i_range is None else i_range
     null = C.POINTER(C.c_double)()
-    rc = lib.orc_count(KINDS[kind], {"plain": 0, "celled": 1}[mode],
-                       n1, _dp(c1[0]), _dp(c1[1]), _dp(c1[2]),
-                       n2, _dp(c2[0]) if c2 else null, _dp(c2[1]) if c2 else null, _dp(c2[2]) if c2 else null,
+    wnull = C.POINTER(C.c_uint32)()
+    w1 = None if w1 is None else np.ascontiguousarray(np.asarray(w1, dtype=np.uint32))
+    w2 = None if w2 is None else np.ascontiguousarray(np.asarray(w2, dtype=np.uint32))
+    wptr = lambda w: wnull if w is None else w.ctypes.data_as(C.POINTER(C.c_uint32))
+    rc = lib.orc_count_w(KINDS[kind], {"plain": 0, "celled": 1}[mode],
+                       n1, _dp(c1[0]), _dp(c1[1]), _dp(c1[2]), wptr(w1),
+                       n2, _dp(c2[0]) if c2 else null, _dp(c2[1]) if c2 else null, _dp(c2[2]) if c2 else null, wptr(w2),
                        C.byref(b), int(i0), int(i1), int(nthreads),
                        _up(hist), _up(amb_cell), _up(amb_e1), _up(amb_e2), _up(npairs))
     if rc:
         raise ValueError(f"orc_count failed ({rc})")
     return dict(hist=hist, amb_cell=amb_cell, amb_e1=amb_e1, amb_e2=amb_e2, npairs=int(npairs[0]))
+
+
+def pixelize(ra, dec, ra0: float, dra: float, u0: float, du: float, n_ra: int, n_u: int):
+    """Pixel map: centres (RA, Dec in degrees) and counts of the non-empty pixels."""
+    ra = np.ascontiguousarray(np.asarray(ra, dtype=np.float64))
+    dec = np.ascontiguousarray(np.asarray(dec, dtype=np.float64))
+    npx = int(n_ra) * int(n_u)
+    pra, pdec, pw = np.zeros(npx), np.zeros(npx), np.zeros(npx, dtype=np.uint32)
+    m = C.c_int64(0)
+    rc = _load().orc_pixelize(ra.size, _dp(ra), _dp(dec), float(ra0), float(dra), float(u0), float(du), int(n_ra), int(n_u),
+                              _dp(pra), _dp(pdec), pw.ctypes.data_as(C.POINTER(C.c_uint32)), C.byref(m))
+    if rc:
+        raise ValueError(f"orc_pixelize failed ({rc})")
+    return pra[:m.value].copy(), pdec[:m.value].copy(), pw[:m.value].copy()
 
 
 def landy_szalay(dd, dr, rr, nd: int, nr: int):

@@ -388,3 +388,80 @@ def test_multipoles_closed_form(oracle):
     assert np.allclose(m[0], a, atol=2e-3) and np.allclose(m[1], b, atol=5e-3) and np.allclose(m[2], c, atol=1e-2)
     m = oracle.multipoles(np.full((n_r, n_mu), 0.7), n_r, n_mu)
     assert np.allclose(m[0], 0.7, atol=1e-14) and np.allclose(m[1], 0, atol=2e-3) and np.allclose(m[2], 0, atol=2e-3)
+
+
+# ------------------------------------------------------------------------------- N2: weights and pixel maps
+@pytest.mark.parametrize("kind", ["angular", "monopole", "rmu"])
+def test_weights_are_repeated_objects(oracle, kind):
+    """reading P2: a catalogue with integer weights gives exactly the counts of the catalogue in which object i is
+    repeated w_i times (the copies of one object being w(w-1)/2 pairs at zero separation), auto and cross, plain and celled"""
+    rng = np.random.default_rng(31)
+    n1, n2 = 300, 200
+    if kind == "angular":
+        c1 = (rng.random(n1) * 6 + 10, rng.random(n1) * 6 - 3)
+        c2 = (rng.random(n2) * 6 + 10, rng.random(n2) * 6 - 3)
+        bins = dict(n1=12, lo1=0.0, hi1=math.radians(2.0))
+    else:
+        c1 = tuple(rng.random((3, n1)) * 100 + 300)
+        c2 = tuple(rng.random((3, n2)) * 100 + 300)
+        bins = dict(n1=10, lo1=0.0, hi1=40.0)
+        if kind == "rmu":
+            bins.update(n2=5, lo2=0.0, hi2=1.0)
+        else:
+            bins.update(box_L=0.0)
+    w1, w2 = rng.integers(1, 5, n1), rng.integers(1, 4, n2)
+    e1 = tuple(np.repeat(c, w1) for c in c1)
+    e2 = tuple(np.repeat(c, w2) for c in c2)
+    for mode in ("plain", "celled"):
+        a = oracle.count(kind, c1, None, bins, mode=mode, w1=w1)
+        b = oracle.count(kind, e1, None, bins, mode=mode)
+        assert np.array_equal(a["hist"], b["hist"]) and a["hist"][0] >= (w1 * (w1 - 1) // 2).sum()
+        a = oracle.count(kind, c1, c2, bins, mode=mode, w1=w1, w2=w2)
+        b = oracle.count(kind, e1, e2, bins, mode=mode)
+        assert np.array_equal(a["hist"], b["hist"])
+    ones = oracle.count(kind, c1, c2, bins, w1=np.ones(n1, dtype=np.uint32), w2=np.ones(n2, dtype=np.uint32))
+    assert np.array_equal(ones["hist"], oracle.count(kind, c1, c2, bins)["hist"])
+
+
+def test_pixel_map(oracle):
+    """reading P1: pixels with constant limits in (RA, sin dec), represented by their centres"""
+    # 2 x 2 pixels over RA [0,20) x sin(dec) [0,0.5): centres RA 5, 15; sin(dec) 0.125, 0.375 -> dec 7.18076, 22.02431 deg
+    ra = np.array([1.0, 2.0, 19.0, 11.0, 3.0])
+    dec = np.array([1.0, 14.0, 16.0, 29.0, 2.0])       # sin: 0.0175, 0.2419, 0.2756, 0.4848, 0.0349
+    pra, pdec, pw = oracle.pixelize(ra, dec, 0.0, 20.0, 0.0, 0.5, 2, 2)
+    assert np.allclose(pra, [5.0, 15.0]) and np.allclose(pdec, [7.18076, 22.02431], atol=1e-5)
+    assert list(pw) == [3, 2]                          # (1,1) (2,14) (3,2) below sin = 0.25 at RA < 10; (19,16) (11,29) above, RA > 10
+    rng = np.random.default_rng(5)
+    n = 5000
+    ra = (355.0 + rng.random(n) * 12.0) % 360.0        # across the RA = 0 seam
+    dec = np.degrees(np.arcsin(rng.random(n) * 0.4 - 0.2))
+    nra, nu = 24, 20
+    pra, pdec, pw = oracle.pixelize(ra, dec, 355.0, 12.0, -0.2, 0.4, nra, nu)
+    assert pw.sum() == n and len(pw) <= nra * nu
+    # every object lies inside the pixel that counts it: rebuild the counts from the centres
+    kx = np.floor(((ra - 355.0) % 360.0) / (12.0 / nra)).astype(int)
+    ky = np.floor((np.sin(np.radians(dec)) + 0.2) / (0.4 / nu)).astype(int)
+    cx = np.floor(((pra - 355.0) % 360.0) / (12.0 / nra)).astype(int)
+    cy = np.floor((np.sin(np.radians(pdec)) + 0.2) / (0.4 / nu)).astype(int)
+    want = np.bincount(ky * nra + kx, minlength=nra * nu)
+    assert np.array_equal(want[cy * nra + cx], pw) and want.sum() == pw.sum()
+    with pytest.raises(ValueError):
+        oracle.pixelize(np.array([30.0]), np.array([0.0]), 0.0, 20.0, -0.5, 1.0, 4, 4)   # outside the map
+
+
+def test_pixelised_counts_approach_the_exact_ones_above_the_pixel_scale(oracle):
+    """"if one is not interested in extremely small angular scales": w_pix pair counts agree with the
+    object counts at separations well above the pixel size, and differ below it"""
+    rng = np.random.default_rng(9)
+    n = 6000
+    ra = rng.random(n) * 20.0 + 100.0
+    dec = np.degrees(np.arcsin(rng.random(n) * 0.3))
+    pra, pdec, pw = oracle.pixelize(ra, dec, 100.0, 20.0, 0.0, 0.3, 100, 86)       # ~0.2 deg pixels
+    bins = dict(n1=8, lo1=math.radians(1.0), hi1=math.radians(5.0))
+    exact = oracle.count("angular", (ra, dec), None, bins)["hist"].astype(float)
+    pix = oracle.count("angular", (pra, pdec), None, bins, w1=pw)["hist"].astype(float)
+    assert np.all(np.abs(pix / exact - 1.0) < 0.04) and np.abs(pix.sum() / exact.sum() - 1.0) < 0.005
+    small = dict(n1=4, lo1=0.0, hi1=math.radians(0.1))
+    a = oracle.count("angular", (ra, dec), None, small)["hist"]
+    b = oracle.count("angular", (pra, pdec), None, small, w1=pw)["hist"]
+    assert b[0] == (pw.astype(np.int64) * (pw.astype(np.int64) - 1) // 2).sum() and b[1:].sum() == 0 and a[1:].sum() > 0
