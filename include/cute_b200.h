@@ -73,6 +73,10 @@ typedef struct cute_catalog {
     int coord;          /* CUTE_COORD_*            */
     int dtype;          /* CUTE_F32 | CUTE_F64     */
     const void *c0, *c1, *c2;
+    const uint32_t *weight; /* optional integer weights, 1 <= w <= 65535 (objects per pixel of a pixel map,        */
+                            /* PAPER.md:233); NULL = unweighted.  CUTE_COORD_RADEC / CUTE_ANGULAR only.  A pair    */
+                            /* counts w_i w_j; in an auto-correlation the w_i objects of one pixel count as        */
+                            /* w_i (w_i - 1)/2 pairs at zero separation (exactly as w_i repeated objects would).   */
 } cute_catalog;
 
 /* How to build the cell list.
@@ -154,6 +158,18 @@ uint64_t cute_launch_count(void);
  * DEVICE pointers; d_tmp is a DEVICE buffer of >= 64 bytes.  Synchronises the stream.  Used to give the
  * two grids of a cross-correlation one common explicit box. */
 int cute_catalog_bounds(const cute_catalog *cat, void *d_tmp, void *stream, double bounds[6]);
+
+/* Pixel map of an angular catalogue ("create a pixel map from the catalog and then correlate the
+ * pixels (weighting each of them by the number of objects that fall inside it)"): n_ra x n_u pixels with constant
+ * limits in RA [ra0, ra0 + dra) (degrees, modulo 360 relative to ra0) and sin(Dec) [u0, u0 + du).
+ * cat: DEVICE, CUTE_COORD_RADEC(Z), unweighted.  Outputs (DEVICE, room for min(n, n_ra*n_u) entries each): centre RA
+ * and Dec [deg, float64] and object count of every NON-EMPTY pixel, in pixel order (sin(Dec)-major); *npix (HOST) =
+ * their number.  The result is a weighted CUTE_COORD_RADEC catalogue for cute_make_grid.  d_workspace: DEVICE,
+ * cute_pixelize_workspace_bytes(n_ra, n_u).  Synchronises the stream. */
+int cute_pixelize_workspace_bytes(int n_ra, int n_u, size_t *bytes);
+int cute_pixelize(const cute_catalog *cat, double ra0, double dra, double u0, double du, int n_ra, int n_u,
+                  double *d_pix_ra, double *d_pix_dec, uint32_t *d_pix_weight, int64_t *npix,
+                  void *d_workspace, size_t bytes, void *stream);
 
 /* Size of the device workspace cute_make_grid needs for this catalogue and spec (256-byte granular). */
 int cute_grid_workspace_bytes(const cute_catalog *cat, const cute_grid_spec *spec, size_t *bytes);

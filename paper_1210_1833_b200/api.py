@@ -24,7 +24,7 @@ WARN_EMPTY_BIN = 1
 
 class cute_catalog(C.Structure):
     _fields_ = [("struct_size", C.c_size_t), ("n", C.c_int64), ("coord", C.c_int), ("dtype", C.c_int),
-                ("c0", C.c_void_p), ("c1", C.c_void_p), ("c2", C.c_void_p)]
+                ("c0", C.c_void_p), ("c1", C.c_void_p), ("c2", C.c_void_p), ("weight", C.c_void_p)]
 
 
 class cute_grid_spec(C.Structure):
@@ -55,7 +55,7 @@ class cute_grid_info(C.Structure):
 
 
 # every symbol include/cute_b200.h declares
-SYMBOLS = ["cute_version", "cute_strerror", "cute_launch_count", "cute_catalog_bounds", "cute_grid_workspace_bytes", "cute_make_grid", "cute_free_grid",
+SYMBOLS = ["cute_version", "cute_strerror", "cute_launch_count", "cute_catalog_bounds", "cute_pixelize_workspace_bytes", "cute_pixelize", "cute_grid_workspace_bytes", "cute_make_grid", "cute_free_grid",
            "cute_grid_get_info", "cute_count_scratch_bytes", "cute_count_pairs", "cute_count_items",
            "cute_count_status", "cute_host_workspace_bytes", "cute_count_pairs_host", "cute_bin_edges",
            "cute_landy_szalay", "cute_natural_estimator", "cute_multipoles", "cute_periodic_rr", "cute_periodic_xi"]
@@ -72,6 +72,9 @@ def _load() -> C.CDLL:
     lib.cute_strerror.argtypes = [C.c_int]
     lib.cute_launch_count.restype = C.c_uint64
     lib.cute_catalog_bounds.argtypes = [C.POINTER(cute_catalog), vp, vp, dp]
+    lib.cute_pixelize_workspace_bytes.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_size_t)]
+    lib.cute_pixelize.argtypes = [C.POINTER(cute_catalog), C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int,
+                                  vp, vp, vp, C.POINTER(C.c_int64), vp, C.c_size_t, vp]
     lib.cute_grid_workspace_bytes.argtypes = [C.POINTER(cute_catalog), C.POINTER(cute_grid_spec), C.POINTER(C.c_size_t)]
     lib.cute_make_grid.argtypes = [C.POINTER(cute_catalog), C.POINTER(cute_grid_spec), vp, C.c_size_t, vp, C.POINTER(vp)]
     lib.cute_free_grid.argtypes = [vp]
@@ -158,8 +161,9 @@ def _stream_ptr(stream=None) -> int:
     return int(s.cuda_stream)
 
 
-def _catalog(cols, coord: int, device_ptrs: bool):
-    """cols: 2 or 3 arrays (torch CUDA tensors when device_ptrs, numpy otherwise), one dtype."""
+def _catalog(cols, coord: int, device_ptrs: bool, weight=None):
+    """cols: 2 or 3 arrays (torch CUDA tensors when device_ptrs, numpy otherwise), one dtype; weight: optional
+    uint32 array of the same kind (torch int32 tensors carry the uint32 bits)."""
     need = 2 if coord == COORD_RADEC else 3
     cols = list(cols)[:need]
     if device_ptrs:
@@ -175,7 +179,16 @@ def _catalog(cols, coord: int, device_ptrs: bool):
         n = cols[0].size
     while len(ptrs) < 3:
         ptrs.append(None)
-    return cute_catalog(C.sizeof(cute_catalog), n, coord, dt, *ptrs), cols
+    wptr = None
+    if weight is not None:
+        if device_ptrs:
+            assert weight.is_cuda and weight.is_contiguous() and weight.element_size() == 4 and weight.numel() == n
+            wptr = weight.data_ptr()
+        else:
+            assert weight.dtype == np.uint32 and weight.flags.c_contiguous and weight.size == n
+            wptr = weight.ctypes.data
+        cols = cols + [weight]
+    return cute_catalog(C.sizeof(cute_catalog), n, coord, dt, *ptrs, wptr), cols
 
 
 # ------------------------------------------------------------------------------- grids
@@ -214,16 +227,37 @@ def cute_catalog_bounds(cols, coord: int, stream=None) -> np.ndarray:
     return out
 
 
+def cute_pixelize(cols, ra0: float, dra: float, u0: float, du: float, n_ra: int, n_u: int, stream=None):
+    """Pixel map of a device RA/Dec catalogue: returns (ra, dec, weight) CUDA tensors of the non-empty
+    pixels (float64 degrees, int32 counts)."""
+    torch = _torch()
+    cat, keep = _catalog(cols, COORD_RADEC, True)
+    nb = C.c_size_t(0)
+    _check(lib.cute_pixelize_workspace_bytes(int(n_ra), int(n_u), C.byref(nb)), "cute_pixelize_workspace_bytes")
+    ws = torch.empty(nb.value + 256, dtype=torch.uint8, device=keep[0].device)
+    off = (-ws.data_ptr()) % 256
+    cap = max(1, min(int(cat.n), int(n_ra) * int(n_u)))
+    pra = torch.empty(cap, dtype=torch.float64, device=keep[0].device)
+    pdec = torch.empty(cap, dtype=torch.float64, device=keep[0].device)
+    pw = torch.empty(cap, dtype=torch.int32, device=keep[0].device)
+    m = C.c_int64(0)
+    _check(lib.cute_pixelize(C.byref(cat), float(ra0), float(dra), float(u0), float(du), int(n_ra), int(n_u),
+                             C.c_void_p(pra.data_ptr()), C.c_void_p(pdec.data_ptr()), C.c_void_p(pw.data_ptr()), C.byref(m),
+                             C.c_void_p(ws.data_ptr() + off), ws.numel() - off, C.c_void_p(_stream_ptr(stream))), "cute_pixelize")
+    k = int(m.value)
+    return pra[:k].contiguous(), pdec[:k].contiguous(), pw[:k].contiguous()
+
+
 def cute_grid_workspace_bytes(cat: cute_catalog, spec: cute_grid_spec) -> int:
     b = C.c_size_t(0)
     _check(lib.cute_grid_workspace_bytes(C.byref(cat), C.byref(spec), C.byref(b)), "cute_grid_workspace_bytes")
     return int(b.value)
 
 
-def cute_make_grid(cols, coord: int, spec: cute_grid_spec, stream=None, workspace=None) -> Grid:
-    """cols: torch CUDA tensors (SoA).  Runs G0-G4 on the device."""
+def cute_make_grid(cols, coord: int, spec: cute_grid_spec, stream=None, workspace=None, weight=None) -> Grid:
+    """cols: torch CUDA tensors (SoA); weight: optional int32/uint32 CUDA tensor.  Runs G0-G4 on the device."""
     torch = _torch()
-    cat, keep = _catalog(cols, coord, True)
+    cat, keep = _catalog(cols, coord, True, weight)
     nbytes = cute_grid_workspace_bytes(cat, spec)
     if workspace is None:
         workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=keep[0].device if keep[0].numel() or True else "cuda")
@@ -276,13 +310,13 @@ def cute_count_status(counter: Counter, stream=None) -> dict:
 
 
 def cute_count_pairs_host(kind: int, cat1, cat2, coord: int, spec: cute_grid_spec, bins: dict, workspace=None, stream=None,
-                          opts: cute_count_opts | None = None):
+                          opts: cute_count_opts | None = None, w1=None, w2=None):
     """End to end with HOST (numpy) buffers: H2D copies, grid build, count, D2H of the histogram."""
     torch = _torch()
-    c1, k1 = _catalog([np.ascontiguousarray(c) for c in cat1], coord, False)
+    c1, k1 = _catalog([np.ascontiguousarray(c) for c in cat1], coord, False, None if w1 is None else np.ascontiguousarray(w1, dtype=np.uint32))
     c2 = k2 = None
     if cat2 is not None:
-        c2, k2 = _catalog([np.ascontiguousarray(c) for c in cat2], coord, False)
+        c2, k2 = _catalog([np.ascontiguousarray(c) for c in cat2], coord, False, None if w2 is None else np.ascontiguousarray(w2, dtype=np.uint32))
     b = bin_spec(bins)
     nb = C.c_size_t(0)
     _check(lib.cute_host_workspace_bytes(C.byref(c1), C.byref(c2) if c2 is not None else None, C.byref(spec), C.byref(b),

@@ -84,6 +84,7 @@ int check_catalog(const cute_catalog *c)
         if (!c->c0 || !c->c1) return CUTE_ERR_INVALID_ARG;
         if (c->coord != CUTE_COORD_RADEC && !c->c2) return CUTE_ERR_INVALID_ARG;
     }
+    if (c->weight && c->coord != CUTE_COORD_RADEC) return CUTE_ERR_UNSUPPORTED;   // weights: pixel maps of angular catalogues
     return CUTE_OK;
 }
 
@@ -186,6 +187,51 @@ int cute_catalog_bounds(const cute_catalog *cat, void *d_tmp, void *stream, doub
     return CUTE_OK;
 }
 
+int cute_pixelize_workspace_bytes(int n_ra, int n_u, size_t *bytes)
+{
+    if (!bytes || n_ra < 1 || n_u < 1 || (int64_t)n_ra * n_u > (1ll << 28)) return CUTE_ERR_INVALID_ARG;
+    const size_t np = (size_t)n_ra * n_u;
+    *bytes = 256 + 2 * align_up((np + 2) * 4, 256) + align_up((np / 4096 + 2) * 4, 256);
+    return CUTE_OK;
+}
+
+int cute_pixelize(const cute_catalog *cat, double ra0, double dra, double u0, double du, int n_ra, int n_u,
+                  double *d_pix_ra, double *d_pix_dec, uint32_t *d_pix_weight, int64_t *npix,
+                  void *d_workspace, size_t bytes, void *stream)
+{
+    int rc = check_catalog(cat);
+    if (rc) return rc;
+    size_t need = 0;
+    if ((rc = cute_pixelize_workspace_bytes(n_ra, n_u, &need))) return rc;
+    if (cat->coord == CUTE_COORD_XYZ || cat->weight) return CUTE_ERR_INVALID_ARG;
+    if (!(dra > 0.0) || dra > 360.0 || !(du > 0.0) || u0 < -1.0 - 1e-12 || u0 + du > 1.0 + 1e-12) return CUTE_ERR_INVALID_ARG;
+    if (!d_pix_ra || !d_pix_dec || !d_pix_weight || !npix || !d_workspace || ((uintptr_t)d_workspace & 255)) return CUTE_ERR_INVALID_ARG;
+    if (bytes < need) return CUTE_ERR_WORKSPACE_TOO_SMALL;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t np = (size_t)n_ra * n_u;
+    unsigned char *w = (unsigned char *)d_workspace;
+    BuildPlan b;
+    memset(&b, 0, sizeof(b));
+    b.c0 = cat->c0; b.c1 = cat->c1; b.c2 = cat->c0;
+    b.n = cat->n; b.coord = CUTE_COORD_RADEC; b.dtype = cat->dtype; b.mode = CUTE_GRID_SPHERE;
+    b.origin[0] = ra0; b.size[0] = dra; b.origin[1] = u0; b.size[1] = du;
+    b.nc[0] = n_ra; b.nc[1] = n_u; b.nc[2] = 1;
+    b.inv_cell[0] = n_ra / dra; b.inv_cell[1] = n_u / du;
+    b.ncells = (int64_t)np; b.nrows = n_u;
+    b.status = (uint32_t *)w;
+    uint32_t *count = (uint32_t *)(w + 256);
+    uint32_t *pos = (uint32_t *)(w + 256 + align_up((np + 2) * 4, 256));
+    uint32_t *tmp = (uint32_t *)(w + 256 + 2 * align_up((np + 2) * 4, 256));
+    if (run_pixelize(b, count, pos, tmp, d_pix_ra, d_pix_dec, d_pix_weight, s) != cudaSuccess) return CUTE_ERR_CUDA;
+    uint32_t st = 0, m = 0;
+    if (cudaMemcpyAsync(&st, b.status, 4, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+        cudaMemcpyAsync(&m, pos + np, 4, cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
+        return CUTE_ERR_CUDA;
+    if (st) return CUTE_ERR_POINT_OUT_OF_BOX;
+    *npix = (int64_t)m;
+    return CUTE_OK;
+}
+
 int cute_grid_workspace_bytes(const cute_catalog *cat, const cute_grid_spec *spec, size_t *bytes)
 {
     int rc = check_catalog(cat);
@@ -221,6 +267,7 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     BuildPlan b;
     memset(&b, 0, sizeof(b));
     b.c0 = cat->c0; b.c1 = cat->c1; b.c2 = cat->coord == CUTE_COORD_RADEC ? cat->c0 : cat->c2;
+    b.weight = cat->weight;
     b.n = cat->n; b.coord = cat->coord; b.dtype = cat->dtype; b.mode = spec->mode; b.periodic = spec->periodic;
     b.want_lo = want_lo; b.want_f64 = want_f64; b.n_pad = L.n_pad;
     b.hi = (float4 *)(w + L.hi); b.lo = want_lo ? (float4 *)(w + L.lo) : nullptr;
@@ -353,8 +400,8 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     g->maxabs = m;
 
     if (run_build(b, s) != cudaSuccess) { delete g; return CUTE_ERR_CUDA; }
-    uint32_t st[2] = {0, 0};
-    if (cudaMemcpyAsync(st, b.status, 8, cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess) {
+    uint32_t st[3] = {0, 0, 0};
+    if (cudaMemcpyAsync(st, b.status, 12, cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess) {
         delete g;
         return CUTE_ERR_CUDA;
     }
@@ -367,6 +414,7 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     v.n = (uint32_t)cat->n; v.n_pad = L.n_pad; v.nchunks = st[1];
     v.ncx = nc[0]; v.ncy = nc[1]; v.ncz = nc[2];
     g->d_perm = b.perm;
+    g->weighted = cat->weight != nullptr; g->wmax = st[2] > 0 ? st[2] : 1u;
     // algorithmic HBM bytes of the build: read the coordinates twice (cell id,
     // scatter), write hi (+lo, +p64) and perm, cell id cache and rank (write + read: 16 B), counts/scan
     const double in_b = (cat->dtype == CUTE_F64 ? 8.0 : 4.0) * (cat->coord == CUTE_COORD_RADEC ? 2 : 3);
@@ -647,9 +695,22 @@ int cute_count_pairs(int kind, const cute_grid *g1, const cute_grid *g2, const c
         if (kind != CUTE_MONOPOLE || bins->box_L != g1->spec.size[0]) return CUTE_ERR_INVALID_ARG;
     } else if (mode == CUTE_GRID_BOX3D && bins->box_L > 0.0) return CUTE_ERR_INVALID_ARG;
 
+    if (g1->weighted != g2->weighted) return CUTE_ERR_INVALID_ARG;
+    if (g1->weighted && kind != CUTE_ANGULAR) return CUTE_ERR_UNSUPPORTED;
     PairParams p;
     memset(&p, 0, sizeof(p));
     p.g1 = g1->view; p.g2 = g2->view;
+    p.weighted = g1->weighted;
+    p.self_bin = (p.weighted && is_auto && bins->lo1 == 0.0 && !bins->log1) ? 0 : -1;
+    p.epoch_j = kEpochJ;
+    if (p.weighted) {
+        // a uint32 counter receives at most 128 increments of w1max*w2max per j-point; the epoch is checked once
+        // per tile, so one tile of slack is kept (epoch 0 = flush after every tile)
+        const uint64_t per_j = 128ull * g1->wmax * g2->wmax;
+        const uint64_t e = 0xffffffffull / per_j;
+        if (e < (uint64_t)kTile) return CUTE_ERR_OVERFLOW;            // w1max * w2max > 2^18
+        p.epoch_j = (uint32_t)(e - kTile < kEpochJ ? e - kTile : kEpochJ);
+    }
     p.kind = kind; p.is_auto = is_auto; p.mode = mode;
     p.periodic = (mode == CUTE_GRID_BOX3D && g1->spec.periodic) ? 1 : 0;
     p.logbins = bins->log1 ? 1 : 0;
@@ -765,7 +826,7 @@ namespace {
 size_t cat_bytes(const cute_catalog *c)
 {
     const size_t col = align_up((size_t)(c->n > 0 ? c->n : 1) * (c->dtype == CUTE_F64 ? 8 : 4), 256);
-    return col * 3;
+    return col * 3 + (c->weight ? align_up((size_t)(c->n > 0 ? c->n : 1) * 4, 256) : 0);
 }
 
 } // namespace
@@ -819,6 +880,11 @@ int cute_count_pairs_host(int kind, const cute_catalog *cat1, const cute_catalog
             if (!src[d]) *dst[d] = nullptr;
         }
         w += col * 3;
+        if (c->weight) {
+            dc.weight = (const uint32_t *)w;
+            if (c->n > 0 && cudaMemcpyAsync(w, c->weight, (size_t)c->n * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = CUTE_ERR_CUDA;
+            w += align_up((size_t)(c->n > 0 ? c->n : 1) * 4, 256);
+        }
         size_t gw = 0;
         if (rc == CUTE_OK) rc = cute_grid_workspace_bytes(c, spec, &gw);
         if (rc == CUTE_OK) rc = cute_make_grid(&dc, spec, w, gw, stream, &grids[k]);

@@ -47,6 +47,8 @@ struct cute_grid {
     cute_grid_spec spec;      // resolved spec (explicit origin/size/ncell)
     int coord, dtype;
     int has_lo, has_f64;
+    int weighted;             // hi.w holds uint32 weights
+    uint32_t wmax;            // largest weight
     double cell[3];
     double maxabs;            // largest |coordinate| (bound used for the float32 error model)
     int64_t ncells, nrows;
@@ -73,6 +75,9 @@ struct PairParams {
     int logbins;                 // variable 1: 0 linear, 1 log
     int angpoly;                 // ANGULAR linear bins: theta = sqrt(q) * poly(q)
     int always_refine;           // 1: every pair passing the coarse test is recomputed in float64
+    int weighted;                // ANGULAR: pairs count w_i * w_j (uint32 bit patterns in hi.w)
+    int self_bin;                // weighted auto-correlation: bin of zero separation (or -1)
+    uint32_t epoch_j;            // flush a warp's uint32 histogram after this many j-points
     int n1, n2, n2eff, nhist;    // nhist = n1 * n2eff
     int colshift;                // histogram columns per warp copy = 1 << colshift (32, 8 or 1)
     float q_hi;                  // coarse float32 range test on q (padded)
@@ -111,6 +116,7 @@ int plan_pair_kernel(PairParams &p, int want_warps, int want_cols);
 struct BuildPlan {
     // inputs
     const void *c0, *c1, *c2;
+    const uint32_t *weight;       // optional (RADEC only): goes into hi.w as a bit pattern, p64[3] as a double
     int64_t n;
     int coord, dtype, mode, periodic;
     int order_only;    // mode NONE: the cells only ORDER the points (spatially coherent warps); one row, all pairs
@@ -125,12 +131,14 @@ struct BuildPlan {
     uint32_t *perm, *cell_id, *rank, *count, *cell_start, *scan_tmp, *row_nchunks, *row_chunk_start;
     Chunk *chunks;
     int *row_kx, *row_ylo, *row_yhi;
-    uint32_t *status;  // [0] err, [1] nchunks
+    uint32_t *status;  // [0] err, [1] nchunks, [2] largest weight
     double *bbox;      // [6] min xyz, max xyz
     int64_t ncells, nrows;
 };
 cudaError_t run_bbox(const BuildPlan &b, cudaStream_t s);       // leaves 6 order-preserving int64 images in b.bbox
 void decode_bbox(const long long raw[6], double out[6]);
 cudaError_t run_build(const BuildPlan &b, cudaStream_t s);
+cudaError_t run_pixelize(const BuildPlan &b, uint32_t *count, uint32_t *pos, uint32_t *scan_tmp, double *pra, double *pdec,
+                         uint32_t *pw, cudaStream_t s);   // b: SPHERE geometry; pos[ncells] = number of non-empty pixels
 
 } // namespace cute

@@ -266,6 +266,12 @@ __global__ void __launch_bounds__(256) k_scatter(BuildPlan b)
         }
         float h[4], l[4];
         for (int d = 0; d < 4; d++) { h[d] = (float)v[d]; l[d] = (float)(v[d] - (double)h[d]); }
+        if (b.weight) {   // integer weight: bit pattern in hi.w (the pair kernel multiplies integers), exact double in p64
+            const uint32_t w = b.weight[i];
+            h[3] = __uint_as_float(w); l[3] = 0.f; v[3] = (double)w;
+            if (w == 0u || w > 65535u) atomicExch(&b.status[0], 1u);
+            atomicMax(&b.status[2], w);
+        }
         b.hi[slot[k]] = make_float4(h[0], h[1], h[2], h[3]);
         if (b.want_lo) b.lo[slot[k]] = make_float4(l[0], l[1], l[2], l[3]);
         if (b.want_f64) for (int d = 0; d < 4; d++) b.p64[(size_t)d * b.n_pad + slot[k]] = v[d];
@@ -346,7 +352,7 @@ cudaError_t run_build(const BuildPlan &b, cudaStream_t s)
     cudaError_t e;
     const int T = 256;
     const int pblocks = (int)((b.n + (int64_t)T * kPts - 1) / ((int64_t)T * kPts));
-    if ((e = cudaMemsetAsync(b.status, 0, 8, s)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(b.status, 0, 12, s)) != cudaSuccess) return e;
     if (b.mode != CUTE_GRID_NONE) {
         if ((e = cudaMemsetAsync(b.count, 0, (size_t)(b.ncells + 1) * 4, s)) != cudaSuccess) return e;
         if (b.n > 0) { k_cellid<<<pblocks, T, 0, s>>>(b); note_launches(1); }
@@ -359,6 +365,56 @@ cudaError_t run_build(const BuildPlan &b, cudaStream_t s)
     k_chunks<<<(max_chunks + T - 1) / T, T, 0, s>>>(b, max_chunks);
     if (b.mode == CUTE_GRID_SPHERE && !b.order_only) { k_sphere_rows<<<(b.nc[1] + T - 1) / T, T, 0, s>>>(b); note_launches(1); }
     note_launches(2);   // k_row_counts, k_chunks
+    return cudaGetLastError();
+}
+
+// ---- pixel map: count per pixel, compact the non-empty pixels, emit their centres ----------
+__global__ void k_pix_count(BuildPlan b, uint32_t *count)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= b.n) return;
+    double a = load_coord(b.c0, b.dtype, i), c1 = load_coord(b.c1, b.dtype, i);
+    uint32_t id;
+    bool ok = cell_of(b, a, c1, 0.0, id);
+    if (!ok || !isfinite(a) || !isfinite(c1)) { atomicExch(&b.status[0], 1u); return; }
+    atomicAdd(&count[id], 1u);
+}
+
+__global__ void k_pix_flag(const uint32_t *count, int64_t n, uint32_t *flag)
+{
+    int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p < n) flag[p] = count[p] ? 1u : 0u;
+}
+
+__global__ void k_pix_emit(BuildPlan b, const uint32_t *count, const uint32_t *pos, double *pra, double *pdec, uint32_t *pw)
+{
+    int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= b.ncells || !count[p]) return;
+    const int kx = (int)(p % b.nc[0]), ky = (int)(p / b.nc[0]);
+    // a pixel is represented by its centre in (RA, sin Dec)  (reading P1)
+    const double r = b.origin[0] + ((double)kx + 0.5) * (b.size[0] / (double)b.nc[0]);
+    double u = b.origin[1] + ((double)ky + 0.5) * (b.size[1] / (double)b.nc[1]);
+    u = fmin(1.0, fmax(-1.0, u));
+    const uint32_t m = pos[p];
+    pra[m] = fmod(r, 360.0);
+    pdec[m] = asin(u) * (180.0 / kPi);
+    pw[m] = count[p];
+}
+
+cudaError_t run_pixelize(const BuildPlan &b, uint32_t *count, uint32_t *pos, uint32_t *scan_tmp, double *pra, double *pdec,
+                         uint32_t *pw, cudaStream_t s)
+{
+    cudaError_t e;
+    const int T = 256;
+    if ((e = cudaMemsetAsync(b.status, 0, 12, s)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(count, 0, (size_t)b.ncells * 4, s)) != cudaSuccess) return e;
+    if (b.n > 0) { k_pix_count<<<(int)((b.n + T - 1) / T), T, 0, s>>>(b, count); note_launches(1); }
+    const int pb = (int)((b.ncells + T - 1) / T);
+    k_pix_flag<<<pb, T, 0, s>>>(count, b.ncells, pos);
+    // in-place exclusive scan of the flags: pos[p] = output slot, pos[ncells] = number of non-empty pixels
+    if ((e = exclusive_scan(pos, b.ncells, pos, scan_tmp, s)) != cudaSuccess) return e;
+    k_pix_emit<<<pb, T, 0, s>>>(b, count, pos, pra, pdec, pw);
+    note_launches(2);
     return cudaGetLastError();
 }
 

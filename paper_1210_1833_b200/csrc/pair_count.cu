@@ -81,6 +81,11 @@ __device__ __forceinline__ void red_shared(uint32_t addr)
     asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(addr) : "memory");
 }
 
+__device__ __forceinline__ void red_shared_add(uint32_t addr, uint32_t v)
+{
+    asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+
 #define CUTE_MAGIC_F 12582912.0f        /* 1.5 * 2^23: adding it with round-down leaves floor(t) in the mantissa */
 #define CUTE_MAGIC_BITS 0x4B400000
 
@@ -223,6 +228,12 @@ __device__ __forceinline__ void flush_hist(const PairParams &p, const WarpSmem &
     __syncwarp();
 }
 
+// weight of a pair: w_i * w_j for weighted catalogues (pixel maps; bit patterns in hi.w), else 1
+__device__ __forceinline__ uint32_t pair_weight(const PairParams &p, uint32_t i, uint32_t j)
+{
+    return p.weighted ? __float_as_uint(p.g1.hi[i].w) * __float_as_uint(p.g2.hi[j].w) : 1u;
+}
+
 // deferred float64 recomputation of the queued pairs, one per lane
 template <int KIND>
 __device__ __forceinline__ uint32_t drain_refine(const PairParams &p, const WarpSmem &s, int lane)
@@ -234,7 +245,7 @@ __device__ __forceinline__ uint32_t drain_refine(const PairParams &p, const Warp
     for (uint32_t e = lane; e < n; e += 32) {
         uint2 ij = s.rq[e];
         int cell = refine_cell<KIND>(p, ij.x, ij.y);
-        if (cell >= 0) atomicAdd(s.hist + (((uint32_t)cell << p.colshift) + (lane & ((1 << p.colshift) - 1))), 1u);
+        if (cell >= 0) atomicAdd(s.hist + (((uint32_t)cell << p.colshift) + (lane & ((1 << p.colshift) - 1))), pair_weight(p, ij.x, ij.y));
         done++;
     }
     __syncwarp();
@@ -282,7 +293,7 @@ __device__ __noinline__ void push_refine(const PairParams &p, const WarpSmem &s,
         else {
             const int cell = refine_cell<KIND>(p, i, j);
             refined_inline++;
-            if (cell >= 0) atomicAdd(s.hist + (((uint32_t)cell << p.colshift) + hoff), 1u);
+            if (cell >= 0) atomicAdd(s.hist + (((uint32_t)cell << p.colshift) + hoff), pair_weight(p, i, j));
         }
     }
 }
@@ -345,7 +356,7 @@ __device__ __forceinline__ BinOut bin_of(const Consts &c, float q, float wi, flo
 }
 
 // COLS32: one histogram column per lane (compile-time shift); ALWAYS: every candidate pair goes to float64
-template <int KIND, bool MINIMG, bool LOGB, bool MASK, bool COLS32, bool ALWAYS>
+template <int KIND, bool MINIMG, bool LOGB, bool MASK, bool COLS32, bool ALWAYS, bool WEIGHTED>
 __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem &s, const Consts &c, const IPoints &ip,
                                              const float4 *th, const float4 *tl, uint32_t cnt, uint32_t j0,
                                              int lane, uint32_t &refined_inline)
@@ -397,7 +408,9 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
                     acc += o.unsure << (8 * r);   // one byte per pair (unsure <= 5)
                     // P4: private column, no conflict.  A pair that is out of range or uncertain increments the
                     // column's dump row instead: one SEL + one ATOMS, no branch.
-                    red_shared((o.unsure == 0u && o.inr) ? hbase_s + (o.kb << (cs + 2u)) : dump_s);
+                    const uint32_t addr = (o.unsure == 0u && o.inr) ? hbase_s + (o.kb << (cs + 2u)) : dump_s;
+                    if (WEIGHTED) red_shared_add(addr, __float_as_uint(ip.w[r]) * __float_as_uint(pj.w));
+                    else red_shared(addr);
                 }
                 if (acc) {   // rare: queue the uncertain pairs for float64
                     uint32_t need = 0;
@@ -483,7 +496,7 @@ __device__ __forceinline__ void expand_row(const PairParams &p, const Chunk &ch,
 }
 
 // ------------------------------------------------------------------------------- the kernel
-template <int KIND, bool MINIMG, bool LOGB, bool COLS32, bool ALWAYS>
+template <int KIND, bool MINIMG, bool LOGB, bool COLS32, bool ALWAYS, bool WEIGHTED>
 __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_constant__ PairParams p)
 {
     const Consts cst = load_consts(p);
@@ -534,6 +547,18 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
             ip.lx[r] = l.x; ip.ly[r] = l.y; ip.lz[r] = l.z; ip.lw[r] = l.w;
         }
 
+        if (WEIGHTED && p.is_auto && p.self_bin >= 0 && sp == 0) {
+            // the w objects of one pixel are w (w - 1) / 2 pairs at zero separation (reading P2)
+            unsigned long long self = 0;
+#pragma unroll
+            for (int r = 0; r < R; r++)
+                if ((uint32_t)(lane + 32 * r) < ch.i_count) {
+                    const unsigned long long w = __float_as_uint(ip.w[r]);
+                    self += w * (w - 1ull) / 2ull;
+                }
+            for (int o = 16; o; o >>= 1) self += __shfl_xor_sync(0xffffffffu, self, o);
+            if (lane == 0 && self) atomicAdd(p.hist + p.self_bin, self);
+        }
         // x-extent of the chunk (the j-ranges are trimmed to it)
         float xmin = 3.0e38f, xmax = -3.0e38f;
 #pragma unroll
@@ -610,7 +635,7 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
                 }
                 const float4 *th = s.thi + stage * kTile, *tl = s.tlo + stage * kTile;
                 if (seg_mask && t_j0 <= i_last) {
-                    compute_tile<KIND, MINIMG, LOGB, true, COLS32, ALWAYS>(p, s, cst, ip, th, tl, t_cnt, t_j0, lane, refined_inline);
+                    compute_tile<KIND, MINIMG, LOGB, true, COLS32, ALWAYS, WEIGHTED>(p, s, cst, ip, th, tl, t_cnt, t_j0, lane, refined_inline);
 #pragma unroll
                     for (int r = 0; r < R; r++) {
                         if (ip.idx0 + 32u * r <= i_last) {
@@ -619,13 +644,13 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
                         }
                     }
                 } else {
-                    compute_tile<KIND, MINIMG, LOGB, false, COLS32, ALWAYS>(p, s, cst, ip, th, tl, t_cnt, t_j0, lane, refined_inline);
+                    compute_tile<KIND, MINIMG, LOGB, false, COLS32, ALWAYS, WEIGHTED>(p, s, cst, ip, th, tl, t_cnt, t_j0, lane, refined_inline);
                     if (lane == 0) evaluated += (unsigned long long)ch.i_count * t_cnt;
                 }
                 __syncwarp();
                 if (*s.rq_count >= 32u) refined += drain_refine<KIND>(p, s, lane);
                 jepoch += t_cnt;
-                if (jepoch >= kEpochJ) { flush_hist(p, s, lane); flushes++; jepoch = 0; }
+                if (jepoch >= p.epoch_j) { flush_hist(p, s, lane); flushes++; jepoch = 0; }
                 stage ^= 1u;
                 t_j0 = n_j0; t_cnt = n_cnt; t_slot = n_slot; have = have_next;
             }
@@ -676,13 +701,14 @@ int plan_pair_kernel(PairParams &p, int want_warps, int want_cols)
     return -1;
 }
 
-template <int KIND, bool MINIMG, bool LOGB, bool COLS32, bool ALWAYS>
+template <int KIND, bool MINIMG, bool LOGB, bool COLS32, bool ALWAYS, bool WEIGHTED>
 static cudaError_t launch_k(const PairParams &p, int blocks, cudaStream_t s)
 {
     const size_t smem = (size_t)p.smem_per_warp * p.warps;
-    cudaError_t e = cudaFuncSetAttribute(pair_kernel<KIND, MINIMG, LOGB, COLS32, ALWAYS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    auto kern = pair_kernel<KIND, MINIMG, LOGB, COLS32, ALWAYS, WEIGHTED>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    pair_kernel<KIND, MINIMG, LOGB, COLS32, ALWAYS><<<blocks, 32 * p.warps, smem, s>>>(p);
+    kern<<<blocks, 32 * p.warps, smem, s>>>(p);
     note_launches(1);
     return cudaGetLastError();
 }
@@ -690,11 +716,18 @@ static cudaError_t launch_k(const PairParams &p, int blocks, cudaStream_t s)
 template <int KIND, bool MINIMG, bool LOGB>
 static cudaError_t launch_t(const PairParams &p, int blocks, cudaStream_t s)
 {
+    if (p.weighted) {   // pixel maps: ANGULAR only, runtime column count
+        if constexpr (KIND == CUTE_ANGULAR) {
+            if (p.always_refine) return launch_k<KIND, MINIMG, LOGB, false, true, true>(p, blocks, s);
+            return launch_k<KIND, MINIMG, LOGB, false, false, true>(p, blocks, s);
+        }
+        return cudaErrorInvalidValue;
+    }
     // the float64-everything variant (RADIAL, force_refine) is not performance critical: one column layout
-    if (p.always_refine) return launch_k<KIND, MINIMG, LOGB, false, true>(p, blocks, s);
+    if (p.always_refine) return launch_k<KIND, MINIMG, LOGB, false, true, false>(p, blocks, s);
     if (KIND == CUTE_RADIAL) return cudaErrorInvalidValue;
-    return p.colshift == 5 ? launch_k<KIND, MINIMG, LOGB, true, false>(p, blocks, s)
-                           : launch_k<KIND, MINIMG, LOGB, false, false>(p, blocks, s);
+    return p.colshift == 5 ? launch_k<KIND, MINIMG, LOGB, true, false, false>(p, blocks, s)
+                           : launch_k<KIND, MINIMG, LOGB, false, false, false>(p, blocks, s);
 }
 
 cudaError_t launch_pair_kernel(const PairParams &p, int blocks, cudaStream_t s)

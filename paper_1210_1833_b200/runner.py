@@ -28,7 +28,8 @@ def to_device(cat, coord: int, dtype=None):
 class Job:
     """One correlation-function job: catalogues resident on the device, grids built, counters ready."""
 
-    def __init__(self, kind: str, data, rand, bins: dict, grid: dict | None = None, opts: dict | None = None):
+    def __init__(self, kind: str, data, rand, bins: dict, grid: dict | None = None, opts: dict | None = None,
+                 w_data=None, w_rand=None):
         self.kind_name = kind
         self.kind = api.KINDS[kind]
         self.coord = api.COORD_OF_KIND[kind]
@@ -37,6 +38,9 @@ class Job:
         self.opts = api.count_opts(**opts) if opts else None
         self.d_data = to_device(data, self.coord)
         self.d_rand = to_device(rand, self.coord) if rand is not None else None
+        import torch
+        as_w = lambda w: None if w is None else torch.from_numpy(np.ascontiguousarray(w, dtype=np.uint32).view(np.int32)).cuda()
+        self.w_data, self.w_rand = as_w(w_data), as_w(w_rand)      # integer weights (pixel maps), uint32 bits
         self.nd = int(self.d_data[0].numel())
         self.nr = int(self.d_rand[0].numel()) if self.d_rand is not None else 0
         self.counter = api.Counter(self.bins)
@@ -50,7 +54,7 @@ class Job:
             self.spec = api.auto_spec(self.kind_name, self.bins, self.grid, cats, self.coord)
         if self.g_data is not None:
             self.g_data.free()
-        self.g_data = api.cute_make_grid(self.d_data, self.coord, self.spec, workspace=getattr(self, "_ws_d", None))
+        self.g_data = api.cute_make_grid(self.d_data, self.coord, self.spec, workspace=getattr(self, "_ws_d", None), weight=self.w_data)
         self._ws_d = self.g_data.workspace
         if self.d_rand is not None and self.spec.mode == api.GRID_BOX3D:
             # the two grids of a cross-correlation must carry one spec: hand the second build the cell counts
@@ -62,7 +66,7 @@ class Job:
         if self.d_rand is not None:
             if self.g_rand is not None:
                 self.g_rand.free()
-            self.g_rand = api.cute_make_grid(self.d_rand, self.coord, self.spec, workspace=getattr(self, "_ws_r", None))
+            self.g_rand = api.cute_make_grid(self.d_rand, self.coord, self.spec, workspace=getattr(self, "_ws_r", None), weight=self.w_rand)
             self._ws_r = self.g_rand.workspace
         return self
 

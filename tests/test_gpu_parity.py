@@ -368,3 +368,73 @@ def test_fuzz_box_grids(rt, oracle, seed):
         out, job = _run(runner, kind, a, b, bins, dict(mode="none"), which=("DD", "DR"))
     _parity(oracle, out["DD"][0], kind, a, None, bins)
     _parity(oracle, out["DR"][0], kind, a, b, bins)
+
+
+# ------------------------------------------------------------------------------- N2: weights and pixel maps
+@pytest.mark.parametrize("grid", ["none", "sphere"])
+def test_weighted_angular(rt, oracle, grid):
+    """pixel maps: a pair counts w_i w_j, the objects of one pixel w(w-1)/2 pairs at zero separation"""
+    api, runner, synth = rt
+    rng = np.random.default_rng(41)
+    n1, n2 = 3000, 2500
+    c1 = (rng.random(n1) * 8 + 40, rng.random(n1) * 8 - 4)
+    c2 = (rng.random(n2) * 8 + 40, rng.random(n2) * 8 - 4)
+    w1 = rng.integers(1, 7, n1).astype(np.uint32)
+    w2 = rng.integers(1, 5, n2).astype(np.uint32)
+    for bins in (dict(n1=24, lo1=0.0, hi1=math.radians(1.5), log1=0, n2=0, lo2=0.0, hi2=0.0, aperture=0.0, box_L=0.0),
+                 dict(n1=20, lo1=math.radians(0.01), hi1=math.radians(1.5), log1=1, n2=0, lo2=0.0, hi2=0.0, aperture=0.0, box_L=0.0)):
+        g = dict(mode="none") if grid == "none" else dict(mode="sphere", thetamax=bins["hi1"], pix=1.0)
+        job = runner.Job("angular", c1, c2, bins, g, None, w_data=w1, w_rand=w2).build()
+        for which, a, b, wa, wb in (("DD", c1, None, w1, None), ("DR", c1, c2, w1, w2), ("RR", c2, None, w2, None)):
+            h, st = job.count(which)
+            orc = oracle.count("angular", a, b, bins, w1=wa, w2=wb)
+            ok, msg = oracle.parity_ok(h, orc)
+            assert ok, f"{which}: {msg}"
+        job.opts = api.count_opts(force_refine=1)
+        h2, _ = job.count("DR")
+        job.opts = None
+        assert np.array_equal(h2, job.count("DR")[0])
+    # heavy weights: the uint32 shared-memory counters are flushed on a short epoch
+    wb1 = rng.integers(1, 400, n1).astype(np.uint32)
+    job = runner.Job("angular", c1, None, bins, dict(mode="none"), None, w_data=wb1).build()
+    h, st = job.count("DD")
+    orc = oracle.count("angular", c1, None, bins, w1=wb1)
+    ok, msg = oracle.parity_ok(h, orc)
+    assert ok, msg
+    assert st["flushes"] > 148 * 8
+    hh, _ = api.cute_count_pairs_host(api.ANGULAR, c1, None, api.COORD_RADEC, api.grid_spec("none"), bins, w1=wb1)
+    assert np.array_equal(hh, h)
+    with pytest.raises(api.CuteError):
+        runner.Job("angular", c1, None, bins, dict(mode="none"), None, w_data=np.full(n1, 70000, dtype=np.uint32)).build()
+
+
+def test_pixel_map_and_wpix(rt, oracle):
+    """cute_pixelize == the oracle's pixel map (counts exact); w_pix(theta) = weighted counts of the pixel catalogues"""
+    import torch
+    api, runner, synth = rt
+    w = synth.workload(2, 0.1)                                   # 20k clustered + 40k random points
+    tm = math.radians(10.0)
+    ra0, dra, u0, du, nra, nu = 155.0, 50.0, 0.17, 0.75 - 0.17, 500, 380      # ~0.1 deg pixels over the cap
+    cats = {}
+    for name, cat in (("d", w.data), ("r", w.rand)):
+        pra, pdec, pw = oracle.pixelize(cat[0], cat[1], ra0, dra, u0, du, nra, nu)
+        g = api.cute_pixelize([torch.from_numpy(np.ascontiguousarray(c)).cuda() for c in cat[:2]], ra0, dra, u0, du, nra, nu)
+        gra, gdec, gw = (t.cpu().numpy() for t in g)
+        assert np.array_equal(gw.view(np.uint32), pw) and pw.sum() == len(cat[0])
+        assert np.allclose(gra, pra, rtol=0, atol=1e-11) and np.allclose(gdec, pdec, rtol=0, atol=1e-11)
+        cats[name] = ((pra, pdec), pw)
+    assert len(cats["d"][1]) < len(w.data[0])                    # clustered data: several objects per pixel
+    bins = dict(n1=16, lo1=math.radians(0.5), hi1=tm, log1=1, n2=0, lo2=0.0, hi2=0.0, aperture=0.0, box_L=0.0)
+    (cd, wd), (cr, wr) = cats["d"], cats["r"]
+    job = runner.Job("angular", cd, cr, bins, dict(mode="none"), None, w_data=wd, w_rand=wr).build()
+    out = {}
+    for which, a, b, wa, wb in (("DD", cd, None, wd, None), ("DR", cd, cr, wd, wr), ("RR", cr, None, wr, None)):
+        out[which], st = job.count(which)
+        orc = oracle.count("angular", a, b, bins, w1=wa, w2=wb)
+        ok, msg = oracle.parity_ok(out[which], orc)
+        assert ok, f"{which}: {msg}"
+    # and w_pix agrees with the un-pixelised w(theta) above the pixel scale (PAPER.md:233)
+    exact, _ = _run(runner, "angular", w.data, w.rand, bins, dict(mode="none"), which=("DD", "DR", "RR"))
+    xi_pix, _ = api.cute_landy_szalay(out["DD"], out["DR"], out["RR"], len(w.data[0]), len(w.rand[0]))
+    xi, _ = api.cute_landy_szalay(exact["DD"][0], exact["DR"][0], exact["RR"][0], len(w.data[0]), len(w.rand[0]))
+    assert np.max(np.abs(xi_pix - xi)) < 0.02
