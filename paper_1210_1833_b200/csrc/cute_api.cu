@@ -668,18 +668,21 @@ int cute_count_scratch_bytes(const cute_bin_spec *bins, const cute_count_opts *o
     return CUTE_OK;
 }
 
-int cute_count_pairs(int kind, const cute_grid *g1, const cute_grid *g2, const cute_bin_spec *bins, uint64_t *d_hist,
-                     void *d_scratch, size_t scratch_bytes, const cute_count_opts *opts, void *stream)
+// plans (and, unless nitems_out is given, enqueues) one pair count
+static int count_impl(int kind, const cute_grid *g1, const cute_grid *g2, const cute_bin_spec *bins, uint64_t *d_hist,
+                      void *d_scratch, size_t scratch_bytes, const cute_count_opts *opts, void *stream, int64_t *nitems_out)
 {
+    const bool dry = nitems_out != nullptr;
     int rc = check_bins(kind, bins);
     if (rc) return rc;
-    if (!g1 || !d_hist || !d_scratch || ((uintptr_t)d_scratch & 15)) return CUTE_ERR_INVALID_ARG;
+    if (!g1) return CUTE_ERR_INVALID_ARG;
+    if (!dry && (!d_hist || !d_scratch || ((uintptr_t)d_scratch & 15))) return CUTE_ERR_INVALID_ARG;
     if (opts && opts->struct_size != sizeof(cute_count_opts)) return CUTE_ERR_INVALID_ARG;
     const bool is_auto = (g2 == nullptr || g2 == g1);
     if (is_auto) g2 = g1;
     if (!is_auto && !same_spec(g1, g2)) return CUTE_ERR_GRID_MISMATCH;
     const ScratchLayout SL = scratch_layout(bins);
-    if (scratch_bytes < SL.total) return CUTE_ERR_WORKSPACE_TOO_SMALL;
+    if (!dry && scratch_bytes < SL.total) return CUTE_ERR_WORKSPACE_TOO_SMALL;
     cudaStream_t s = (cudaStream_t)stream;
     const int mode = g1->spec.mode;
     // kind / coordinates / grid compatibility
@@ -742,12 +745,15 @@ int cute_count_pairs(int kind, const cute_grid *g1, const cute_grid *g2, const c
     std::vector<double> e((size_t)bins->n1 + 1 + (size_t)bins->n2 + 1);
     fill_edges(bins, 0, e.data());
     if (bins->n2 > 0) fill_edges(bins, 1, e.data() + bins->n1 + 1);
-    if (cudaMemsetAsync(sc, 0, 64, s) != cudaSuccess) return CUTE_ERR_CUDA;
-    if (cudaMemcpyAsync(sc + SL.edges1, e.data(), e.size() * 8, cudaMemcpyHostToDevice, s) != cudaSuccess) return CUTE_ERR_CUDA;
-    if (cudaMemsetAsync(d_hist, 0, (size_t)p.nhist * 8, s) != cudaSuccess) return CUTE_ERR_CUDA;
-    if (p.g1.n == 0 || p.g2.n == 0 || (is_auto && p.g1.n < 2)) return CUTE_OK;   // N in {0,1}: zeros
+    if (!dry) {
+        if (cudaMemsetAsync(sc, 0, 64, s) != cudaSuccess) return CUTE_ERR_CUDA;
+        if (cudaMemcpyAsync(sc + SL.edges1, e.data(), e.size() * 8, cudaMemcpyHostToDevice, s) != cudaSuccess) return CUTE_ERR_CUDA;
+        if (cudaMemsetAsync(d_hist, 0, (size_t)p.nhist * 8, s) != cudaSuccess) return CUTE_ERR_CUDA;
+    }
+    if (p.g1.n == 0 || p.g2.n == 0 || (is_auto && p.g1.n < 2)) { if (dry) *nitems_out = 0; return CUTE_OK; }   // N in {0,1}: zeros
 
     if (plan_pair_kernel(p, opts ? opts->warps : 0, opts ? opts->hist_cols : 0) < 0) return CUTE_ERR_UNSUPPORTED;
+    if (p.hist_shared) p.epoch_j = p.epoch_j / (uint32_t)p.warps > 0 ? p.epoch_j / (uint32_t)p.warps : 1u;   // all warps feed one counter
     const int blocks = (opts && opts->blocks > 0) ? opts->blocks : sm_count();
     // work items: grid mode = chunks; brute force = chunks x j-splits, enough for ~16 items per warp
     uint64_t nitems = p.g1.nchunks;
@@ -764,7 +770,19 @@ int cute_count_pairs(int kind, const cute_grid *g1, const cute_grid *g2, const c
         p.nsplit = (uint32_t)(((uint64_t)p.g2.n + js - 1) / js);
         nitems *= p.nsplit;
     }
+    else {
+        // cell lists: a chunk's neighbour rows are dealt to nsplit items (row nb goes to item nb % nsplit) when the
+        // chunks alone would leave fewer than ~8 items per warp (sparse catalogues: C3 has 4088 chunks for 2368 warps)
+        const uint64_t target = 8ull * (uint64_t)blocks * p.warps;
+        int rows_nb = mode == CUTE_GRID_BOX3D ? (2 * p.ky + 1) * (2 * p.kz + 1) : 3;
+        if (p.is_auto) rows_nb = (rows_nb + 1) / 2;
+        uint64_t ns = nitems > 0 ? (target + nitems - 1) / nitems : 1;
+        ns = ns < 1 ? 1 : (ns > (uint64_t)rows_nb ? (uint64_t)rows_nb : ns);
+        p.nsplit = (uint32_t)ns;
+        nitems *= p.nsplit;
+    }
     if (nitems > 0xfffffff0ull) return CUTE_ERR_OVERFLOW;
+    if (dry) { *nitems_out = (int64_t)nitems; return CUTE_OK; }
     p.item_begin = 0; p.item_end = (uint32_t)nitems;
     if (opts && (opts->item_begin || opts->item_end)) {
         if (opts->item_begin < 0 || opts->item_end < opts->item_begin) return CUTE_ERR_INVALID_ARG;
@@ -776,31 +794,18 @@ int cute_count_pairs(int kind, const cute_grid *g1, const cute_grid *g2, const c
     return CUTE_OK;
 }
 
+int cute_count_pairs(int kind, const cute_grid *g1, const cute_grid *g2, const cute_bin_spec *bins, uint64_t *d_hist,
+                     void *d_scratch, size_t scratch_bytes, const cute_count_opts *opts, void *stream)
+{
+    return count_impl(kind, g1, g2, bins, d_hist, d_scratch, scratch_bytes, opts, stream, nullptr);
+}
+
 int cute_count_items(int kind, const cute_grid *g1, const cute_grid *g2, const cute_bin_spec *bins, const cute_count_opts *opts,
                      int64_t *nitems)
 {
-    // number of work items cute_count_pairs would enumerate (for sharding with item_begin/item_end)
-    if (!g1 || !nitems || !bins) return CUTE_ERR_INVALID_ARG;
-    if (!g2) g2 = g1;
-    uint64_t n = g1->view.nchunks;
-    if (g1->spec.mode == CUTE_GRID_NONE && n > 0 && g2->view.n > 0) {
-        PairParams p;
-        memset(&p, 0, sizeof(p));
-        p.kind = kind;
-        p.nhist = bins->n1 * (bins->n2 > 0 ? bins->n2 : 1);
-        if (plan_pair_kernel(p, opts ? opts->warps : 0, opts ? opts->hist_cols : 0) < 0) return CUTE_ERR_UNSUPPORTED;
-        const int blocks = (opts && opts->blocks > 0) ? opts->blocks : sm_count();
-        const uint64_t target = 16ull * (uint64_t)blocks * p.warps;
-        uint64_t ns = (target + n - 1) / n;
-        const uint64_t max_ns = ((uint64_t)g2->view.n + kTile - 1) / kTile;
-        ns = ns < 1 ? 1 : (ns > max_ns ? max_ns : ns);
-        uint64_t js = ((uint64_t)g2->view.n + ns - 1) / ns;
-        js = (js + kTile - 1) / kTile * kTile;
-        if (js > (1u << 21)) js = 1u << 21;
-        n *= ((uint64_t)g2->view.n + js - 1) / js;
-    }
-    *nitems = (int64_t)n;
-    return CUTE_OK;
+    // number of work items cute_count_pairs enumerates for these arguments (for sharding with item_begin/item_end)
+    if (!nitems) return CUTE_ERR_INVALID_ARG;
+    return count_impl(kind, g1, g2, bins, nullptr, nullptr, 0, opts, nullptr, nitems);
 }
 
 int cute_count_status(void *d_scratch, void *stream, uint64_t stats[4])

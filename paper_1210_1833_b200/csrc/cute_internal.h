@@ -80,6 +80,7 @@ struct PairParams {
     uint32_t epoch_j;            // flush a warp's uint32 histogram after this many j-points
     int n1, n2, n2eff, nhist;    // nhist = n1 * n2eff
     int colshift;                // histogram columns per warp copy = 1 << colshift (32, 8 or 1)
+    int hist_shared;             // 1: one histogram copy per CTA (large 2-D histograms), flushed with atomicExch
     float q_hi;                  // coarse float32 range test on q (padded)
     float dz_hi;                 // RADIAL: coarse test on |dz|
     FastAxis a1, a2;

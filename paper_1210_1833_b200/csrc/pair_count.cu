@@ -202,10 +202,15 @@ __device__ __forceinline__ WarpSmem carve(unsigned char *ws)
     return s;
 }
 
-static inline uint32_t warp_smem_bytes(bool needlo, int nhist, int colshift)
+static inline uint32_t hist_bytes(int nhist, int colshift)
+{
+    return ((((uint32_t)(nhist + 1) << colshift) * 4 + 15) & ~15u);   // + one dump row
+}
+
+static inline uint32_t warp_smem_bytes(bool needlo, int nhist, int colshift, bool shared_hist)
 {
     uint32_t b = kStages * kTileBytes * (needlo ? 2 : 1) + kSegSlots * 16 + kRefineCap * 8 + 32;
-    b += (((uint32_t)(nhist + 1) << colshift) * 4 + 15) & ~15u;   // + one dump row
+    if (!shared_hist) b += hist_bytes(nhist, colshift);
     return (b + 127) & ~127u;
 }
 
@@ -220,8 +225,8 @@ __device__ __forceinline__ void flush_hist(const PairParams &p, const WarpSmem &
         uint32_t *row = s.hist + ((size_t)c << p.colshift);
         for (int k = 0; k < C; k++) {
             int col = (k + lane) & (C - 1);
-            sum += row[col];
-            row[col] = 0;
+            if (p.hist_shared) sum += atomicExch(row + col, 0u);   // other warps keep adding: read-and-clear in one step
+            else { sum += row[col]; row[col] = 0; }
         }
         if (sum) atomicAdd(p.hist + c, sum);
     }
@@ -438,11 +443,11 @@ __device__ __forceinline__ float image_shift(uint32_t code, int axis, float L)
 // around it", with k = ceil(Rmax/a) -- DESIGN.md reading G3; on the sphere the rows
 // and the RA window of the repaired Eq. 16).
 __device__ __forceinline__ void expand_row(const PairParams &p, const Chunk &ch, float xmin, float xmax, int nb, int nrows_nb,
-                                           uint4 *out)
+                                           uint32_t part, uint4 *out)
 {
     uint4 none = make_uint4(0u, 0u, 0u, 0u);
     out[0] = out[1] = out[2] = none;
-    if (nb >= nrows_nb) return;
+    if (nb >= nrows_nb || (uint32_t)nb % p.nsplit != part) return;   // this row belongs to another item of the chunk
     const GridView &g = p.g2;
     const int ncx = g.ncx, ncy = g.ncy, ncz = g.ncz;
     const int cy = (int)(ch.row % (uint32_t)ncy), cz = (int)(ch.row / (uint32_t)ncy);
@@ -503,9 +508,15 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
     constexpr bool NEEDLO = (KIND == CUTE_ANGULAR || KIND == CUTE_RMU || KIND == CUTE_PISIGMA);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const WarpSmem s = carve<NEEDLO>(smem_raw + (size_t)warp * p.smem_per_warp);
+    WarpSmem s = carve<NEEDLO>(smem_raw + (size_t)warp * p.smem_per_warp);
+    if (p.hist_shared) {   // large (2-D) histograms: one copy per CTA, so that more warps fit
+        s.hist = reinterpret_cast<uint32_t *>(smem_raw + (size_t)p.warps * p.smem_per_warp);
+        for (uint32_t k = threadIdx.x; k < (uint32_t)(p.nhist + 1); k += blockDim.x) s.hist[k] = 0;
+        __syncthreads();   // the only block-wide barrier of the kernel, before any work
+    }
 
-    for (uint32_t k = lane; k < ((uint32_t)(p.nhist + 1) << p.colshift); k += 32) s.hist[k] = 0;
+    if (!p.hist_shared)
+        for (uint32_t k = lane; k < ((uint32_t)(p.nhist + 1) << p.colshift); k += 32) s.hist[k] = 0;
     if (lane == 0) {
         for (int k = 0; k < kStages; k++) mbar_init(s.bar[k], 1);
         *s.rq_count = 0;
@@ -586,7 +597,7 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
                 if (lane == 0) s.segs[0] = make_uint4(jb, max(jb, je), code, 0u);
                 nslots = 1;
             } else {
-                expand_row(p, ch, xmin, xmax, nb0 + lane, nrows_nb, s.segs + 3 * lane);
+                expand_row(p, ch, xmin, xmax, nb0 + lane, nrows_nb, sp, s.segs + 3 * lane);
                 nslots = 3 * min(kSegBatch, nrows_nb - nb0);
             }
             __syncwarp();
@@ -684,27 +695,39 @@ int plan_pair_kernel(PairParams &p, int want_warps, int want_cols)
 {
     // Warps hide the latency of the dependent MUFU/FFMA chains and ncu shows throughput growing with the warp
     // count up to 16, while the number of private histogram columns (32, 8, 1) makes no measurable difference
-    // (ATOMS.POPC.INC merges lanes that hit one address): default = 8 columns, as many warps as fit.
+    // (ATOMS.POPC.INC merges lanes that hit one address): default = 8 columns, as many warps as fit.  A histogram
+    // too large for 8 warps with private copies (the 2-D kinds) becomes ONE copy per CTA shared by all its warps.
     const bool needlo = (p.kind == CUTE_ANGULAR || p.kind == CUTE_RMU || p.kind == CUTE_PISIGMA);
+    p.hist_shared = 0;
     const int clist[] = {3, 0, 5};
     for (int ci = 0; ci < 3; ci++) {
         if (want_cols > 0 && (1 << clist[ci]) != want_cols) continue;
-        const uint32_t per = warp_smem_bytes(needlo, p.nhist, clist[ci]);
+        const uint32_t per = warp_smem_bytes(needlo, p.nhist, clist[ci], false);
         int w = (int)((size_t)kSmemBudget / per);
         if (w > kMaxWarps) w = kMaxWarps;
         if (want_warps > 0) { if (want_warps > w) continue; w = want_warps; }
-        else if (want_cols <= 0 && clist[ci] == 3 && w < 8) continue;   // wide histograms: one column
+        else if (want_cols <= 0 && w < kMaxWarps && clist[ci] != 5) continue;   // would cost warps: share instead
+        else if (want_cols <= 0 && clist[ci] == 5) continue;
         if (w < 1) continue;
         p.colshift = clist[ci]; p.warps = w; p.smem_per_warp = per;
         return (int)(per * (uint32_t)w);
     }
-    return -1;
+    if (want_cols > 0) return -1;
+    {   // shared copy, one column
+        const uint32_t per = warp_smem_bytes(needlo, p.nhist, 0, true), hb = hist_bytes(p.nhist, 0);
+        if ((size_t)hb + per > (size_t)kSmemBudget) return -1;
+        int w = (int)(((size_t)kSmemBudget - hb) / per);
+        if (w > kMaxWarps) w = kMaxWarps;
+        if (want_warps > 0) { if (want_warps > w) return -1; w = want_warps; }
+        p.hist_shared = 1; p.colshift = 0; p.warps = w; p.smem_per_warp = per;
+        return (int)(per * (uint32_t)w + hb);
+    }
 }
 
 template <int KIND, bool MINIMG, bool LOGB, bool COLS32, bool ALWAYS, bool WEIGHTED>
 static cudaError_t launch_k(const PairParams &p, int blocks, cudaStream_t s)
 {
-    const size_t smem = (size_t)p.smem_per_warp * p.warps;
+    const size_t smem = (size_t)p.smem_per_warp * p.warps + (p.hist_shared ? hist_bytes(p.nhist, 0) : 0);
     auto kern = pair_kernel<KIND, MINIMG, LOGB, COLS32, ALWAYS, WEIGHTED>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
