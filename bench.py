@@ -403,6 +403,7 @@ def main():
                        f"grid={w.grid.get('mode', 'none')})",
            "scale": args.scale, "l2": "256 MiB buffer written between timed iterations (L2 flush)",
            "parallelism": f"work items sharded over {args.gpus} GPU(s), catalogues replicated, one all-reduce of the histogram"}
+    w.grid = dict(w.grid, no_perm=1)      # pair counting never reads the sort permutation: do not write it
     if args.impl == "reference":
         run_reference(args, w, cfg)
     else:

@@ -100,6 +100,8 @@ typedef struct cute_grid_spec {
     double rmax;
     int kind_mask; /* bit k set: the grid will be used for kind k (CUTE_ANGULAR=0 ...); 0 = any kind the   */
                    /* coordinates allow.  Lets the build skip arrays a kind does not read (the low parts). */
+    int no_perm;   /* != 0: do not write the sorted-slot -> input-index permutation (cute_grid_info.d_perm = NULL); */
+                   /* pair counting never reads it, and it is a random 4-byte store per object                     */
 } cute_grid_spec;
 
 /* Binning.  Variable 1: theta [rad] (ANGULAR), r (MONOPOLE, RMU), zbar (RADIAL), pi (PISIGMA); linear or, if

@@ -30,7 +30,7 @@ class cute_catalog(C.Structure):
 class cute_grid_spec(C.Structure):
     _fields_ = [("struct_size", C.c_size_t), ("mode", C.c_int), ("periodic", C.c_int),
                 ("origin", C.c_double * 3), ("size", C.c_double * 3), ("ncell", C.c_int * 3),
-                ("rmax", C.c_double), ("kind_mask", C.c_int)]
+                ("rmax", C.c_double), ("kind_mask", C.c_int), ("no_perm", C.c_int)]
 
 
 class cute_bin_spec(C.Structure):
@@ -134,10 +134,10 @@ def bin_spec(bins: dict) -> cute_bin_spec:
 
 
 def grid_spec(mode="none", periodic=False, origin=(0, 0, 0), size=(0, 0, 0), ncell=(0, 0, 0), rmax=0.0,
-              kind_mask=0) -> cute_grid_spec:
+              kind_mask=0, no_perm=0) -> cute_grid_spec:
     m = {"none": GRID_NONE, "box3d": GRID_BOX3D, "sphere": GRID_SPHERE}[mode] if isinstance(mode, str) else int(mode)
     return cute_grid_spec(C.sizeof(cute_grid_spec), m, int(bool(periodic)), (C.c_double * 3)(*map(float, origin)),
-                          (C.c_double * 3)(*map(float, size)), (C.c_int * 3)(*map(int, ncell)), float(rmax), int(kind_mask))
+                          (C.c_double * 3)(*map(float, size)), (C.c_int * 3)(*map(int, ncell)), float(rmax), int(kind_mask), int(no_perm))
 
 
 def count_opts(**kw) -> cute_count_opts:
@@ -393,17 +393,18 @@ def auto_spec(kind: str, bins: dict, grid: dict, cats_dev, coord: int) -> cute_g
     cats_dev: the device catalogues that will share the spec (their common bounding box is used)."""
     k = KINDS[kind]
     mode = grid.get("mode", "none")
+    npm = int(grid.get("no_perm", 0))
     if mode == "none":
-        return grid_spec("none", kind_mask=1 << k)
+        return grid_spec("none", kind_mask=1 << k, no_perm=npm)
     if mode == "box3d":
         L = float(bins.get("box_L", 0.0))
         ncell = grid.get("ncell", (0, 0, 0))
         if L > 0:
-            return grid_spec("box3d", periodic=True, size=(L, L, L), rmax=grid["rmax"], ncell=ncell, kind_mask=1 << k)
+            return grid_spec("box3d", periodic=True, size=(L, L, L), rmax=grid["rmax"], ncell=ncell, kind_mask=1 << k, no_perm=npm)
         bb = np.array([cute_catalog_bounds(c, coord) for c in cats_dev if c[0].numel() > 0])
         lo, hi = bb[:, :3].min(axis=0), bb[:, 3:].max(axis=0)
         pad = 1e-6 * np.maximum(hi - lo, 1.0) + 1e-9 * np.maximum(np.abs(lo), np.abs(hi))
-        return grid_spec("box3d", origin=lo - pad, size=(hi - lo) + 2 * pad, rmax=grid["rmax"], ncell=ncell, kind_mask=1 << k)
+        return grid_spec("box3d", origin=lo - pad, size=(hi - lo) + 2 * pad, rmax=grid["rmax"], ncell=ncell, kind_mask=1 << k, no_perm=npm)
     # sphere: pixels with constant limits in (RA, sin Dec); RA must not wrap inside the footprint
     tm = float(grid["thetamax"])
     pix = float(grid.get("pix", 2.0)) * tm                      # pixel side [rad]
@@ -420,4 +421,4 @@ def auto_spec(kind: str, bins: dict, grid: dict, cats_dev, coord: int) -> cute_g
     cmax = np.cos(np.radians(min(abs(de_lo), abs(de_hi)) if de_lo * de_hi > 0 else 0.0))
     nra = int(max(1, min(65535, np.floor(np.radians(dra) * cmax / pix))))
     nu = int(max(1, min(1 << 20, np.floor(du / pix))))
-    return grid_spec("sphere", origin=(ra0, u_lo, 0), size=(dra, du, 0), ncell=(nra, nu, 1), rmax=tm, kind_mask=1 << k)
+    return grid_spec("sphere", origin=(ra0, u_lo, 0), size=(dra, du, 0), ncell=(nra, nu, 1), rmax=tm, kind_mask=1 << k, no_perm=npm)

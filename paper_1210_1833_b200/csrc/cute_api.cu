@@ -33,7 +33,7 @@ inline int sm_count()
 
 // ---- workspace layout of one grid -------------------------------------------------------------
 struct Layout {
-    size_t hi, lo, p64, perm, cell_id, rank, count, cell_start, scan_tmp, row_nchunks, row_chunk_start, chunks,
+    size_t hi, lo, p64, perm, count, cell_start, scan_tmp, row_nchunks, row_chunk_start, chunks,
         row_kx, row_ylo, row_yhi, status, bbox, total;
     uint32_t n_pad;
     int64_t max_cells, max_rows, max_chunks;
@@ -58,8 +58,6 @@ Layout make_layout(int64_t n, int want_lo, int want_f64, int64_t max_cells, int6
     L.lo = want_lo ? take((size_t)L.n_pad * 16) : 0;
     L.p64 = want_f64 ? take((size_t)L.n_pad * 32) : 0;
     L.perm = take((size_t)L.n_pad * 4);
-    L.cell_id = take((size_t)L.n_pad * 4);
-    L.rank = take((size_t)L.n_pad * 4);
     L.count = take((size_t)(max_cells + 2) * 4);
     L.cell_start = take((size_t)(max_cells + 2) * 4);
     int64_t m = max_cells > max_rows ? max_cells : max_rows;
@@ -272,8 +270,7 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     b.want_lo = want_lo; b.want_f64 = want_f64; b.n_pad = L.n_pad;
     b.hi = (float4 *)(w + L.hi); b.lo = want_lo ? (float4 *)(w + L.lo) : nullptr;
     b.p64 = want_f64 ? (double *)(w + L.p64) : nullptr;
-    b.perm = (uint32_t *)(w + L.perm);
-    b.cell_id = (uint32_t *)(w + L.cell_id); b.rank = (uint32_t *)(w + L.rank);
+    b.perm = spec->no_perm ? nullptr : (uint32_t *)(w + L.perm);
     b.count = (uint32_t *)(w + L.count); b.cell_start = (uint32_t *)(w + L.cell_start);
     b.scan_tmp = (uint32_t *)(w + L.scan_tmp); b.row_nchunks = (uint32_t *)(w + L.row_nchunks);
     b.row_chunk_start = (uint32_t *)(w + L.row_chunk_start); b.chunks = (Chunk *)(w + L.chunks);
@@ -416,10 +413,9 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     g->d_perm = b.perm;
     g->weighted = cat->weight != nullptr; g->wmax = st[2] > 0 ? st[2] : 1u;
     // algorithmic HBM bytes of the build: read the coordinates twice (cell id,
-    // scatter), write hi (+lo, +p64) and perm, cell id cache and rank (write + read: 16 B), counts/scan
+    // scatter), write hi (+lo, +p64) and perm; counts, scan and cursors per cell
     const double in_b = (cat->dtype == CUTE_F64 ? 8.0 : 4.0) * (cat->coord == CUTE_COORD_RADEC ? 2 : 3);
-    g->build_bytes = (double)cat->n * (2 * in_b + 16 + (want_lo ? 16 : 0) + (want_f64 ? 32 : 0) + 4 +
-                                       16) + (double)b.ncells * 12;
+    g->build_bytes = (double)cat->n * (2 * in_b + 16 + (want_lo ? 16 : 0) + (want_f64 ? 32 : 0) + (spec->no_perm ? 0 : 4)) + (double)b.ncells * 20;
     *out = g;
     return CUTE_OK;
 }

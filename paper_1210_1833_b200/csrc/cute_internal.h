@@ -129,7 +129,7 @@ struct BuildPlan {
     float4 *hi, *lo;
     double *p64;
     uint32_t n_pad;
-    uint32_t *perm, *cell_id, *rank, *count, *cell_start, *scan_tmp, *row_nchunks, *row_chunk_start;
+    uint32_t *perm, *count, *cell_start, *scan_tmp, *row_nchunks, *row_chunk_start;
     Chunk *chunks;
     int *row_kx, *row_ylo, *row_yhi;
     uint32_t *status;  // [0] err, [1] nchunks, [2] largest weight

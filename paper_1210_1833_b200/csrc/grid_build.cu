@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(256) k_cellid(BuildPlan b)
             if (b.coord != CUTE_COORD_RADEC) c2[k] = load_coord(b.c2, b.dtype, i);
         }
     }
-    uint32_t id[kPts], rk[kPts];
+    uint32_t id[kPts];
     bool bad = false;
 #pragma unroll
     for (int k = 0; k < kPts; k++) {
@@ -136,12 +136,7 @@ __global__ void __launch_bounds__(256) k_cellid(BuildPlan b)
     }
 #pragma unroll
     for (int k = 0; k < kPts; k++)
-        rk[k] = (base + (int64_t)k * blockDim.x < b.n) ? atomicAdd(&b.count[id[k]], 1u) : 0u;   // rank inside the cell (order arbitrary, pin V4)
-#pragma unroll
-    for (int k = 0; k < kPts; k++) {
-        const int64_t i = base + (int64_t)k * blockDim.x;
-        if (i < b.n) { b.cell_id[i] = id[k]; b.rank[i] = rk[k]; }
-    }
+        if (base + (int64_t)k * blockDim.x < b.n) atomicAdd(&b.count[id[k]], 1u);   // cell histogram (no return value: RED)
     if (bad) atomicExch(&b.status[0], 1u);
 }
 
@@ -237,19 +232,20 @@ __global__ void __launch_bounds__(256) k_scatter(BuildPlan b)
         if (i < b.n) {
             a[k] = load_coord(b.c0, b.dtype, i); c1[k] = load_coord(b.c1, b.dtype, i);
             if (b.coord != CUTE_COORD_RADEC) c2[k] = load_coord(b.c2, b.dtype, i);
-            slot[k] = (b.mode == CUTE_GRID_NONE) ? (uint32_t)i : b.cell_id[i];
+            slot[k] = (uint32_t)i;
         }
     }
     if (b.mode != CUTE_GRID_NONE) {
-        uint32_t rk[kPts];
+        // slot = the cell's cursor (a copy of cell_start kept in `count`), advanced atomically: the order inside a
+        // cell is arbitrary and the histogram must not depend on it (pin V4).  The cell id is recomputed from the
+        // coordinates already in registers instead of being cached in HBM.
 #pragma unroll
         for (int k = 0; k < kPts; k++) {
             const int64_t i = base + (int64_t)k * blockDim.x;
-            rk[k] = (i < b.n) ? b.rank[i] : 0u;
-            slot[k] = (i < b.n) ? b.cell_start[slot[k]] : 0u;
+            uint32_t id;
+            cell_of(b, a[k], c1[k], c2[k], id);
+            if (i < b.n) slot[k] = atomicAdd(&b.count[id], 1u);
         }
-#pragma unroll
-        for (int k = 0; k < kPts; k++) slot[k] += rk[k];
     }
 #pragma unroll
     for (int k = 0; k < kPts; k++) {
@@ -275,7 +271,7 @@ __global__ void __launch_bounds__(256) k_scatter(BuildPlan b)
         b.hi[slot[k]] = make_float4(h[0], h[1], h[2], h[3]);
         if (b.want_lo) b.lo[slot[k]] = make_float4(l[0], l[1], l[2], l[3]);
         if (b.want_f64) for (int d = 0; d < 4; d++) b.p64[(size_t)d * b.n_pad + slot[k]] = v[d];
-        b.perm[slot[k]] = (uint32_t)i;
+        if (b.perm) b.perm[slot[k]] = (uint32_t)i;
     }
 }
 
@@ -357,6 +353,8 @@ cudaError_t run_build(const BuildPlan &b, cudaStream_t s)
         if ((e = cudaMemsetAsync(b.count, 0, (size_t)(b.ncells + 1) * 4, s)) != cudaSuccess) return e;
         if (b.n > 0) { k_cellid<<<pblocks, T, 0, s>>>(b); note_launches(1); }
         if ((e = exclusive_scan(b.count, b.ncells, b.cell_start, b.scan_tmp, s)) != cudaSuccess) return e;
+        // the counters become the per-cell write cursors of the scatter
+        if ((e = cudaMemcpyAsync(b.count, b.cell_start, (size_t)b.ncells * 4, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) return e;
     }
     if (b.n > 0) { k_scatter<<<pblocks, T, 0, s>>>(b); note_launches(1); }
     k_row_counts<<<(int)((b.nrows + T - 1) / T), T, 0, s>>>(b);
