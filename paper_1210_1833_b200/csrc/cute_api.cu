@@ -489,6 +489,24 @@ inline double theta_over_chord(double q)
     return 2.0 * asin(fmin(1.0, 0.5 * c)) / c;
 }
 
+// c0 + c1 q + c2 q^2 + c3 q^3 through F at the four Chebyshev nodes of [0, qmax]: a near-minimax cubic, orders of
+// magnitude closer than the Taylor coefficients at the far end of the range (theta up to tens of degrees)
+template <class Fn>
+void fit_cubic(Fn F, double qmax, double c[4])
+{
+    double x[4], d[4];
+    for (int k = 0; k < 4; k++) { x[k] = 0.5 * qmax * (1.0 + cos((2 * k + 1) * kPi / 8.0)); d[k] = F(x[k]); }
+    for (int j = 1; j < 4; j++)                       // Newton divided differences, in place
+        for (int k = 3; k >= j; k--) d[k] = (d[k] - d[k - 1]) / (x[k] - x[k - j]);
+    // expand d0 + d1 (q-x0) + d2 (q-x0)(q-x1) + d3 (q-x0)(q-x1)(q-x2) into monomials (Horner from the top)
+    double p[4] = {d[3], 0.0, 0.0, 0.0};
+    for (int j = 2; j >= 0; j--) {
+        for (int k = 3; k > 0; k--) p[k] = p[k - 1] - x[j] * p[k];   // multiply by (q - x_j)
+        p[0] = -x[j] * p[0] + d[j];
+    }
+    c[0] = p[0]; c[1] = p[1]; c[2] = p[2]; c[3] = p[3];
+}
+
 // The float32 error model.  Fills a1, a2, q_hi, dz_hi.  `tau` bounds |t_float32 - t_exact| in bins;
 // derivation in DESIGN.md "Precision".
 int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid *g2, const cute_bin_spec *b, double tau_scale)
@@ -536,9 +554,17 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
             const double sc = n1 / log(b->hi1 / b->lo1);       // dt = sc * dr/r
             A.S = (float)(0.5 * sc * log(2.0));                // t = sc*ln(r/lo) = (sc ln2 / 2) * log2(q) - sc ln(lo)
             A.O = (float)(-sc * log(b->lo1));
-            tau1 = sc * (e_r / b->lo1 + rel) + 0.5 * sc * log(2.0) * (1.0 / 2097152.0) +
-                   4.0 * kU * (fabs((double)A.S) * 260.0 + fabs((double)A.O) + n1 + 1.0);
-            rpad = b->hi1 * (1.0 + 2.0 * tau1 / sc);
+            if (kind == CUTE_MONOPOLE) {
+                // pair-dependent: tau = tau1 + tau_w / r (kernel), tau_w = sc e_r
+                tau1 = sc * rel + 0.5 * sc * log(2.0) * (1.0 / 2097152.0) +
+                       4.0 * kU * (fabs((double)A.S) * 260.0 + fabs((double)A.O) + n1 + 1.0);
+                A.tau_w = (float)(1.25 * tau_scale * sc * e_r);
+                rpad = b->hi1 * (1.0 + 2.0 * (tau1 + sc * e_r / b->hi1) / sc);
+            } else {
+                tau1 = sc * (e_r / b->lo1 + rel) + 0.5 * sc * log(2.0) * (1.0 / 2097152.0) +
+                       4.0 * kU * (fabs((double)A.S) * 260.0 + fabs((double)A.O) + n1 + 1.0);
+                rpad = b->hi1 * (1.0 + 2.0 * tau1 / sc);
+            }
         } else {
             const double inv = n1 / (b->hi1 - b->lo1);
             A.S = (float)inv;
@@ -583,11 +609,14 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
             A.S = (float)(0.5 * sc * log(2.0));
             A.O = (float)(-sc * log(b->lo1));
             // theta^2 = 4 asin^2(c/2) = q (1 + q/12 + q^2/90 + q^3/560 + ...): the kernel takes log2 of q*poly(q)
-            A.c1 = 1.0f; A.c2 = (float)(1.0 / 12.0); A.c3 = (float)(1.0 / 90.0);
+            // (Taylor: 1, 1/12, 1/90; fitted over the range actually binned instead)
+            double cf[4];
+            fit_cubic([](double q) { const double t = theta_over_chord(q); return t * t; }, fmin(4.0, q_hi * 1.02), cf);
+            A.c1 = (float)cf[0]; A.c2 = (float)cf[1]; A.c3 = (float)cf[2]; A.c4 = (float)cf[3];
             for (int i = 1; i <= NS; i++) {
                 const double q = fmin(4.0, q_hi * 1.02) * (double)i / NS;
                 const double toc = theta_over_chord(q);
-                const double se = (double)A.c1 + q * ((double)A.c2 + q * (double)A.c3);
+                const double se = (double)A.c1 + q * ((double)A.c2 + q * ((double)A.c3 + q * (double)A.c4));
                 series_err = fmax(series_err, 0.5 * sc * fabs(log(toc * toc / se)));
             }
             const double lgmax = fabs(log2(fmax(c_lo * c_lo * 0.25, 1e-37))) + 2.0;
@@ -601,12 +630,15 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
             const double inv = n1 / (b->hi1 - b->lo1);
             A.S = (float)inv;
             A.O = (float)(-b->lo1 * inv);
-            A.c1 = 1.0f; A.c2 = (float)(1.0 / 24.0); A.c3 = (float)(3.0 / 640.0);
+            // (Taylor: 1, 1/24, 3/640; fitted over the range actually binned instead)
+            double cf[4];
+            fit_cubic([](double q) { return theta_over_chord(q); }, fmin(4.0, q_hi * 1.02), cf);
+            A.c1 = (float)cf[0]; A.c2 = (float)cf[1]; A.c3 = (float)cf[2]; A.c4 = (float)cf[3];
             for (int i = 0; i <= NS; i++) {
                 const double q = fmin(4.0, q_hi * 1.02) * (double)i / NS;
                 const double c = sqrt(q);
                 const double ex = c * theta_over_chord(q);
-                const double se = c * ((double)A.c1 + q * ((double)A.c2 + q * (double)A.c3));
+                const double se = c * ((double)A.c1 + q * ((double)A.c2 + q * ((double)A.c3 + q * (double)A.c4)));
                 series_err = fmax(series_err, fabs(ex - se));
             }
             tau1 = inv * (stretch * (e_abs + rel * c_hi) + 1.5 * series_err) + 4.0 * kU * (inv * th_hi + fabs((double)A.O) + n1 + 1.0);

@@ -63,7 +63,7 @@ namespace cute {
 // g = sqrt(q) (linear bins) or log2(q) (log bins).  The pair is binned by the fast path only if
 // floor(t - tau) == floor(t + tau); otherwise it is recomputed in float64.
 struct FastAxis {
-    float S, O, c1, c2, c3;
+    float S, O, c1, c2, c3, c4;
     float tau, tau_w;      // tau_eff = tau + tau_w * w   (w: kind-specific, see pair_count.cu)
     float Oa, Ob;          // O - tau, O + tau
     int n;

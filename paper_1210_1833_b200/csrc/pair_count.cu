@@ -268,7 +268,7 @@ struct IPoints {           // the R i-points of this lane (float32 fast path)
 
 struct Consts {            // loop constants held in registers (not re-read from the constant bank)
     float q_hi, dz_hi, Lf;
-    float S1, Oa1, Ob1, c1, c2, c3;
+    float S1, Oa1, Ob1, c1, c2, c3, c4;
     float O1, tau1, tauw1;     // PISIGMA: the pi axis has a pair-dependent tau too
     float S2, O2, tau2, tauw2;
     uint32_t n1, n2;
@@ -278,7 +278,7 @@ __device__ __forceinline__ Consts load_consts(const PairParams &p)
 {
     Consts c;
     c.q_hi = p.q_hi; c.dz_hi = p.dz_hi; c.Lf = p.Lf;
-    c.S1 = p.a1.S; c.Oa1 = p.a1.Oa; c.Ob1 = p.a1.Ob; c.c1 = p.a1.c1; c.c2 = p.a1.c2; c.c3 = p.a1.c3;
+    c.S1 = p.a1.S; c.Oa1 = p.a1.Oa; c.Ob1 = p.a1.Ob; c.c1 = p.a1.c1; c.c2 = p.a1.c2; c.c3 = p.a1.c3; c.c4 = p.a1.c4;
     c.O1 = p.a1.O; c.tau1 = p.a1.tau; c.tauw1 = p.a1.tau_w;
     c.S2 = p.a2.S; c.O2 = p.a2.O; c.tau2 = p.a2.tau; c.tauw2 = p.a2.tau_w;
     c.n1 = (uint32_t)p.n1; c.n2 = (uint32_t)p.n2;
@@ -331,9 +331,20 @@ __device__ __forceinline__ BinOut bin_of(const Consts &c, float q, float wi, flo
         o.kb = k1 * c.n2 + k2 + (uint32_t)CUTE_MAGIC_BITS;
         return o;
     }
+    if (KIND == CUTE_MONOPOLE && LOGB) {
+        // log bins in r: the absolute float32 error e_r of r is an error e_r / r in ln r, so tau depends on the pair:
+        // tau = a + b / r  (with a fixed tau sized for r = lo every pair would be uncertain when lo << e_r)
+        const float g = fast_lg2(q), w = fast_rsqrt(q);
+        const float t = fmaf(g, c.S1, c.O1), tau = fmaf(w, c.tauw1, c.tau1);
+        const float fa = __fadd_rd(t - tau, CUTE_MAGIC_F), fb = __fadd_rd(t + tau, CUTE_MAGIC_F);
+        o.kb = __float_as_uint(fa);
+        o.unsure = min(__float_as_uint(fb) - __float_as_uint(fa), 15u);   // q = 0: NaN bits, clamped into the byte
+        o.inr = (o.kb - (uint32_t)CUTE_MAGIC_BITS) < c.n1;
+        return o;
+    }
     float g;
     if (KIND == CUTE_ANGULAR) {
-        const float poly = fmaf(q, fmaf(q, c.c3, c.c2), c.c1);
+        const float poly = fmaf(q, fmaf(q, fmaf(q, c.c4, c.c3), c.c2), c.c1);   // cubic fitted on the host over [0, q_hi]
         if (LOGB) g = fast_lg2(q * poly);                      // log2(theta^2), theta^2 = q (1 + q/12 + ...)
         else { const float h = fast_sqrt(q); g = h * poly; }   // theta = c (1 + q/24 + ...)
     } else g = LOGB ? fast_lg2(q) : fast_sqrt(q);

@@ -438,3 +438,19 @@ def test_pixel_map_and_wpix(rt, oracle):
     xi_pix, _ = api.cute_landy_szalay(out["DD"], out["DR"], out["RR"], len(w.data[0]), len(w.rand[0]))
     xi, _ = api.cute_landy_szalay(exact["DD"][0], exact["DR"][0], exact["RR"][0], len(w.data[0]), len(w.rand[0]))
     assert np.max(np.abs(xi_pix - xi)) < 0.02
+
+
+def test_monopole_log_bins_far_from_origin(rt, oracle):
+    """the paper's logarithmic monopole (256 bins, 50 per decade, r < 100) on float64 coordinates of
+    magnitude ~2000: the float32 error of r is far larger than the lowest edge, so tau must depend on the pair"""
+    api, runner, synth = rt
+    w = synth.workload(3, 0.02)
+    bins = dict(n1=256, lo1=100.0 * 10 ** (-256 / 50), hi1=100.0, log1=1, n2=0, lo2=0.0, hi2=0.0, aperture=0.0, box_L=0.0)
+    out, job = _run(runner, "monopole", w.data, w.rand, bins, dict(mode="box3d", rmax=100.0), which=("DD", "DR"))
+    _parity(oracle, out["DD"][0], "monopole", w.data, None, bins, "celled")
+    _parity(oracle, out["DR"][0], "monopole", w.data, w.rand, bins, "celled")
+    assert out["DD"][1]["refined"] < 0.05 * out["DD"][0].sum()      # not everything goes through float64
+    # coincident points (r = 0) are dropped by log bins, exactly as in the oracle
+    x = tuple(np.concatenate([c[:500], c[:500]]) for c in w.data)
+    out2, _ = _run(runner, "monopole", x, None, bins, dict(mode="none"))
+    _parity(oracle, out2["DD"][0], "monopole", x, None, bins)
