@@ -260,7 +260,7 @@ def cute_make_grid(cols, coord: int, spec: cute_grid_spec, stream=None, workspac
     cat, keep = _catalog(cols, coord, True, weight)
     nbytes = cute_grid_workspace_bytes(cat, spec)
     if workspace is None:
-        workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=keep[0].device if keep[0].numel() or True else "cuda")
+        workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=keep[0].device)
     base = workspace.data_ptr()
     off = (-base) % 256
     h = C.c_void_p()
