@@ -108,7 +108,9 @@ typedef struct cute_grid_spec {
  * log1 != 0, logarithmic: e_k = lo1 (hi1/lo1)^(k/n1) ("logarithmic binning").
  * Variable 2 (n2 = 0 for 1-D kinds): mu in [lo2,hi2] (RMU; mu = 1 belongs to the last bin when
  * hi2 >= 1), dz (RADIAL), sigma (PISIGMA; a grid must then have rmax >= sqrt(hi1^2 + hi2^2)); always linear.  aperture_rad: RADIAL only, strict theta < aperture.
- * box_L > 0: periodic box of side L, minimum-image separations (MONOPOLE only; needs hi1 <= L/2). */
+ * box_L > 0: periodic box of side L, minimum-image separations (MONOPOLE only; needs hi1 <= L/2).  Brute force
+ * (grid mode NONE) then needs the catalogues to span at most L per axis (coordinates wrapped into one box side;
+ * else CUTE_ERR_POINT_OUT_OF_BOX); a periodic BOX3D grid needs them inside [0, L). */
 typedef struct cute_bin_spec {
     size_t struct_size;
     int n1; double lo1, hi1; int log1;
@@ -122,7 +124,7 @@ typedef struct cute_count_opts {
     size_t struct_size;
     int blocks;            /* persistent CTAs to launch (default: one per SM)                        */
     int64_t item_begin;    /* shard of the work-item list [item_begin, item_end) handled by this call */
-    int64_t item_end;      /* (0,0 = all). Items partition the pairs, so shards add up exactly       */
+    int64_t item_end;      /* (0,0 with shard == 0 = all). Items partition the pairs, so shards add up exactly */
     double tau_scale;      /* multiplies the refine half-width (>1 refines more pairs; results must   */
                            /* not change).  0 = 1.0                                                   */
     int force_refine;      /* != 0: every in-range pair is recomputed in float64                      */
@@ -130,6 +132,8 @@ typedef struct cute_count_opts {
                            /* the uint32 epoch logic); 0 = only when the epoch bound requires it      */
     int warps;             /* warps per CTA (1,2,4,6,8,12,16); 0 = chosen by the library              */
     int hist_cols;         /* private histogram columns per warp: 32 (one per lane), 8 or 1; 0 = auto */
+    int shard;             /* != 0: [item_begin, item_end) is honoured even when it is empty (a rank whose   */
+                           /* share of the items is [0,0) counts nothing instead of everything)               */
 } cute_count_opts;
 
 /* Facts about a built grid (for tests and reports). */
@@ -215,6 +219,16 @@ int cute_host_workspace_bytes(const cute_catalog *cat1, const cute_catalog *cat2
 int cute_count_pairs_host(int kind, const cute_catalog *cat1, const cute_catalog *cat2, const cute_grid_spec *spec,
                           const cute_bin_spec *bins, const cute_count_opts *opts, uint64_t *h_hist, void *d_workspace,
                           size_t bytes, void *stream);
+
+/* Microbenchmarks of the units the pair kernel's roofline is made of (FP32 / packed FP32x2 /
+ * integer issue rates, MUFU, shared-memory atomics versus same-address multiplicity, broadcast LDS, and mixes that
+ * show which instructions share an issue port).  One persistent 512-thread CTA per SM, timed with clock64() inside the
+ * kernels.  Outputs (HOST, n >= cute_peak_count() entries each): lane-operations per clock per SM (a packed f32x2
+ * instruction counts 2 per lane) and warp-instructions per clock per SM (may be NULL); cute_peak_name(k) names entry k.
+ * d_tmp: DEVICE scratch, 256-byte aligned, >= 1 MiB.  Synchronises the stream. */
+int cute_peak_count(void);
+const char *cute_peak_name(int idx);
+int cute_measure_peaks(double *lane_ops_per_clk_sm, double *instr_per_clk_sm, int n, void *d_tmp, size_t bytes, void *stream);
 
 /* ---- host-side helpers (all pointers HOST) ---- */
 /* Bin edges, the single definition: n+1 doubles for axis 0 or 1. */

@@ -42,7 +42,7 @@ class cute_bin_spec(C.Structure):
 class cute_count_opts(C.Structure):
     _fields_ = [("struct_size", C.c_size_t), ("blocks", C.c_int), ("item_begin", C.c_int64),
                 ("item_end", C.c_int64), ("tau_scale", C.c_double), ("force_refine", C.c_int),
-                ("flush_items", C.c_int), ("warps", C.c_int), ("hist_cols", C.c_int)]
+                ("flush_items", C.c_int), ("warps", C.c_int), ("hist_cols", C.c_int), ("shard", C.c_int)]
 
 
 class cute_grid_info(C.Structure):
@@ -58,7 +58,8 @@ class cute_grid_info(C.Structure):
 SYMBOLS = ["cute_version", "cute_strerror", "cute_launch_count", "cute_catalog_bounds", "cute_pixelize_workspace_bytes", "cute_pixelize", "cute_grid_workspace_bytes", "cute_make_grid", "cute_free_grid",
            "cute_grid_get_info", "cute_count_scratch_bytes", "cute_count_pairs", "cute_count_items",
            "cute_count_status", "cute_host_workspace_bytes", "cute_count_pairs_host", "cute_bin_edges",
-           "cute_landy_szalay", "cute_natural_estimator", "cute_multipoles", "cute_periodic_rr", "cute_periodic_xi"]
+           "cute_landy_szalay", "cute_natural_estimator", "cute_multipoles", "cute_periodic_rr", "cute_periodic_xi",
+           "cute_peak_count", "cute_peak_name", "cute_measure_peaks"]
 
 
 def _load() -> C.CDLL:
@@ -89,6 +90,10 @@ def _load() -> C.CDLL:
                                               C.POINTER(cute_bin_spec), C.POINTER(C.c_size_t)]
     lib.cute_count_pairs_host.argtypes = [C.c_int, C.POINTER(cute_catalog), C.POINTER(cute_catalog), C.POINTER(cute_grid_spec),
                                           C.POINTER(cute_bin_spec), C.POINTER(cute_count_opts), up, vp, C.c_size_t, vp]
+    lib.cute_peak_count.restype = C.c_int
+    lib.cute_peak_name.restype = C.c_char_p
+    lib.cute_peak_name.argtypes = [C.c_int]
+    lib.cute_measure_peaks.argtypes = [dp, dp, C.c_int, vp, C.c_size_t, vp]
     lib.cute_bin_edges.argtypes = [C.POINTER(cute_bin_spec), C.c_int, dp]
     lib.cute_landy_szalay.argtypes = [up, up, up, C.c_uint64, C.c_uint64, C.c_int, dp]
     lib.cute_natural_estimator.argtypes = [up, up, C.c_uint64, C.c_uint64, C.c_int, dp]
@@ -382,6 +387,18 @@ def cute_periodic_xi(dd, n: int, L: float, bins: dict):
     xi = np.zeros(b.n1)
     rc = _check(lib.cute_periodic_xi(_up(dd), int(n), float(L), C.byref(b), _dp(xi)), "cute_periodic_xi")
     return xi, rc
+
+
+def cute_measure_peaks(stream=None) -> dict:
+    """{name: (lane-operations per clock per SM, warp-instructions per clock per SM)} measured on the current device."""
+    torch = _torch()
+    n = int(lib.cute_peak_count())
+    ops, ins = np.zeros(n), np.zeros(n)
+    tmp = torch.empty((1 << 20) + 256, dtype=torch.uint8, device="cuda")
+    off = (-tmp.data_ptr()) % 256
+    _check(lib.cute_measure_peaks(_dp(ops), _dp(ins), n, C.c_void_p(tmp.data_ptr() + off), tmp.numel() - off,
+                                  C.c_void_p(_stream_ptr(stream))), "cute_measure_peaks")
+    return {lib.cute_peak_name(k).decode(): (float(ops[k]), float(ins[k])) for k in range(n)}
 
 
 # ------------------------------------------------------------------------------- workload convenience

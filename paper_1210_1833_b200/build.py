@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcute_b200.so")
-SOURCES = ["cute_api.cu", "grid_build.cu", "pair_count.cu"]
+SOURCES = ["cute_api.cu", "grid_build.cu", "pair_count.cu", "peaks.cu"]
 HEADERS = [os.path.join(CSRC, "cute_internal.h"), os.path.join(HERE, "..", "include", "cute_b200.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]

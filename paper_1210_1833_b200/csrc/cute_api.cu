@@ -395,6 +395,8 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     if (cat->coord == CUTE_COORD_XYZ) for (int d = 0; d < 6; d++) m = fmax(m, fabs(bbox[d]));
     else m = fmax(fabs(bbox[2]), fabs(bbox[5]));   // RADECZ: |z| (unit vectors are <= 1)
     g->maxabs = m;
+    for (int d = 0; d < 6; d++) g->bbox[d] = bbox[d];
+    g->has_bbox = need_bbox ? 1 : 0;
 
     if (run_build(b, s) != cudaSuccess) { delete g; return CUTE_ERR_CUDA; }
     uint32_t st[3] = {0, 0, 0};
@@ -726,6 +728,14 @@ static int count_impl(int kind, const cute_grid *g1, const cute_grid *g2, const 
         if (kind != CUTE_MONOPOLE || bins->box_L != g1->spec.size[0]) return CUTE_ERR_INVALID_ARG;
     } else if (mode == CUTE_GRID_BOX3D && bins->box_L > 0.0) return CUTE_ERR_INVALID_ARG;
 
+    if (mode == CUTE_GRID_NONE && bins->box_L > 0.0 && g1->view.n > 0 && g2->view.n > 0) {
+        // the float32 fast path takes the minimum image as min(|d|, L - |d|), which needs |d| <= L: refuse
+        // catalogues that span more than one box side (unwrapped coordinates) instead of binning them wrongly
+        for (int d = 0; d < 3; d++) {
+            const double lo = fmin(g1->bbox[d], g2->bbox[d]), hi = fmax(g1->bbox[3 + d], g2->bbox[3 + d]);
+            if (!g1->has_bbox || !g2->has_bbox || !(hi - lo <= bins->box_L)) return CUTE_ERR_POINT_OUT_OF_BOX;
+        }
+    }
     if (g1->weighted != g2->weighted) return CUTE_ERR_INVALID_ARG;
     if (g1->weighted && kind != CUTE_ANGULAR) return CUTE_ERR_UNSUPPORTED;
     PairParams p;
@@ -762,6 +772,8 @@ static int count_impl(int kind, const cute_grid *g1, const cute_grid *g2, const 
         p.ax = (float)g1->cell[0]; p.ay = (float)g1->cell[1]; p.az = (float)g1->cell[2];
         p.rmax2 = (float)(rr * rr * 1.001);
         p.ox = (float)g1->spec.origin[0]; p.inv_ax = (float)(1.0 / g1->cell[0]);
+        // the trim is float32 arithmetic on float32 coordinates: cover its rounding (a few ulp of the largest |x|)
+        p.trim_pad = (float)(16.0 * kU * (fmax(g1->maxabs, g2->maxabs) + fabs(g1->spec.origin[0]) + rr));
     }
     if (mode == CUTE_GRID_SPHERE) p.ring = g1->spec.size[0] >= 360.0 ? 1 : 0;
 
@@ -781,7 +793,16 @@ static int count_impl(int kind, const cute_grid *g1, const cute_grid *g2, const 
     if (p.g1.n == 0 || p.g2.n == 0 || (is_auto && p.g1.n < 2)) { if (dry) *nitems_out = 0; return CUTE_OK; }   // N in {0,1}: zeros
 
     if (plan_pair_kernel(p, opts ? opts->warps : 0, opts ? opts->hist_cols : 0) < 0) return CUTE_ERR_UNSUPPORTED;
-    if (p.hist_shared) p.epoch_j = p.epoch_j / (uint32_t)p.warps > 0 ? p.epoch_j / (uint32_t)p.warps : 1u;   // all warps feed one counter
+    if (p.hist_shared) {
+        // all warps feed one counter, and each of them may overshoot its share by one tile before it checks
+        if (p.weighted) {
+            const uint64_t per_j = 128ull * g1->wmax * g2->wmax;
+            const uint64_t e = 0xffffffffull / per_j;
+            if (e < (uint64_t)kTile * (uint64_t)p.warps + (uint64_t)p.warps) return CUTE_ERR_OVERFLOW;
+            const uint64_t share = (e - (uint64_t)kTile * (uint64_t)p.warps) / (uint64_t)p.warps;
+            p.epoch_j = (uint32_t)(share < (uint64_t)p.epoch_j ? share : (uint64_t)p.epoch_j);
+        } else p.epoch_j = p.epoch_j / (uint32_t)p.warps > 0 ? p.epoch_j / (uint32_t)p.warps : 1u;
+    }
     const int blocks = (opts && opts->blocks > 0) ? opts->blocks : sm_count();
     // work items: grid mode = chunks; brute force = chunks x j-splits, enough for ~16 items per warp
     uint64_t nitems = p.g1.nchunks;
@@ -812,7 +833,7 @@ static int count_impl(int kind, const cute_grid *g1, const cute_grid *g2, const 
     if (nitems > 0xfffffff0ull) return CUTE_ERR_OVERFLOW;
     if (dry) { *nitems_out = (int64_t)nitems; return CUTE_OK; }
     p.item_begin = 0; p.item_end = (uint32_t)nitems;
-    if (opts && (opts->item_begin || opts->item_end)) {
+    if (opts && (opts->shard || opts->item_begin || opts->item_end)) {
         if (opts->item_begin < 0 || opts->item_end < opts->item_begin) return CUTE_ERR_INVALID_ARG;
         p.item_begin = (uint32_t)(opts->item_begin < (int64_t)nitems ? opts->item_begin : (int64_t)nitems);
         p.item_end = (uint32_t)(opts->item_end < (int64_t)nitems ? opts->item_end : (int64_t)nitems);

@@ -51,6 +51,8 @@ struct cute_grid {
     uint32_t wmax;            // largest weight
     double cell[3];
     double maxabs;            // largest |coordinate| (bound used for the float32 error model)
+    double bbox[6];           // min xyz, max xyz of the raw coordinates (zeros when not computed)
+    int has_bbox;
     int64_t ncells, nrows;
     const uint32_t *d_perm;
     double build_bytes;
@@ -94,6 +96,7 @@ struct PairParams {
     float ax, ay, az;            // cell sizes
     float ox, inv_ax;            // BOX3D: origin and 1/cell along x
     float rmax2;                 // row-pruning radius^2 (padded)
+    float trim_pad;              // added to the x half-width of a trimmed row: float32 rounding of the trim itself
     int ring;                    // SPHERE: RA axis covers 360 deg (neighbour window wraps)
     // work
     uint32_t *queue;             // [0] next item

@@ -19,9 +19,9 @@
 //    1.5*2^23.  The bin is taken from float32 only if floor(t-tau) == floor(t+tau), tau = a bound on
 //    the float32 error; otherwise the pair is queued and recomputed in float64 (the definition), so
 //    the histogram equals the float64 definition except at float64-rounding distance of an edge.
-//  * histogram: per-warp private uint32 copies in shared memory, one COLUMN PER LANE when it fits
-//    ([bin][lane]: conflict-free by construction), flushed to the uint64 global histogram with
-//    64-bit atomics before 2^32 increments can accumulate and at the end.
+//  * histogram: per-warp private uint32 copies in shared memory, [bin][column] with 8, 32 or 1 columns per
+//    warp (a 2-D histogram too large for that is kept once per CTA), flushed to the uint64 global
+//    histogram with 64-bit atomics before 2^32 increments can accumulate and at the end.
 #include "cute_internal.h"
 #include <math.h>
 
@@ -482,7 +482,7 @@ __device__ __forceinline__ void expand_row(const PairParams &p, const Chunk &ch,
         if (my * my + mz * mz > p.rmax2) return;
         // ... and trim the row's cells the same way: only x within w = sqrt(rmax^2 - my^2 - mz^2) of the chunk's
         // own x-extent can hold a pair (rmax2 is padded by 0.1 %, far above the float32 rounding here)
-        const float w = sqrtf(p.rmax2 - (my * my + mz * mz));
+        const float w = sqrtf(p.rmax2 - (my * my + mz * mz)) + p.trim_pad;
         lo_x = (int)floorf((xmin - w - p.ox) * p.inv_ax);
         hi_x = (int)floorf((xmax + w - p.ox) * p.inv_ax);
         y = cy + dy; z = cz + dz;
@@ -505,7 +505,19 @@ __device__ __forceinline__ void expand_row(const PairParams &p, const Chunk &ch,
     } else if (a0 <= a1) {
         out[0] = make_uint4(cs[a0], cs[a1 + 1], code, 0u);
     }
-    if (wrapx) {
+    if (wrapx && self && p.mode == CUTE_GRID_SPHERE) {
+        // Own row on a ring: a pair is the SAME chord whichever way round the ring it is found, so it must be met
+        // exactly once -- by the chunk of its lower sorted index.  Besides the masked direct range above, that chunk
+        // takes the cells near the END of the ring that reach its low cells through the seam (all later in sorted
+        // order, hence unmasked), clipped to start after the direct range; no chunk looks backwards through the seam.
+        // (Decided per pair, not per chunk: a chunk whose window covers the whole ring simply gets the rest of the row.)
+        if (lo < 0) {
+            const int s0 = max(lo + ncx, a1 + 1);
+            if (s0 <= ncx - 1) out[1] = make_uint4(cs[s0], cs[ncx], code, 0u);
+        }
+    } else if (wrapx) {
+        // BOX3D: the wrapped ranges are met through a periodic IMAGE (a different separation; at most one of the
+        // images is within rmax because ncx >= 2k+1), so the direct and the wrapped range may hold the same point
         if (lo < 0 && !self) out[1] = make_uint4(cs[max(ncx + lo, 0)], cs[ncx], code | (p.mode == CUTE_GRID_SPHERE ? 0u : 1u), 0u);
         if (hi >= ncx) out[2] = make_uint4(cs[0], cs[min(hi - ncx, ncx - 1) + 1], code | (p.mode == CUTE_GRID_SPHERE ? 0u : 2u), 0u);
     }
