@@ -122,7 +122,7 @@ void wants(const cute_catalog *c, const cute_grid_spec *s, int *want_lo, int *wa
         *want_lo = (mask == 0) || (mask & ((1 << CUTE_RMU) | (1 << CUTE_PISIGMA)));
         *want_f64 = c->dtype == CUTE_F64;
     } else {
-        *want_lo = (mask == 0) || (mask & (1 << CUTE_ANGULAR));
+        *want_lo = 0;    // the angular fast path reads the float32 unit vectors only; tiny angles go to float64
         *want_f64 = 1;   // unit vectors are computed in float64 whatever the input type
     }
 }
@@ -396,7 +396,7 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     else m = fmax(fabs(bbox[2]), fabs(bbox[5]));   // RADECZ: |z| (unit vectors are <= 1)
     g->maxabs = m;
     for (int d = 0; d < 6; d++) g->bbox[d] = bbox[d];
-    g->has_bbox = need_bbox ? 1 : 0;
+    g->has_bbox = (need_bbox || box_given) ? 1 : 0;
 
     if (run_build(b, s) != cudaSuccess) { delete g; return CUTE_ERR_CUDA; }
     uint32_t st[3] = {0, 0, 0};
@@ -546,9 +546,11 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
         A.c3 = (float)(inv2 * rmaxp * 1.01);
         const double rpad = (rmaxp * (1.0 + 1e-4) + e_r) * (1.0 + 16.0 * kU);
         p.q_hi = (float)(rpad * rpad * (1.0 + 8.0 * kU));
+        if (b->lo1 == 0.0 && b->lo2 == 0.0) p.simple = 1;
     } else if (kind == CUTE_MONOPOLE || kind == CUTE_RMU) {
         // error of one separation component: input rounding, subtraction rounding, periodic image
-        double e_d = (f64in ? 2.0 * kU * M : 0.0) + kU * (minimg ? b->box_L : b->hi1 * 1.01);
+        // (minimum image by d - L rint(d/L): a d within rounding of L/2 may take the other image, |d'| off by <= 2uL)
+        double e_d = (f64in ? 2.0 * kU * M : 0.0) + kU * (minimg ? 3.0 * b->box_L : b->hi1 * 1.01);
         if (p.periodic && !minimg) e_d += 2.0 * kU * 2.0 * b->box_L;
         const double e_r = sqrt(3.0) * e_d;                    // | |d+e| - |d| | <= |e|
         const double rel = 8.0 * kU;                           // q accumulation + MUFU sqrt/lg2
@@ -587,9 +589,26 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
             // |l|^2 = 2(|x_i|^2 + |x_j|^2) - q cancels when |l| << |x| (a catalogue around the origin): its
             // error 8u 3M^2 enters mu as mu * 4u 3M^2 / |l|^2, and 1/|l|^2 = w^2 q in the kernel
             A.c1 = (float)(1.25 * tau_scale * inv2 * 4.0 * kU * (3.0 * M * M + 1.0));
-        }
+            // A catalogue far from the origin (every survey footprint): |l| = |2 x_i + (x_j - x_i)| >= 2 dmin - r, so the
+            // |l|^-2 term is bounded by a constant and folded into tau; with bins from 0 this is the PK_SIMPLE variant
+            auto dmin = [](const cute_grid *g) {
+                double d2 = 0.0;
+                for (int d = 0; d < 3; d++) {
+                    const double lo = g->bbox[d], hi = g->bbox[3 + d];
+                    const double a = lo > 0.0 ? lo : (hi < 0.0 ? -hi : 0.0);
+                    d2 += a * a;
+                }
+                return g->has_bbox ? sqrt(d2) : 0.0;
+            };
+            const double lmin = 2.0 * fmax(dmin(g1), dmin(g2)) * (1.0 - 1e-6) - sqrt((double)p.q_hi) * 1.001;
+            if (lmin > 0.0 && b->lo1 == 0.0 && b->lo2 == 0.0) {
+                B.tau = (float)((double)B.tau + (double)A.c1 / (lmin * lmin) * 1.001);
+                p.simple = 1;
+            }
+        } else if (b->lo1 == 0.0 && !b->log1) p.simple = 1;
     } else {
-        // unit vectors.  ANGULAR: hi/lo pairs, |dd| <= 3u|d| + sqrt3 2^-47 ; RADIAL: coarse test only.
+        // unit vectors.  ANGULAR: float32 components (each within u of the float64 one), so the chord carries an
+        // ABSOLUTE error sqrt3 * 2u ~ 2e-7; RADIAL: coarse test only.
         const double th_hi = kind == CUTE_ANGULAR ? b->hi1 : b->aperture_rad;
         const double c_hi = chord_of(th_hi), q_hi = c_hi * c_hi;
         if (kind == CUTE_RADIAL) {
@@ -600,7 +619,7 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
             return CUTE_OK;
         }
         const double c_lo = chord_of(b->lo1 > 0.0 ? b->lo1 : 0.0);
-        const double e_abs = sqrt(3.0) * ldexp(1.0, -46);
+        const double e_abs = sqrt(3.0) * 2.0 * kU * 1.001;
         const double stretch = 1.0 / sqrt(fmax(1e-6, 1.0 - 0.25 * q_hi));     // d theta / d chord
         const double rel = 12.0 * kU;
         const int NS = 4096;
@@ -621,8 +640,17 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
                 const double se = (double)A.c1 + q * ((double)A.c2 + q * ((double)A.c3 + q * (double)A.c4));
                 series_err = fmax(series_err, 0.5 * sc * fabs(log(toc * toc / se)));
             }
-            const double lgmax = fabs(log2(fmax(c_lo * c_lo * 0.25, 1e-37))) + 2.0;
-            tau1 = sc * stretch * (e_abs / fmax(c_lo, 1e-18) + rel) + (double)A.S * (1.0 / 2097152.0 + 2.0 * kU * lgmax) +
+            // The absolute chord error is a RELATIVE error e_abs / c of theta: pairs closer than c_min always go to
+            // float64 (kernel: q < q_small), the others carry tau ~ sc e_abs / c_min.  For a uniform density the number
+            // of always-refined pairs grows as c_min^2 and the number of near-edge pairs as 1 / c_min: the total is
+            // least at c_min^3 = sc e_abs c_hi^2.  Below lo nothing can be mis-binned INTO range as long as lo >> e_abs.
+            if (c_lo < 16.0 * e_abs) p.always_refine = 1;          // (bins finer than the float32 unit vectors resolve)
+            double c_min = cbrt(sc * stretch * e_abs * c_hi * c_hi);
+            c_min = fmin(c_min, 0.5 * c_hi);
+            if (c_min <= c_lo) { c_min = c_lo; p.q_small = 0.f; }
+            else { const double cs = c_min * 1.001 + 2.0 * e_abs; p.q_small = (float)(cs * cs * (1.0 + 16.0 * kU)); }
+            const double lgmax = fabs(log2(fmax(c_min * c_min * 0.25, 1e-37))) + 2.0;
+            tau1 = sc * stretch * (e_abs / fmax(c_min, 1e-18) + rel) + (double)A.S * (1.0 / 2097152.0 + 2.0 * kU * lgmax) +
                    4.0 * kU * ((double)A.S * lgmax + fabs((double)A.O) + n1 + 1.0) + 1.5 * series_err;
             tau1 *= 1.25 * tau_scale;
             const double cp = chord_of(fmin(kPi, b->hi1 * (1.0 + 2.0 * tau1 / sc))) * (1.0 + 32.0 * kU) + e_abs;
@@ -650,6 +678,7 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
             p.angpoly = 1;
         }
         if (p.q_hi >= 4.0f) p.q_hi = 5.0f;   // whole sphere in range
+        if (tau1 > 0.2) p.always_refine = 1;  // bins too fine for float32 unit vectors: everything in float64
     }
     A.tau = (float)tau1;
     A.Oa = (float)((double)A.O - tau1);
@@ -719,7 +748,7 @@ static int count_impl(int kind, const cute_grid *g1, const cute_grid *g2, const 
     const bool xyz = g1->coord == CUTE_COORD_XYZ;
     if ((kind == CUTE_MONOPOLE || kind == CUTE_RMU || kind == CUTE_PISIGMA) != xyz) return CUTE_ERR_INVALID_ARG;
     if (kind == CUTE_RADIAL && (g1->coord != CUTE_COORD_RADECZ || g2->coord != CUTE_COORD_RADECZ)) return CUTE_ERR_INVALID_ARG;
-    if ((kind == CUTE_ANGULAR || kind == CUTE_RMU || kind == CUTE_PISIGMA) && (!g1->has_lo || !g2->has_lo)) return CUTE_ERR_INVALID_ARG;
+    if ((kind == CUTE_RMU || kind == CUTE_PISIGMA) && (!g1->has_lo || !g2->has_lo)) return CUTE_ERR_INVALID_ARG;
     if ((kind == CUTE_RMU || kind == CUTE_PISIGMA) && mode == CUTE_GRID_BOX3D && g1->spec.periodic) return CUTE_ERR_UNSUPPORTED;
     const double vmax = kind == CUTE_RADIAL ? bins->aperture_rad
                                            : (kind == CUTE_PISIGMA ? sqrt(bins->hi1 * bins->hi1 + bins->hi2 * bins->hi2) : bins->hi1);
@@ -756,6 +785,7 @@ static int count_impl(int kind, const cute_grid *g1, const cute_grid *g2, const 
     p.periodic = (mode == CUTE_GRID_BOX3D && g1->spec.periodic) ? 1 : 0;
     p.logbins = bins->log1 ? 1 : 0;
     p.n1 = bins->n1; p.n2 = bins->n2; p.n2eff = bins->n2 > 0 ? bins->n2 : 1; p.nhist = p.n1 * p.n2eff;
+    p.n2p = bins->n2 > 0 ? bins->n2 + 2 : 1; p.nhist_pad = (p.n1 + 2) * p.n2p;   // dump borders (pair_kernel.cuh)
     p.lo1 = bins->lo1; p.hi1 = bins->hi1; p.lo2 = bins->lo2; p.hi2 = bins->hi2;
     p.L = kind == CUTE_MONOPOLE ? bins->box_L : 0.0; p.aperture = bins->aperture_rad;
     p.Lf = (float)p.L;
@@ -797,7 +827,7 @@ static int count_impl(int kind, const cute_grid *g1, const cute_grid *g2, const 
         // all warps feed one counter, and each of them may overshoot its share by one tile before it checks
         if (p.weighted) {
             const uint64_t per_j = 128ull * g1->wmax * g2->wmax;
-            const uint64_t e = 0xffffffffull / per_j;
+            const uint64_t e = 0x7fffffffull / per_j;   // (the shared copy is read as a signed 32-bit number: undone increments)
             if (e < (uint64_t)kTile * (uint64_t)p.warps + (uint64_t)p.warps) return CUTE_ERR_OVERFLOW;
             const uint64_t share = (e - (uint64_t)kTile * (uint64_t)p.warps) / (uint64_t)p.warps;
             p.epoch_j = (uint32_t)(share < (uint64_t)p.epoch_j ? share : (uint64_t)p.epoch_j);

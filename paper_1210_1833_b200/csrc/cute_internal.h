@@ -16,7 +16,10 @@ constexpr int kStages = 2;                        // double buffering
 constexpr int kSegBatch = 32;                     // neighbour rows expanded per batch (one per lane)
 constexpr int kSegSlots = 3 * kSegBatch;          // <= 3 contiguous j-segments per neighbour row
 constexpr int kRefineCap = 64;                    // deferred float64 recomputations queued per warp
-constexpr int kMaxWarps = 16;
+#ifndef CUTE_MAX_WARPS
+#define CUTE_MAX_WARPS 16                         // warps per CTA = per SM (registers: 65536 / (32 * warps) per thread)
+#endif
+constexpr int kMaxWarps = CUTE_MAX_WARPS;
 constexpr float kSentinel = 1.0e18f;              // coordinate of a padding i-point (never in range)
 constexpr uint32_t kEpochJ = 1u << 22;            // flush a warp's uint32 histogram after this many j
 
@@ -61,9 +64,9 @@ struct cute_grid {
 namespace cute {
 
 // ---- pair-kernel parameters ------------------------------------------------------------------
-// float32 bin map of one variable: t = S*g(q) + O + q*(c1 + q*(c2 + q*c3)) in units of bins, where
-// g = sqrt(q) (linear bins) or log2(q) (log bins).  The pair is binned by the fast path only if
-// floor(t - tau) == floor(t + tau); otherwise it is recomputed in float64.
+// float32 bin map of one variable: t = S*g(q) + O in units of bins, where g = sqrt(q) (linear bins) or
+// log2(q) (log bins) [angular: of q times a fitted cubic c1..c4].  The pair is binned by the fast path only
+// if t is farther than tau from every integer; otherwise it is recomputed in float64.
 struct FastAxis {
     float S, O, c1, c2, c3, c4;
     float tau, tau_w;      // tau_eff = tau + tau_w * w   (w: kind-specific, see pair_count.cu)
@@ -81,9 +84,12 @@ struct PairParams {
     int self_bin;                // weighted auto-correlation: bin of zero separation (or -1)
     uint32_t epoch_j;            // flush a warp's uint32 histogram after this many j-points
     int n1, n2, n2eff, nhist;    // nhist = n1 * n2eff
+    int n2p, nhist_pad;          // shared-memory histogram with dump borders: n2p = n2 + 2 (1-D: 1), nhist_pad = (n1 + 2) * n2p
+    int simple;                  // linear bins from 0 on every axis (and, r-mu, the |l|^-2 term folded): kernel variant PK_SIMPLE
     int colshift;                // histogram columns per warp copy = 1 << colshift (32, 8 or 1)
     int hist_shared;             // 1: one histogram copy per CTA (large 2-D histograms), flushed with atomicExch
     float q_hi;                  // coarse float32 range test on q (padded)
+    float q_small;               // ANGULAR: pairs with q below this are always recomputed in float64 (theta < theta_min)
     float dz_hi;                 // RADIAL: coarse test on |dz|
     FastAxis a1, a2;
     // float64 side (refine path): exact definition
@@ -112,8 +118,13 @@ struct PairParams {
 // number of kernels this library has launched (reported by cute_launch_count)
 void note_launches(int n);
 
-// host-side launchers (pair_count.cu / grid_build.cu)
+// host-side launchers (pair_count.cu / pair_kind_*.cu / grid_build.cu)
 cudaError_t launch_pair_kernel(const PairParams &p, int blocks, cudaStream_t s);
+cudaError_t launch_kind_monopole(const PairParams &p, int blocks, size_t smem, cudaStream_t s);
+cudaError_t launch_kind_angular(const PairParams &p, int blocks, size_t smem, cudaStream_t s);
+cudaError_t launch_kind_rmu(const PairParams &p, int blocks, size_t smem, cudaStream_t s);
+cudaError_t launch_kind_radial(const PairParams &p, int blocks, size_t smem, cudaStream_t s);
+cudaError_t launch_kind_pisigma(const PairParams &p, int blocks, size_t smem, cudaStream_t s);
 // fills colshift, warps, smem_per_warp; returns total dynamic shared memory or -1 if it cannot fit
 int plan_pair_kernel(PairParams &p, int want_warps, int want_cols);
 
