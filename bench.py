@@ -4,10 +4,14 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input: the cell-list
-build (G0-G4, cute_make_grid) of the data and random catalogues, the DD, DR and RR pair counts
-(P1-P5, cute_count_pairs) and the Landy-Szalay estimator on the host (H1).  The default workload
-is BASELINE.json configs[1] ("C2": angular w(theta), 200k data x 400k randoms, 64 log bins,
-brute force, 1.8e11 pairs per step).  One JSON line is printed by rank 0.
+build (G0-G4, cute_make_grid) of the data and random catalogues, the pair counts the config names
+(P1-P5, cute_count_pairs: DD, DR, RR) and the estimator on the host (H1).  The headline workload is
+BASELINE.json configs[4] ("C5": periodic-box monopole, 10M x 10M float32 points through the 3-D
+cell list, DD + DR, 1.6e12 separations per step) -- the largest single-GPU configuration.  The same
+JSON line carries `per_config`: every one of the five configurations at full size, each with its
+per-count times, the three rates of SURVEY.md 8(d) (evaluated / binned / brute-equivalent pairs per
+second), the pair kernel's roofline, the cell build against the HBM roofline, the end-to-end
+number through cute_count_pairs_host and the oracle timed on the host cores beside it.
 
 N > 1 (torchrun): the work-item list of every pair count is split over the ranks (catalogues and
 grids replicated), and the partial uint64 histograms are summed with one NCCL all-reduce -- the
@@ -20,7 +24,6 @@ from __future__ import annotations
 
 import argparse
 import json
-import math
 import os
 import sys
 import threading
@@ -34,31 +37,8 @@ if ROOT not in sys.path:
 
 METRIC = "pairs/sec (1e9) counted into bins on 1 B200; % of pair-kernel roofline"
 UNIT = "1e9 pairs/s"
-SM_COUNT, LANES_PER_SM, SM_MAX_MHZ = 148, 128, 1965.0
-# dram__bytes_read.sum + dram__bytes_write.sum per pair-kernel launch from the committed `ncu --set full` capture
-# (profiles/r01_pair_kernel_c2.md: 11.3 MB DD, 33.8 MB DR; RR as DR), averaged over the 3 launches of a C2 step
-NCU_TRAFFIC_BYTES = {2: (11.29e6 + 33.82e6 + 33.82e6) / 3.0}
-
-
-# ------------------------------------------------------------------------------- sharding (host logic)
-def shard_bounds(nitems: int, rank: int, world: int, nchunks: int, is_auto_brute: bool):
-    """[begin, end) of the work-item list for this rank.  Items are chunk-major (item = chunk*nsplit
-    + split).  Cross-correlations and grid-assisted counts have ~uniform work per item; a brute-force
-    auto-correlation is a triangle (chunk c meets only j > i), so its boundaries are placed at equal
-    areas: the fraction of work before chunk fraction x is 1-(1-x)^2."""
-    if world <= 1:
-        return 0, nitems
-    nsplit = max(1, nitems // max(nchunks, 1))
-
-    def cut(r):
-        f = r / world
-        x = 1.0 - math.sqrt(max(0.0, 1.0 - f)) if is_auto_brute else f
-        c = int(round(x * nchunks))
-        return min(nitems, max(0, c * nsplit))
-    b, e = cut(rank), cut(rank + 1)
-    if rank == world - 1:
-        e = nitems
-    return b, e
+HEADLINE = 5
+SM_MAX_MHZ_FALLBACK = 1965.0
 
 
 # ------------------------------------------------------------------------------- clocks
@@ -108,8 +88,8 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------- the oracle legs
-def oracle_sample(w, seconds: float = 15.0):
-    """Time the oracle, as it stands, on a bounded sample of the workload's DR count (all host cores).
+def oracle_sample(w, seconds: float = 10.0):
+    """Time the oracle, as it stands, on a bounded sample of the workload's cross (or only) count, all host cores.
     Returns (pairs per second, cores, description)."""
     from oracle import oracle as o
     o.build()
@@ -118,17 +98,16 @@ def oracle_sample(w, seconds: float = 15.0):
     mode = "plain" if w.grid.get("mode", "none") == "none" else "celled"
     n1 = len(w.data[0])
     m = min(n1, 256)
-    t0 = time.perf_counter()
-    r = o.count(w.kind, w.data, c2, w.bins, mode=mode, i_range=(0, m))
-    dt = time.perf_counter() - t0
-    rate = r["npairs"] / max(dt, 1e-9)
-    per_row = r["npairs"] / m
-    m2 = int(min(n1, max(m, seconds * rate / max(per_row, 1.0))))
-    t0 = time.perf_counter()
-    r = o.count(w.kind, w.data, c2, w.bins, mode=mode, i_range=(0, m2))
-    dt = time.perf_counter() - t0
+    for _ in range(8):   # grow the slice until it lasts about `seconds` (the oracle's own set-up is part of its time)
+        t0 = time.perf_counter()
+        r = o.count(w.kind, w.data, c2, w.bins, mode=mode, i_range=(0, m))
+        dt = time.perf_counter() - t0
+        if dt >= 0.4 * seconds or m >= n1:
+            break
+        m = int(min(n1, max(2 * m, m * 0.8 * seconds / max(dt, 1e-3))))
+    m2 = m
     what = "DR" if c2 is not None else "DD"
-    return r["npairs"] / dt, cores, f"{what} rows [0,{m2}) of {n1} x all of catalogue 2, mode {mode}: {r['npairs']} separations in {dt:.2f} s"
+    return r["npairs"] / dt, cores, f"{what} rows [0,{m2}) of {n1} x all of catalogue 2, oracle mode {mode}: {r['npairs']} separations in {dt:.2f} s"
 
 
 def run_reference(args, w, cfg):
@@ -163,37 +142,284 @@ def run_reference(args, w, cfg):
 
 
 # ------------------------------------------------------------------------------- our arm
-# Algorithmic FP32-lane instructions per pair: (every evaluated pair, extra per binned pair)
-ALG_INSTR = {
-    ("angular", "none"): (13.0, 15.0),    # 9 FADD + FMUL + 2 FFMA + range test | LG2 + 3 poly + 2 + 2 FFMA + 2 floor + cmp + range + addr + atomic
-    ("angular", "sphere"): (13.0, 15.0),
-    ("monopole", "none"): (16.0, 9.0),    # periodic brute: + 9 for the minimum image | SQRT + 2 FFMA + 2 floor + cmp + range + addr + atomic
-    ("monopole", "box3d"): (7.0, 9.0),    # 3 FADD + FMUL + 2 FFMA + range test
-    ("rmu", "box3d"): (7.0, 21.0),        # + 3 FADD (s.l) + 2 (|l|^2) + FMUL + RSQ + FMUL + 2 FFMA + 2 FADD + 2 floor + cmp + range + IMAD
-    ("rmu", "none"): (7.0, 21.0),
-    ("pisigma", "box3d"): (7.0, 24.0),
-    ("pisigma", "none"): (7.0, 24.0),
-    ("radial", "sphere"): (8.0, 0.0),
-    ("radial", "none"): (8.0, 0.0),
+# Algorithmic lane-operations per pair: what the METHOD needs, independent of our SASS, counted as scalar
+# float32/int operations.  all = every evaluated pair; bin = extra per binned pair.  fp = the float32-pipe part of it
+# (packed f32x2 halves the instruction SLOTS, not the lane-operations), mufu and atom per binned pair.
+ALG = {
+    "angular": dict(all=7.0, bin=15.0, fp_all=6.0, fp_bin=8.0, mufu=1.0, atom=1.0),    # 3 FADD + FMUL + 2 FFMA + range | cubic (3) + FMUL + LG2 + FFMA + 3 (rint, frac) + 2 clamps + test + address + increment
+    "monopole": dict(all=7.0, bin=9.0, fp_all=6.0, fp_bin=4.0, mufu=1.0, atom=1.0),    # 3 FADD + FMUL + 2 FFMA + range | SQRT + FFMA + 3 (rint, frac) + clamp + test + address + increment
+    "monopole_minimg": dict(all=16.0, bin=9.0, fp_all=15.0, fp_bin=4.0, mufu=1.0, atom=1.0),   # + 3 per axis for the minimum image
+    "rmu": dict(all=7.0, bin=21.0, fp_all=6.0, fp_bin=15.0, mufu=2.0, atom=1.0),       # + s.l (3), |l|^2 (2), FMUL, RSQ, FMUL, second axis (4), tau (2), IMAD
+    "pisigma": dict(all=7.0, bin=24.0, fp_all=6.0, fp_bin=18.0, mufu=2.0, atom=1.0),
+    "radial": dict(all=8.0, bin=0.0, fp_all=6.0, fp_bin=0.0, mufu=0.0, atom=0.0),
 }
 
 
-def build_report(job, build_ms):
-    """The cell-list build (G0-G4) against the HBM roofline: algorithmic bytes / CUDA-event time of
-    cute_make_grid for all catalogues of the step (includes its host read-backs)."""
-    peak, src = 6650.0, "fallback (B200_PROFILING.md)"
+def alg_for(w):
+    if w.kind == "monopole" and w.grid.get("mode", "none") == "none" and w.bins.get("box_L", 0.0) > 0:
+        return ALG["monopole_minimg"]
+    return ALG[w.kind]
+
+
+def hbm_peak():
     try:
-        peak, src = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
     except Exception:
-        pass
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(cfg_id: int):
+    """dram bytes per pair-kernel launch from the committed ncu capture of this round, if there is one."""
+    try:
+        t = json.load(open(os.path.join(ROOT, "profiles", "r02_traffic.json")))
+        e = t.get(f"C{cfg_id}")
+        return (e["dram_bytes_per_launch"], e["source"]) if e else (None, None)
+    except Exception:
+        return None, None
+
+
+def workload_for(cfg_id: int, scale: float, args=None):
+    from paper_1210_1833_b200 import synth
+    w = synth.workload(cfg_id, scale)
+    if args is not None:
+        if args.grid == "none":
+            w.grid = dict(mode="none")
+        elif args.grid == "sphere":
+            w.grid = dict(mode="sphere", thetamax=w.bins["aperture"] if w.kind == "radial" else w.bins["hi1"], pix=args.pix)
+        elif args.grid == "box3d":
+            w.grid = dict(mode="box3d", rmax=w.bins["hi1"])
+    w.grid = dict(w.grid, no_perm=1)      # pair counting never reads the sort permutation: do not write it
+    return w
+
+
+def describe(cfg_id, w, scale):
+    return (f"BASELINE.json configs[{cfg_id - 1}] ({w.name}: {w.kind}, {'+'.join(w.pairs)}, "
+            f"nd={len(w.data[0])}, nr={len(w.rand[0]) if w.rand is not None else 0}, bins={w.bins['n1']}x{max(w.bins.get('n2', 0), 1)}, "
+            f"grid={w.grid.get('mode', 'none')}, scale={scale})")
+
+
+class Runner:
+    """One configuration resident on the device; times steps of the whole hot path."""
+
+    def __init__(self, cfg_id, w, rank, world, dist, flush):
+        from paper_1210_1833_b200 import api, runner
+        import torch
+        self.api, self.torch = api, torch
+        self.cfg_id, self.w, self.rank, self.world, self.dist, self.flush = cfg_id, w, rank, world, dist, flush
+        self.job = runner.job_for_workload(w)          # catalogues resident in HBM from here on
+        self.whichs = list(w.pairs)
+        self.brute = w.grid.get("mode", "none") == "none"
+        nh = self.job.counter.nhist
+        self.acc = {k: torch.zeros(nh, dtype=torch.int64, device="cuda") for k in self.whichs}
+        # launch-latency-scale counts (C1, C4) are looped inside the events (SURVEY.md 8(d)): one count = the mean of `inner`
+        self.inner = 100 if cfg_id in (1, 4) else 1
+
+    def step(self, record=None):
+        """One pass: build both grids, every pair count, all-reduce (N > 1), estimator on the host."""
+        torch, api, job = self.torch, self.api, self.job
+        b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        b0.record()
+        job.build()                                           # G0-G4 for both catalogues
+        b1.record()
+        evs = []
+        for which in self.whichs:
+            g1, g2 = job.grids(which)
+            skipped = False
+            if self.world > 1:
+                n = api.cute_count_items(job.kind, g1, g2, job.counter)
+                b, e = api.cute_shard_items(n, g1.info().nchunks, self.rank, self.world, self.brute and g2 is None)
+                job.opts = api.count_opts(item_begin=b, item_end=e, shard=1)
+                skipped = e <= b
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            if skipped:
+                job.counter.hist.zero_()
+            else:
+                job.enqueue(which)                            # P1-P5
+            e1.record()
+            st = api.cute_count_status(job.counter) if not skipped else {"evaluated": 0, "refined": 0}
+            self.acc[which].copy_(job.counter.hist)
+            evs.append((e0, e1, st))
+        if self.dist is not None:                             # the one exchange step: sum of partial histograms
+            allh = torch.stack([self.acc[k] for k in self.whichs])
+            self.dist.all_reduce(allh)
+            for i, k in enumerate(self.whichs):
+                self.acc[k].copy_(allh[i])
+        hs = {k: self.acc[k].cpu().numpy().astype(np.uint64) for k in self.whichs}
+        w = self.w
+        if set(self.whichs) >= {"DD", "DR", "RR"}:            # H1: Landy-Szalay on the host
+            api.cute_landy_szalay(hs["DD"], hs["DR"], hs["RR"], job.nd, job.nr)
+        elif w.bins.get("box_L", 0.0) > 0 and self.whichs == ["DD"]:
+            api.cute_periodic_xi(hs["DD"], job.nd, w.bins["box_L"], w.bins)
+        torch.cuda.synchronize()
+        ev_pairs = 0
+        for (e0, e1, st), k in zip(evs, self.whichs):
+            ev_pairs += st["evaluated"]
+            if record is not None:
+                record["counts"].setdefault(k, []).append(dict(ms=e0.elapsed_time(e1), evaluated=st["evaluated"], refined=st["refined"],
+                                                               binned=int(hs[k].sum()) if self.world == 1 else None))
+        if record is not None:
+            record["build_ms"].append(b0.elapsed_time(b1))
+        return ev_pairs
+
+    def time_counts_looped(self, record):
+        """C1 / C4: one pair count lasts ~0.2-0.4 ms, so it is looped >= 100x inside one pair of events."""
+        torch, job = self.torch, self.job
+        for which in self.whichs:
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(self.inner):
+                job.enqueue(which)
+            e1.record()
+            torch.cuda.synchronize()
+            for c in record["counts"][which]:
+                c["ms"] = e0.elapsed_time(e1) / self.inner
+                c["looped"] = self.inner
+
+    def timed(self, steps, warmup, sampler=None):
+        torch = self.torch
+        for _ in range(warmup):
+            self.step(None)
+        record = {"counts": {}, "build_ms": []}
+        if self.dist is not None:
+            self.dist.barrier()
+        torch.cuda.synchronize()
+        if sampler is not None:
+            sampler.start()
+        total_ms, total_pairs = 0.0, 0
+        for _ in range(steps):
+            self.flush.fill_(1)                               # L2 flush between timed iterations (untimed)
+            torch.cuda.synchronize()
+            s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            s0.record()
+            total_pairs += self.step(record)
+            s1.record()
+            torch.cuda.synchronize()
+            total_ms += s0.elapsed_time(s1)
+        if self.dist is not None:
+            self.dist.barrier()
+        torch.cuda.synchronize()
+        clocks = sampler.stop() if sampler is not None else None
+        if self.inner > 1 and self.world == 1:
+            self.time_counts_looped(record)
+        return total_ms, total_pairs, record, clocks
+
+    def e2e(self, steps):
+        """The same metric through cute_count_pairs_host: pinned host buffers in, host histogram out, every step."""
+        torch, api, job, w = self.torch, self.api, self.job, self.w
+        host = {}
+        for name, cat in (("data", w.data), ("rand", w.rand)):
+            if cat is None:
+                continue
+            need = 2 if job.coord == api.COORD_RADEC else 3
+            host[name] = [(torch.from_numpy(np.ascontiguousarray(c)).pin_memory()).numpy() for c in list(cat)[:need]]
+        ws = None
+        h2d = d2h = 0
+
+        def one():
+            nonlocal ws, h2d, d2h
+            h2d = d2h = 0
+            for which in self.whichs:
+                c1 = host["data"] if which in ("DD", "DR") else host["rand"]
+                c2 = host["rand"] if which == "DR" else None
+                opts = None
+                if self.world > 1:
+                    g1, g2 = job.grids(which)
+                    n = api.cute_count_items(job.kind, g1, g2, job.counter)
+                    b, e = api.cute_shard_items(n, g1.info().nchunks, self.rank, self.world, self.brute and g2 is None)
+                    if e <= b:
+                        continue
+                    opts = api.count_opts(item_begin=b, item_end=e, shard=1)
+                h, ws = api.cute_count_pairs_host(job.kind, c1, c2, job.coord, job.spec, w.bins, workspace=ws, opts=opts)
+                h2d += sum(a.nbytes for a in c1) + (sum(a.nbytes for a in c2) if c2 is not None else 0)
+                d2h += h.nbytes
+
+        one()
+        if self.dist is not None:
+            self.dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            one()
+        torch.cuda.synchronize()
+        if self.dist is not None:
+            self.dist.barrier()
+        return time.perf_counter() - t0, h2d, d2h
+
+
+def summarise(cfg_id, w, scale, rn, total_ms, total_pairs, record, steps, peaks, clock_mhz, e2e=None, cpu=None):
+    """The per-config entry: times, the three rates, rooflines."""
+    job = rn.job
+    a = alg_for(w)
+    counts = {}
+    kern_ms = ops = fp_ops = 0.0
+    evaluated = binned = brute = mufu = atoms = 0.0
+    for which, lst in record["counts"].items():
+        ms = float(np.mean([c["ms"] for c in lst]))
+        ev = float(np.mean([c["evaluated"] for c in lst]))
+        bn = float(np.mean([c["binned"] or 0 for c in lst]))
+        tot = float(job.total_pairs(which))
+        counts[which] = {"ms": ms, "evaluated_pairs": ev, "binned_pairs": bn, "brute_equivalent_pairs": tot, "refined_pairs": float(np.mean([c["refined"] for c in lst])),
+                         "evaluated_per_s": ev / (ms * 1e-3), "binned_per_s": bn / (ms * 1e-3), "brute_equivalent_per_s": tot / (ms * 1e-3)}
+        if lst[0].get("looped"):
+            counts[which]["looped_inside_events"] = lst[0]["looped"]
+        kern_ms += ms
+        evaluated += ev; binned += bn; brute += tot
+        ops += ev * a["all"] + bn * a["bin"]
+        fp_ops += ev * a["fp_all"] + bn * a["fp_bin"]
+        mufu += bn * a["mufu"]; atoms += bn * a["atom"]
+    kern_s = kern_ms * 1e-3
+    sms = peaks["sms"]
+    clk = clock_mhz * 1e6
+    issue_peak = peaks["lane_instr_per_clk_sm"] * sms * clk / 1e12           # T lane-instr/s
+    achieved = ops / kern_s / 1e12 if kern_s > 0 else 0.0
+    # the other units of SURVEY.md 8(d) R2, as upper bounds on evaluated pairs per second for THIS workload's mix
+    per_pair = lambda x: x / max(evaluated, 1.0)
+    bounds = {"issue": peaks["lane_instr_per_clk_sm"] / max(per_pair(ops), 1e-9),
+              "fp32_pipe": peaks["fp32_lane_ops_per_clk_sm"] / max(per_pair(fp_ops), 1e-9),
+              "mufu": peaks["mufu_per_clk_sm"] / max(per_pair(mufu), 1e-9) if mufu > 0 else None,
+              "shared_atomic": peaks["atoms_per_clk_sm"] / max(per_pair(atoms), 1e-9) if atoms > 0 else None}
+    bounds_s = {k: (v * sms * clk if v is not None else None) for k, v in bounds.items()}
+    binding = min((k for k in bounds_s if bounds_s[k] is not None), key=lambda k: bounds_s[k])
     nbytes = job.g_data.info().build_bytes + (job.g_rand.info().build_bytes if job.g_rand is not None else 0.0)
-    ms = float(np.mean(build_ms)) if build_ms else 0.0
-    gbs = nbytes / (ms * 1e-3) / 1e9 if ms > 0 else 0.0
-    return {"bound": "hbm", "ms": ms, "algorithmic_bytes": nbytes, "achieved": gbs, "peak": peak, "unit": "GB/s",
-            "frac": gbs / peak, "peak_source": src}
+    bms = float(np.mean(record["build_ms"])) if record["build_ms"] else 0.0
+    hbm, hsrc = hbm_peak()
+    gbs = nbytes / (bms * 1e-3) / 1e9 if bms > 0 else 0.0
+    traffic, tsrc = ncu_traffic(cfg_id) if scale == 1.0 else (None, None)
+    out = {"config": f"C{cfg_id}", "workload": describe(cfg_id, w, scale), "steps": steps, "ms_per_step": total_ms / steps,
+           "counts": counts,
+           "rates": {"evaluated_per_s": evaluated / kern_s if kern_s else 0.0, "binned_per_s": binned / kern_s if kern_s else 0.0,
+                     "brute_equivalent_per_s": brute / kern_s if kern_s else 0.0, "in_range_fraction": binned / max(evaluated, 1.0),
+                     "time_to_solution_ms": total_ms / steps},
+           "roofline": {"bound": "alu", "kernel": "pair_kernel", "achieved": achieved, "peak": issue_peak, "unit": "T lane-instr/s",
+                        "frac": achieved / issue_peak if issue_peak else 0.0, "alg_instr_per_pair": [a["all"], a["bin"]],
+                        "alg_instr_per_evaluated_pair": per_pair(ops), "binding_unit": binding,
+                        "bounds_pairs_per_s": bounds_s, "frac_of_binding_bound": (evaluated / kern_s) / bounds_s[binding] if kern_s else 0.0,
+                        "pair_kernel_share_of_step": kern_s / (total_ms / steps * 1e-3) if rn.inner == 1 else None,
+                        "traffic": traffic, "traffic_source": tsrc},
+           "build": {"bound": "hbm", "ms": bms, "algorithmic_bytes": nbytes, "achieved": gbs, "peak": hbm, "unit": "GB/s",
+                     "frac": gbs / hbm, "peak_source": hsrc}}
+    if e2e is not None:
+        out["e2e"] = e2e
+    if cpu is not None:
+        out["cpu_baseline"] = cpu
+    return out
 
 
-def run_ours(args, w, cfg):
+def measured_peaks(api, torch):
+    """Roofline denominators measured on this device in this run (cute_measure_peaks: SURVEY.md 8(d) R2)."""
+    pk = api.cute_measure_peaks()
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    return {"sms": sms,
+            "lane_instr_per_clk_sm": max(pk["ffma"][0], pk["fmnmx"][0], pk["iadd"][0]),   # one instruction slot per lane and clock
+            "fp32_lane_ops_per_clk_sm": max(pk["ffma2"][0], pk["fadd2"][0], pk["ffma"][0]),
+            "mufu_per_clk_sm": pk["mufu_sqrt"][0],
+            "atoms_per_clk_sm": pk["atoms_inc_cols8_random_bins"][0],
+            "table": {k: v[0] for k, v in pk.items()},
+            "source": "cute_measure_peaks (clock64 microbenchmarks on this device, this run): lane-operations per clock per SM"}
+
+
+def run_ours(args):
     import torch
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -203,88 +429,16 @@ def run_ours(args, w, cfg):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    from paper_1210_1833_b200 import api, runner
+    from paper_1210_1833_b200 import api
 
-    job = runner.job_for_workload(w)          # catalogues resident in HBM from here on
-    whichs = list(w.pairs)
-    brute = w.grid.get("mode", "none") == "none"
+    peaks = measured_peaks(api, torch)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    nh = job.counter.nhist
-    acc = {k: torch.zeros(nh, dtype=torch.int64, device="cuda") for k in whichs}
-    pair_ms, pair_pairs, pair_binned = [], [], []
-
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    build_ms = []
-
-    def one_step(record):
-        b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        b0.record()
-        job.build()                                           # G0-G4 for both catalogues
-        b1.record()
-        evs = []
-        for which in whichs:
-            g1, g2 = job.grids(which)
-            n = api.cute_count_items(job.kind, g1, g2, job.counter)
-            b, e = shard_bounds(n, rank, world, g1.info().nchunks, brute and g2 is None)
-            job.opts = api.count_opts(item_begin=b, item_end=max(e, b)) if world > 1 else None
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            if not (world > 1 and e <= b):
-                job.enqueue(which)                            # P1-P5
-            else:
-                job.counter.hist.zero_()
-            e1.record()
-            skipped = world > 1 and e <= b
-            st = api.cute_count_status(job.counter) if not skipped else {"evaluated": 0}
-            acc[which].copy_(job.counter.hist)
-            evs.append((e0, e1, st["evaluated"]))
-        if dist is not None:                                  # the one exchange step: sum of partial histograms
-            allh = torch.stack([acc[k] for k in whichs])
-            dist.all_reduce(allh)
-            for i, k in enumerate(whichs):
-                acc[k].copy_(allh[i])
-        hs = {k: acc[k].cpu().numpy().astype(np.uint64) for k in whichs}
-        xi = None
-        if set(whichs) >= {"DD", "DR", "RR"}:                 # H1: Landy-Szalay on the host
-            xi, _ = api.cute_landy_szalay(hs["DD"], hs["DR"], hs["RR"], job.nd, job.nr)
-        elif w.bins.get("box_L", 0.0) > 0 and whichs == ["DD"]:
-            xi, _ = api.cute_periodic_xi(hs["DD"], job.nd, w.bins["box_L"], w.bins)
-        torch.cuda.synchronize()
-        ev_pairs = 0
-        if record:
-            build_ms.append(b0.elapsed_time(b1))
-        for (e0, e1, npairs), k in zip(evs, whichs):
-            ev_pairs += npairs
-            if record:
-                pair_ms.append(e0.elapsed_time(e1))
-                pair_pairs.append(npairs)
-                pair_binned.append(int(hs[k].sum()) if world == 1 else None)
-        return ev_pairs, hs, xi
-
-    for _ in range(args.warmup):
-        one_step(False)
+    head_id = args.config
+    w = workload_for(head_id, args.scale, args)
+    rn = Runner(head_id, w, rank, world, dist, flush)
     sampler = ClockSampler(local)
     launches0 = api.cute_launch_count()
-    barrier()
-    sampler.start()
-    total_ms, total_pairs = 0.0, 0
-    hs = None
-    for _ in range(args.steps):
-        flush.fill_(1)                                        # L2 flush between timed iterations (untimed)
-        torch.cuda.synchronize()
-        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        s0.record()
-        npairs, hs, xi = one_step(True)
-        s1.record()
-        torch.cuda.synchronize()
-        total_ms += s0.elapsed_time(s1)
-        total_pairs += npairs
-    barrier()
-    clocks = sampler.stop()
+    total_ms, total_pairs, record, clocks = rn.timed(args.steps, args.warmup, sampler)
     launches = api.cute_launch_count() - launches0
     t = torch.tensor([total_ms, float(total_pairs)], dtype=torch.float64, device="cuda")
     if dist is not None:
@@ -293,85 +447,68 @@ def run_ours(args, w, cfg):
         dist.all_reduce(t, op=dist.ReduceOp.SUM)
         total_ms, total_pairs = float(tmax[0]), float(t[1])
     value = total_pairs / (total_ms * 1e-3) / 1e9
+    clock_mhz = (clocks or {}).get("sm_mhz") or (clocks or {}).get("sm_max_mhz") or SM_MAX_MHZ_FALLBACK
 
-    # ---- end to end through the public host API: host buffers in, host histogram out
-    import torch as _t
-    host = {}
-    for name, cat in (("data", w.data), ("rand", w.rand)):
-        if cat is None:
-            continue
-        need = 2 if job.coord == api.COORD_RADEC else 3
-        host[name] = [(_t.from_numpy(np.ascontiguousarray(c)).pin_memory()).numpy() for c in list(cat)[:need]]
-    e2e_ws = None
-    h2d = d2h = 0
-
-    def e2e_step():
-        nonlocal e2e_ws, h2d, d2h
-        h2d = d2h = 0
-        pairs = 0
-        for which in whichs:
-            c1 = host["data"] if which in ("DD", "DR") else host["rand"]
-            c2 = host["rand"] if which == "DR" else None
-            opts = None
-            if world > 1:
-                g1, g2 = job.grids(which)
-                n = api.cute_count_items(job.kind, g1, g2, job.counter)
-                b, e = shard_bounds(n, rank, world, g1.info().nchunks, brute and g2 is None)
-                opts = api.count_opts(item_begin=b, item_end=max(e, b))
-                if e <= b:
-                    continue
-            h, e2e_ws = api.cute_count_pairs_host(job.kind, c1, c2, job.coord, job.spec, w.bins, workspace=e2e_ws, opts=opts)
-            h2d += sum(a.nbytes for a in c1) + (sum(a.nbytes for a in c2) if c2 is not None else 0)
-            d2h += h.nbytes
-            n1, n2 = len(c1[0]), (len(c2[0]) if c2 is not None else 0)
-            pairs += n1 * n2 if c2 is not None else n1 * (n1 - 1) // 2
-        return pairs
-
-    e2e_step()
-    barrier()
-    t0 = time.perf_counter()
-    e2e_pairs = 0
-    for _ in range(args.steps):
-        e2e_pairs += e2e_step()
-    barrier()
-    e2e_s = time.perf_counter() - t0
-    if brute and world == 1:
-        e2e_val = e2e_pairs / e2e_s / 1e9
-    else:   # grid-assisted or sharded: the evaluated separations are the device arm's
-        e2e_val = (total_pairs / args.steps) * args.steps / e2e_s / 1e9 if world == 1 else None
+    # ---- end to end through the public host API
+    e2e_s, h2d, d2h = rn.e2e(args.steps)
     if dist is not None:
         te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
         dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        e2e_val = total_pairs / float(te[0]) / 1e9
-
+        e2e_s = float(te[0])
+    e2e_val = total_pairs / e2e_s / 1e9       # the same evaluated separations, over the end-to-end wall time
+    e2e = {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+           "ms_per_step": 1e3 * e2e_s / args.steps, "api": "cute_count_pairs_host"}
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
-    # ---- roofline of the dominant kernel (the pair kernel): algorithmic lane-instructions / duration
-    i_all, i_bin = ALG_INSTR[(w.kind, w.grid.get("mode", "none"))]
-    ops = sum(p * i_all + (b or 0) * i_bin for p, b in zip(pair_pairs, pair_binned))
-    kern_s = sum(pair_ms) * 1e-3
-    achieved = ops / kern_s / 1e12 if kern_s > 0 else 0.0
-    peak = SM_COUNT * LANES_PER_SM * SM_MAX_MHZ * 1e6 / 1e12
-    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-           "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
-           "dtype": "f32", "data": "synthetic", "config": cfg, "clocks": clocks, "gpu_launches": int(launches),
-           "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
-           "roofline": {"bound": "alu", "kernel": "pair_kernel", "achieved": achieved, "peak": peak, "unit": "T lane-instr/s",
-                        "frac": achieved / peak,
-                        "traffic": NCU_TRAFFIC_BYTES.get(args.config) if args.scale == 1.0 and world == 1 else None,
-                        "traffic_unit": "bytes of DRAM per pair-kernel launch (ncu, profiles/r01_pair_kernel_c2.md)",
-                        "peak_source": "148 SMs x 128 FP32 lanes x 1965 MHz (guide unit counts and max clock; DESIGN.md)",
-                        "pair_kernel_share_of_step": kern_s / (total_ms * 1e-3),
-                        "pairs_per_s_in_kernel": sum(pair_pairs) / kern_s if kern_s > 0 else 0.0,
-                        "alg_instr_per_pair": [i_all, i_bin]},
-           "build": build_report(job, build_ms),
-           "rates": {"evaluated_pairs_per_step": total_pairs / args.steps,
-                     "binned_pairs_per_step": (sum(b for b in pair_binned if b is not None) / args.steps) if world == 1 else None}}
+
+    cpu = None
     if world == 1 and not args.no_cpu_baseline:
         v, cores, sample = oracle_sample(w)
-        out["cpu_baseline"] = {"value": v / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        cpu = {"value": v / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+    head = summarise(head_id, w, args.scale, rn, total_ms, total_pairs, record, args.steps, peaks, clock_mhz, e2e, cpu) if world == 1 else None
+    del rn
+    torch.cuda.empty_cache()
+
+    # ---- every other configuration at full size (world == 1; the headline's own entry is reused)
+    per_config = []
+    if world == 1 and not args.only:
+        for cid in (1, 2, 3, 4, 5):
+            if cid == head_id:
+                per_config.append(head)
+                continue
+            wc = workload_for(cid, args.scale)
+            rc = Runner(cid, wc, 0, 1, None, flush)
+            ksteps = max(3, min(args.steps, 5))
+            tms, tp, rec, _ = rc.timed(ksteps, 3)
+            es, eh, ed = rc.e2e(ksteps)
+            ec = {"value": tp / es / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(eh), "d2h_bytes_per_step": int(ed),
+                  "ms_per_step": 1e3 * es / ksteps, "api": "cute_count_pairs_host"}
+            cc = None
+            if not args.no_cpu_baseline:
+                v, cores, sample = oracle_sample(wc, seconds=6.0)
+                cc = {"value": v / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+            per_config.append(summarise(cid, wc, args.scale, rc, tms, tp, rec, ksteps, peaks, clock_mhz, ec, cc))
+            del rc
+            torch.cuda.empty_cache()
+
+    cfg = {"workload": describe(head_id, w, args.scale), "scale": args.scale,
+           "l2": "256 MiB buffer written between timed iterations (L2 flush)",
+           "parallelism": f"work items sharded over {world} GPU(s), catalogues replicated, one all-reduce of the histogram"}
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+           "dtype": "f32", "data": "synthetic", "config": cfg, "clocks": clocks, "gpu_launches": int(launches), "e2e": e2e,
+           "value_is": "evaluated separations per second over the whole step (build + counts + estimator); binned pairs/s is in rates"}
+    if head is not None:
+        out["roofline"] = dict(head["roofline"], peak_source=peaks["source"], clock_mhz_used=clock_mhz)
+        out["build"] = head["build"]
+        out["rates"] = head["rates"]
+        out["counts"] = head["counts"]
+        if cpu is not None:
+            out["cpu_baseline"] = cpu
+        out["per_config"] = per_config
+    out["peaks"] = {k: peaks[k] for k in ("lane_instr_per_clk_sm", "fp32_lane_ops_per_clk_sm", "mufu_per_clk_sm", "atoms_per_clk_sm", "source")}
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
@@ -383,31 +520,21 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config 1..5 (default 2: the metric's workload)")
-    ap.add_argument("--scale", type=float, default=1.0, help="shrink the catalogues (debugging only; 1.0 = the named config)")
+    ap.add_argument("--config", type=int, default=HEADLINE, help="headline BASELINE.json config 1..5 (default 5: the largest single-GPU one)")
+    ap.add_argument("--scale", type=float, default=1.0, help="shrink the catalogues (debugging only; 1.0 = the named configs)")
+    ap.add_argument("--only", action="store_true", help="measure the headline config only (no per_config sweep)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--grid", default="default", choices=["default", "none", "sphere", "box3d"],
-                    help="override the workload's neighbour search (default: the one BASELINE.json names)")
+                    help="override the headline workload's neighbour search (default: the one BASELINE.json names)")
     ap.add_argument("--pix", type=float, default=0.1, help="--grid sphere: pixel side in units of theta_max")
     args = ap.parse_args()
-    from paper_1210_1833_b200 import synth
-    w = synth.workload(args.config, args.scale)
-    if args.grid == "none":
-        w.grid = dict(mode="none")
-    elif args.grid == "sphere":
-        w.grid = dict(mode="sphere", thetamax=w.bins["aperture"] if w.kind == "radial" else w.bins["hi1"], pix=args.pix)
-    elif args.grid == "box3d":
-        w.grid = dict(mode="box3d", rmax=w.bins["hi1"])
-    cfg = {"workload": f"BASELINE.json configs[{args.config - 1}] ({w.name}: {w.kind}, {'+'.join(w.pairs)}, "
-                       f"nd={len(w.data[0])}, nr={len(w.rand[0]) if w.rand is not None else 0}, bins={w.bins['n1']}x{max(w.bins.get('n2', 0), 1)}, "
-                       f"grid={w.grid.get('mode', 'none')})",
-           "scale": args.scale, "l2": "256 MiB buffer written between timed iterations (L2 flush)",
-           "parallelism": f"work items sharded over {args.gpus} GPU(s), catalogues replicated, one all-reduce of the histogram"}
-    w.grid = dict(w.grid, no_perm=1)      # pair counting never reads the sort permutation: do not write it
     if args.impl == "reference":
+        w = workload_for(args.config, args.scale, args)
+        cfg = {"workload": describe(args.config, w, args.scale), "scale": args.scale,
+               "parallelism": "oracle on the host cores (rank 0 only)"}
         run_reference(args, w, cfg)
     else:
-        run_ours(args, w, cfg)
+        run_ours(args)
 
 
 if __name__ == "__main__":

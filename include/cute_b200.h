@@ -206,6 +206,22 @@ int cute_count_pairs(int kind, const cute_grid *g1, const cute_grid *g2, const c
 int cute_count_items(int kind, const cute_grid *g1, const cute_grid *g2, const cute_bin_spec *bins,
                      const cute_count_opts *opts, int64_t *nitems);
 
+/* Sharding of a pair count over `world` ranks: [*begin, *end) of the nitems work items that rank
+ * `rank` handles (pass them as cute_count_opts.item_begin / item_end with shard = 1).  Items are chunk-major (item =
+ * chunk * nsplit + split, nchunks from cute_grid_info).  Cross-correlations and cell-list counts have ~uniform work per
+ * item; a brute-force AUTO-correlation (auto_brute != 0) is a triangle -- chunk c meets only j > i -- so its cuts are
+ * placed at equal areas, 1 - (1 - x)^2.  The shards partition [0, nitems): integer partial histograms add up exactly. */
+int cute_shard_items(int64_t nitems, int64_t nchunks, int rank, int world, int auto_brute, int64_t *begin, int64_t *end);
+
+/* Grid sizing from the data ("a box encompassing the whole catalog is first determined", PAPER.md:208-215
+ * for pixels): fills *spec for `kind` with mode BOX3D or SPHERE so that ONE spec serves all the ncat catalogues (DEVICE
+ * pointers) of a correlation function -- their common bounding box, padded; BOX3D: box_L > 0 gives the periodic box
+ * [0,L)^3, ncell is left to cute_make_grid unless given; SPHERE: pixels of side pix_frac * rmax [rad] with constant
+ * limits in RA and sin(Dec), the full ring when the footprint is wider than 180 degrees in RA (or straddles RA = 0).
+ * rmax: largest separation (r, or theta in rad).  d_tmp: DEVICE >= 64 bytes.  Synchronises the stream. */
+int cute_auto_grid_spec(int kind, int mode, const cute_catalog *const *cats, int ncat, double rmax, double box_L,
+                        double pix_frac, const int ncell[3], int no_perm, void *d_tmp, void *stream, cute_grid_spec *spec);
+
 /* Synchronises `stream` and returns the deferred status of the last cute_count_pairs that used
  * d_scratch.  stats (host, may be NULL): [0] separations evaluated, [1] pairs recomputed in float64,
  * [2] work items, [3] shared-memory histogram flushes. */

@@ -59,7 +59,7 @@ SYMBOLS = ["cute_version", "cute_strerror", "cute_launch_count", "cute_catalog_b
            "cute_grid_get_info", "cute_count_scratch_bytes", "cute_count_pairs", "cute_count_items",
            "cute_count_status", "cute_host_workspace_bytes", "cute_count_pairs_host", "cute_bin_edges",
            "cute_landy_szalay", "cute_natural_estimator", "cute_multipoles", "cute_periodic_rr", "cute_periodic_xi",
-           "cute_peak_count", "cute_peak_name", "cute_measure_peaks"]
+           "cute_peak_count", "cute_peak_name", "cute_measure_peaks", "cute_shard_items", "cute_auto_grid_spec"]
 
 
 def _load() -> C.CDLL:
@@ -90,6 +90,9 @@ def _load() -> C.CDLL:
                                               C.POINTER(cute_bin_spec), C.POINTER(C.c_size_t)]
     lib.cute_count_pairs_host.argtypes = [C.c_int, C.POINTER(cute_catalog), C.POINTER(cute_catalog), C.POINTER(cute_grid_spec),
                                           C.POINTER(cute_bin_spec), C.POINTER(cute_count_opts), up, vp, C.c_size_t, vp]
+    lib.cute_shard_items.argtypes = [C.c_int64, C.c_int64, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    lib.cute_auto_grid_spec.argtypes = [C.c_int, C.c_int, C.POINTER(C.POINTER(cute_catalog)), C.c_int, C.c_double, C.c_double,
+                                        C.c_double, C.POINTER(C.c_int), C.c_int, vp, vp, C.POINTER(cute_grid_spec)]
     lib.cute_peak_count.restype = C.c_int
     lib.cute_peak_name.restype = C.c_char_p
     lib.cute_peak_name.argtypes = [C.c_int]
@@ -405,37 +408,30 @@ def cute_measure_peaks(stream=None) -> dict:
 COORD_OF_KIND = {"monopole": COORD_XYZ, "rmu": COORD_XYZ, "pisigma": COORD_XYZ, "angular": COORD_RADEC, "radial": COORD_RADECZ}
 
 
+def cute_shard_items(nitems: int, nchunks: int, rank: int, world: int, auto_brute: bool):
+    """[begin, end) of the work-item list for this rank (the library's sharding policy; needs no GPU)."""
+    b, e = C.c_int64(0), C.c_int64(0)
+    _check(lib.cute_shard_items(int(nitems), int(nchunks), int(rank), int(world), int(bool(auto_brute)), C.byref(b), C.byref(e)),
+           "cute_shard_items")
+    return int(b.value), int(e.value)
+
+
 def auto_spec(kind: str, bins: dict, grid: dict, cats_dev, coord: int) -> cute_grid_spec:
-    """Grid spec for a workload: `grid` is synth.Workload.grid (mode + rmax/thetamax [+ ncell, pix]);
-    cats_dev: the device catalogues that will share the spec (their common bounding box is used)."""
-    k = KINDS[kind]
-    mode = grid.get("mode", "none")
-    npm = int(grid.get("no_perm", 0))
-    if mode == "none":
-        return grid_spec("none", kind_mask=1 << k, no_perm=npm)
-    if mode == "box3d":
-        L = float(bins.get("box_L", 0.0))
-        ncell = grid.get("ncell", (0, 0, 0))
-        if L > 0:
-            return grid_spec("box3d", periodic=True, size=(L, L, L), rmax=grid["rmax"], ncell=ncell, kind_mask=1 << k, no_perm=npm)
-        bb = np.array([cute_catalog_bounds(c, coord) for c in cats_dev if c[0].numel() > 0])
-        lo, hi = bb[:, :3].min(axis=0), bb[:, 3:].max(axis=0)
-        pad = 1e-6 * np.maximum(hi - lo, 1.0) + 1e-9 * np.maximum(np.abs(lo), np.abs(hi))
-        return grid_spec("box3d", origin=lo - pad, size=(hi - lo) + 2 * pad, rmax=grid["rmax"], ncell=ncell, kind_mask=1 << k, no_perm=npm)
-    # sphere: pixels with constant limits in (RA, sin Dec); RA must not wrap inside the footprint
-    tm = float(grid["thetamax"])
-    pix = float(grid.get("pix", 2.0)) * tm                      # pixel side [rad]
-    bb = np.array([cute_catalog_bounds(c, coord) for c in cats_dev if c[0].numel() > 0])
-    ra_lo, ra_hi = bb[:, 0].min(), bb[:, 3].max()
-    de_lo, de_hi = bb[:, 1].min(), bb[:, 4].max()
-    dra = min(360.0, (ra_hi - ra_lo) * (1 + 1e-9) + 1e-9)
-    if dra > 180.0:                      # wide or seam-straddling footprint: pixels over the full ring (RA wraps)
-        dra = 360.0
-    ra0 = ra_lo - 0.5 * (dra - (ra_hi - ra_lo)) if dra < 360.0 else 0.0
-    u_lo = max(-1.0, np.sin(np.radians(de_lo)) - 1e-12)
-    u_hi = min(1.0, np.sin(np.radians(de_hi)) + 1e-12)
-    du = u_hi - u_lo
-    cmax = np.cos(np.radians(min(abs(de_lo), abs(de_hi)) if de_lo * de_hi > 0 else 0.0))
-    nra = int(max(1, min(65535, np.floor(np.radians(dra) * cmax / pix))))
-    nu = int(max(1, min(1 << 20, np.floor(du / pix))))
-    return grid_spec("sphere", origin=(ra0, u_lo, 0), size=(dra, du, 0), ncell=(nra, nu, 1), rmax=tm, kind_mask=1 << k, no_perm=npm)
+    """Grid spec for a workload (cute_auto_grid_spec): `grid` is synth.Workload.grid (mode + rmax/thetamax [+ ncell, pix]);
+    cats_dev: the device catalogues that will share the spec.  Marshalling only: the geometry is the library's."""
+    torch = _torch()
+    mode = {"none": GRID_NONE, "box3d": GRID_BOX3D, "sphere": GRID_SPHERE}[grid.get("mode", "none")]
+    cats, keep = [], []
+    for c in cats_dev:
+        cat, k = _catalog(c, coord, True)
+        cats.append(cat)
+        keep.append(k)
+    arr = (C.POINTER(cute_catalog) * len(cats))(*[C.pointer(c) for c in cats])
+    rmax = float(grid.get("rmax", grid.get("thetamax", 0.0)))
+    ncell = (C.c_int * 3)(*map(int, grid.get("ncell", (0, 0, 0))))
+    tmp = torch.empty(16, dtype=torch.float64, device="cuda")
+    spec = cute_grid_spec()
+    _check(lib.cute_auto_grid_spec(KINDS[kind], mode, arr, len(cats), rmax, float(bins.get("box_L", 0.0)) if mode == GRID_BOX3D else 0.0,
+                                   float(grid.get("pix", 2.0)), ncell, int(grid.get("no_perm", 0)), C.c_void_p(tmp.data_ptr()),
+                                   C.c_void_p(_stream_ptr()), C.byref(spec)), "cute_auto_grid_spec")
+    return spec

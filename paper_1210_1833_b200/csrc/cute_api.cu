@@ -887,6 +887,84 @@ int cute_count_items(int kind, const cute_grid *g1, const cute_grid *g2, const c
     return count_impl(kind, g1, g2, bins, nullptr, nullptr, 0, opts, nullptr, nitems);
 }
 
+int cute_shard_items(int64_t nitems, int64_t nchunks, int rank, int world, int auto_brute, int64_t *begin, int64_t *end)
+{
+    if (!begin || !end || nitems < 0 || nchunks < 0 || world < 1 || rank < 0 || rank >= world) return CUTE_ERR_INVALID_ARG;
+    if (world == 1) { *begin = 0; *end = nitems; return CUTE_OK; }
+    const int64_t nsplit = nchunks > 0 && nitems / nchunks > 0 ? nitems / nchunks : 1;
+    auto cut = [&](int r) -> int64_t {
+        if (r <= 0) return 0;
+        if (r >= world) return nitems;
+        const double f = (double)r / (double)world;
+        const double x = auto_brute ? 1.0 - sqrt(fmax(0.0, 1.0 - f)) : f;
+        int64_t c = (int64_t)llround(x * (double)nchunks) * nsplit;
+        return c < 0 ? 0 : (c > nitems ? nitems : c);
+    };
+    *begin = cut(rank); *end = cut(rank + 1);
+    if (*end < *begin) *end = *begin;
+    return CUTE_OK;
+}
+
+int cute_auto_grid_spec(int kind, int mode, const cute_catalog *const *cats, int ncat, double rmax, double box_L,
+                        double pix_frac, const int ncell[3], int no_perm, void *d_tmp, void *stream, cute_grid_spec *spec)
+{
+    if (!spec || !cats || ncat < 1 || ncat > 8 || kind < CUTE_ANGULAR || kind > CUTE_PISIGMA) return CUTE_ERR_INVALID_ARG;
+    if (mode < CUTE_GRID_NONE || mode > CUTE_GRID_SPHERE) return CUTE_ERR_INVALID_ARG;
+    memset(spec, 0, sizeof(*spec));
+    spec->struct_size = sizeof(*spec);
+    spec->mode = mode; spec->kind_mask = 1 << kind; spec->no_perm = no_perm;
+    if (mode == CUTE_GRID_NONE) return CUTE_OK;
+    if (!(rmax > 0.0)) return CUTE_ERR_INVALID_ARG;
+    spec->rmax = rmax;
+    if (ncell) for (int d = 0; d < 3; d++) spec->ncell[d] = ncell[d];
+    if (mode == CUTE_GRID_BOX3D && box_L > 0.0) {
+        spec->periodic = 1;
+        for (int d = 0; d < 3; d++) spec->size[d] = box_L;
+        return CUTE_OK;
+    }
+    // common bounding box of the raw coordinates
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    bool any = false;
+    for (int k = 0; k < ncat; k++) {
+        if (!cats[k]) return CUTE_ERR_INVALID_ARG;
+        if (cats[k]->n == 0) continue;
+        double b[6];
+        int rc = cute_catalog_bounds(cats[k], d_tmp, stream, b);
+        if (rc) return rc;
+        for (int d = 0; d < 3; d++) { lo[d] = fmin(lo[d], b[d]); hi[d] = fmax(hi[d], b[3 + d]); }
+        any = true;
+    }
+    if (!any) for (int d = 0; d < 3; d++) { lo[d] = 0.0; hi[d] = 1.0; }
+    if (mode == CUTE_GRID_BOX3D) {
+        for (int d = 0; d < 3; d++) {
+            const double ext = hi[d] - lo[d];
+            const double pad = 1e-6 * (ext > 1.0 ? ext : 1.0) + 1e-9 * fmax(fabs(lo[d]), fabs(hi[d]));
+            spec->origin[d] = lo[d] - pad;
+            spec->size[d] = ext + 2.0 * pad;
+        }
+        return CUTE_OK;
+    }
+    // SPHERE: pixels with constant limits in (RA, sin Dec); RA must not wrap inside the footprint
+    if (!(pix_frac > 0.0)) pix_frac = 2.0;
+    const double pix = pix_frac * rmax;                       // pixel side [rad]
+    double dra = fmin(360.0, (hi[0] - lo[0]) * (1.0 + 1e-9) + 1e-9);
+    if (dra > 180.0) dra = 360.0;                             // wide or seam-straddling footprint: pixels over the full ring
+    const double ra0 = dra < 360.0 ? lo[0] - 0.5 * (dra - (hi[0] - lo[0])) : 0.0;
+    const double u_lo = fmax(-1.0, sin(fmax(-90.0, lo[1]) * (kPi / 180.0)) - 1e-12);
+    const double u_hi = fmin(1.0, sin(fmin(90.0, hi[1]) * (kPi / 180.0)) + 1e-12);
+    const double du = fmax(u_hi - u_lo, 1e-12);
+    const double dmin = (lo[1] * hi[1] > 0.0) ? fmin(fabs(lo[1]), fabs(hi[1])) : 0.0;   // the widest parallel of the footprint
+    const double cmax = cos(dmin * (kPi / 180.0));
+    double nra = floor(dra * (kPi / 180.0) * cmax / pix), nu = floor(du / pix);
+    nra = nra < 1.0 ? 1.0 : (nra > 65535.0 ? 65535.0 : nra);
+    nu = nu < 1.0 ? 1.0 : (nu > 1048576.0 ? 1048576.0 : nu);
+    spec->origin[0] = ra0; spec->origin[1] = u_lo;
+    spec->size[0] = dra; spec->size[1] = du;
+    if (!(ncell && ncell[0] > 0 && ncell[1] > 0)) { spec->ncell[0] = (int)nra; spec->ncell[1] = (int)nu; }
+    spec->ncell[2] = 1;
+    return CUTE_OK;
+}
+
 int cute_count_status(void *d_scratch, void *stream, uint64_t stats[4])
 {
     if (!d_scratch) return CUTE_ERR_INVALID_ARG;

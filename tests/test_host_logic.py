@@ -123,9 +123,8 @@ def test_product_path_does_not_touch_the_oracle():
 
 
 # ------------------------------------------------------------------------------- sharding
-def test_shard_bounds_partition():
-    sys.path.insert(0, ROOT)
-    from bench import shard_bounds
+def test_shard_bounds_partition(api):
+    shard_bounds = lambda nitems, r, world, nchunks, auto: api.cute_shard_items(nitems, nchunks, r, world, auto)
     for nchunks, nsplit, world, auto in [(1563, 19, 2, True), (1563, 19, 8, True), (3125, 10, 4, False), (7, 1, 8, False),
                                          (78326, 1, 8, False), (1, 5, 4, True)]:
         nitems = nchunks * nsplit
@@ -144,7 +143,8 @@ _WORKER = r"""
 import os, sys
 import numpy as np, torch, torch.distributed as dist
 sys.path.insert(0, sys.argv[1])
-from bench import shard_bounds
+from paper_1210_1833_b200 import api
+shard_bounds = lambda nitems, r, world, nchunks, auto: api.cute_shard_items(nitems, nchunks, r, world, auto)
 dist.init_process_group("gloo", rank=int(os.environ["RANK"]), world_size=int(os.environ["WORLD_SIZE"]))
 r, w = dist.get_rank(), dist.get_world_size()
 # a fake pair count: item k contributes 1 to bin k % 7 and k to bin 7; shards must add up to the whole
