@@ -102,6 +102,9 @@ typedef struct cute_grid_spec {
                    /* coordinates allow.  Lets the build skip arrays a kind does not read (the low parts). */
     int no_perm;   /* != 0: do not write the sorted-slot -> input-index permutation (cute_grid_info.d_perm = NULL); */
                    /* pair counting never reads it, and it is a random 4-byte store per object                     */
+    int build_path; /* 0: chosen by size (catalogues of >= 2^20 objects are built by a two-level partition: coarse   */
+                   /* buckets of consecutive cells, then one CTA per bucket in shared memory); 1: one-pass counting */
+                   /* sort; 2: partition.  Same result up to the (arbitrary) order inside a cell.                  */
 } cute_grid_spec;
 
 /* Binning.  Variable 1: theta [rad] (ANGULAR), r (MONOPOLE, RMU), zbar (RADIAL), pi (PISIGMA); linear or, if

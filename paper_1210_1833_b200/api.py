@@ -30,7 +30,7 @@ class cute_catalog(C.Structure):
 class cute_grid_spec(C.Structure):
     _fields_ = [("struct_size", C.c_size_t), ("mode", C.c_int), ("periodic", C.c_int),
                 ("origin", C.c_double * 3), ("size", C.c_double * 3), ("ncell", C.c_int * 3),
-                ("rmax", C.c_double), ("kind_mask", C.c_int), ("no_perm", C.c_int)]
+                ("rmax", C.c_double), ("kind_mask", C.c_int), ("no_perm", C.c_int), ("build_path", C.c_int)]
 
 
 class cute_bin_spec(C.Structure):
@@ -142,10 +142,10 @@ def bin_spec(bins: dict) -> cute_bin_spec:
 
 
 def grid_spec(mode="none", periodic=False, origin=(0, 0, 0), size=(0, 0, 0), ncell=(0, 0, 0), rmax=0.0,
-              kind_mask=0, no_perm=0) -> cute_grid_spec:
+              kind_mask=0, no_perm=0, build_path=0) -> cute_grid_spec:
     m = {"none": GRID_NONE, "box3d": GRID_BOX3D, "sphere": GRID_SPHERE}[mode] if isinstance(mode, str) else int(mode)
     return cute_grid_spec(C.sizeof(cute_grid_spec), m, int(bool(periodic)), (C.c_double * 3)(*map(float, origin)),
-                          (C.c_double * 3)(*map(float, size)), (C.c_int * 3)(*map(int, ncell)), float(rmax), int(kind_mask), int(no_perm))
+                          (C.c_double * 3)(*map(float, size)), (C.c_int * 3)(*map(int, ncell)), float(rmax), int(kind_mask), int(no_perm), int(build_path))
 
 
 def count_opts(**kw) -> cute_count_opts:
@@ -434,4 +434,5 @@ def auto_spec(kind: str, bins: dict, grid: dict, cats_dev, coord: int) -> cute_g
     _check(lib.cute_auto_grid_spec(KINDS[kind], mode, arr, len(cats), rmax, float(bins.get("box_L", 0.0)) if mode == GRID_BOX3D else 0.0,
                                    float(grid.get("pix", 2.0)), ncell, int(grid.get("no_perm", 0)), C.c_void_p(tmp.data_ptr()),
                                    C.c_void_p(_stream_ptr()), C.byref(spec)), "cute_auto_grid_spec")
+    spec.build_path = int(grid.get("build_path", 0))
     return spec

@@ -34,7 +34,8 @@ inline int sm_count()
 // ---- workspace layout of one grid -------------------------------------------------------------
 struct Layout {
     size_t hi, lo, p64, perm, count, cell_start, scan_tmp, row_nchunks, row_chunk_start, chunks,
-        row_kx, row_ylo, row_yhi, status, bbox, total;
+        row_kx, row_ylo, row_yhi, status, bbox, part_tmp, part_table, total;
+    int part_G;
     uint32_t n_pad;
     int64_t max_cells, max_rows, max_chunks;
 };
@@ -43,7 +44,20 @@ constexpr int64_t kOrderCellsMax = 65536;   // mode NONE: cells that only order 
 
 inline int64_t cell_cap(int64_t n) { return n * 2 > 4096 ? n * 2 : 4096; }
 
-Layout make_layout(int64_t n, int want_lo, int want_f64, int64_t max_cells, int64_t max_rows)
+inline int part_ctas() { return 2 * sm_count(); }
+
+// rec_bytes: bytes of one raw record of the partition path (16: float32 xyz, 32: otherwise); used when n >= kPartMinN
+// Measured on B200 (profiles/r02_build.md): the partition wins for float64 / RA-Dec catalogues (32-byte records that carry
+// their cell, so sin() and the FP64 cell arithmetic run twice instead of four times: C4 0.42 -> 0.34 ms), and loses for
+// float32 xyz (C5: 0.86 ms against 0.70 ms one-pass -- the 160 MB of grouped records do not fit L2 and make a round trip
+// through HBM), so float32 xyz keeps the one-pass counting sort unless build_path = 2 asks otherwise.
+inline bool use_partition(int64_t n, const cute_catalog *c, const cute_grid_spec *s)
+{
+    const bool f32xyz = c->dtype == CUTE_F32 && c->coord == CUTE_COORD_XYZ;
+    return n > 0 && (s->build_path == 2 || (s->build_path == 0 && n >= kPartMinN && !f32xyz));
+}
+
+Layout make_layout(int64_t n, int want_lo, int want_f64, int64_t max_cells, int64_t max_rows, int rec_bytes)
 {
     Layout L;
     memset(&L, 0, sizeof(L));
@@ -61,6 +75,15 @@ Layout make_layout(int64_t n, int want_lo, int want_f64, int64_t max_cells, int6
     L.count = take((size_t)(max_cells + 2) * 4);
     L.cell_start = take((size_t)(max_cells + 2) * 4);
     int64_t m = max_cells > max_rows ? max_cells : max_rows;
+    L.part_G = part_ctas();
+    if (rec_bytes > 0) {
+        int B, cpb;
+        part_shape(max_cells, &B, &cpb);
+        const int64_t tab = (int64_t)B * L.part_G;
+        L.part_tmp = take((size_t)L.n_pad * (size_t)rec_bytes);
+        L.part_table = take((size_t)(2 * tab + 128) * 4);
+        if (tab > m) m = tab;
+    }
     L.scan_tmp = take((size_t)(m / 4096 + 2) * 4);
     L.row_nchunks = take((size_t)(max_rows + 2) * 4);
     L.row_chunk_start = take((size_t)(max_rows + 2) * 4);
@@ -241,7 +264,7 @@ int cute_grid_workspace_bytes(const cute_catalog *cat, const cute_grid_spec *spe
     wants(cat, spec, &want_lo, &want_f64);
     cell_bounds(cat, spec, &mc, &mr);
     if (mc > 0x7ffffff0ll) return CUTE_ERR_INVALID_ARG;
-    *bytes = make_layout(cat->n, want_lo, want_f64, mc, mr).total;
+    *bytes = make_layout(cat->n, want_lo, want_f64, mc, mr, !use_partition(cat->n, cat, spec) ? 0 : (cat->dtype == CUTE_F32 && cat->coord == CUTE_COORD_XYZ) ? 16 : 32).total;
     return CUTE_OK;
 }
 
@@ -258,7 +281,7 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     int64_t mc, mr;
     wants(cat, spec, &want_lo, &want_f64);
     cell_bounds(cat, spec, &mc, &mr);
-    const Layout L = make_layout(cat->n, want_lo, want_f64, mc, mr);
+    const Layout L = make_layout(cat->n, want_lo, want_f64, mc, mr, !use_partition(cat->n, cat, spec) ? 0 : (cat->dtype == CUTE_F32 && cat->coord == CUTE_COORD_XYZ) ? 16 : 32);
     if (bytes < L.total) return CUTE_ERR_WORKSPACE_TOO_SMALL;
     unsigned char *w = (unsigned char *)d_workspace;
 
@@ -398,6 +421,12 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     for (int d = 0; d < 6; d++) g->bbox[d] = bbox[d];
     g->has_bbox = (need_bbox || box_given) ? 1 : 0;
 
+    if (use_partition(cat->n, cat, spec) && b.mode != CUTE_GRID_NONE) {   // large catalogue: two-level partition (grid_build.cu)
+        b.part_tmp = w + L.part_tmp; b.part_table = (uint32_t *)(w + L.part_table); b.part_G = L.part_G;
+        part_shape(b.ncells, &b.part_B, &b.part_cpb);
+        b.part_shift = 0;
+        while ((1 << b.part_shift) < b.part_cpb) b.part_shift++;
+    }
     if (run_build(b, s) != cudaSuccess) { delete g; return CUTE_ERR_CUDA; }
     uint32_t st[3] = {0, 0, 0};
     if (cudaMemcpyAsync(st, b.status, 12, cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess) {

@@ -149,7 +149,23 @@ struct BuildPlan {
     uint32_t *status;  // [0] err, [1] nchunks, [2] largest weight
     double *bbox;      // [6] min xyz, max xyz
     int64_t ncells, nrows;
+    // two-level partition of large catalogues (grid_build.cu): records grouped by bucket, per-(bucket, CTA) counts
+    void *part_tmp;
+    uint32_t *part_table;
+    int part_G, part_B, part_cpb;   // CTAs of the coarse pass, buckets, fine cells per bucket (0: one-pass build)
+    int part_shift;                 // log2(part_cpb)
 };
+
+// large catalogues are built by a coarse partition into buckets of consecutive cells + one CTA per bucket
+constexpr int64_t kPartMinN = 1 << 20;
+constexpr int kPartMaxBuckets = 1024, kPartMaxCellsPerBucket = 16384;
+inline void part_shape(int64_t ncells, int *B, int *cpb)
+{
+    int64_t c = 1;   // a power of two: bucket = cell >> log2(cpb)
+    while (c * kPartMaxBuckets < ncells && c < kPartMaxCellsPerBucket) c *= 2;
+    *cpb = (int)c;
+    *B = (int)((ncells + c - 1) / c);
+}
 cudaError_t run_bbox(const BuildPlan &b, cudaStream_t s);       // leaves 6 order-preserving int64 images in b.bbox
 void decode_bbox(const long long raw[6], double out[6]);
 cudaError_t run_build(const BuildPlan &b, cudaStream_t s);

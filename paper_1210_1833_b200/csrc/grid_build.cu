@@ -83,31 +83,78 @@ cudaError_t run_bbox(const BuildPlan &b, cudaStream_t s)
 // BOX3D: c = floor((x - x0)/a) per axis, id = (cz*ncy + cy)*ncx + cx (x fastest, so a row of
 // neighbours along x is one contiguous range of the sorted array).  SPHERE: pixels with constant
 // limits in (sin dec, RA) -- the paper's "spherical cubes".
-__device__ __forceinline__ bool cell_of(const BuildPlan &b, double a, double c1, double c2, uint32_t &id)
+// floor of a double in [-2^31, 2^31) without a conversion instruction: a round-down add of 2^52 + 2^51 leaves it in the
+// low word (the float64 conversion / rounding instructions run at a fraction of the FP64 add rate)
+__device__ __forceinline__ int floor_magic(double t) { return __double2loint(__dadd_rd(t, 6755399441055744.0)); }
+
+// rare: a point on or outside a face of the box (or not finite): clamp its cell, say whether it is legal.
+// Returns the cell id in the low word and "legal" in bit 32 (everything by value: nothing goes through local memory).
+__device__ __noinline__ unsigned long long cell_fix_box(const BuildPlan &b, double a, double c1, double c2)
+{
+    const double v[3] = {a, c1, c2};
+    int k[3];
+    bool ok = true;
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+        const double t = (v[d] - b.origin[d]) * b.inv_cell[d];
+        int kk = floor_magic(t);
+        // NaN / inf / far-away coordinates fail the magnitude test (their floor_magic is meaningless);
+        // a point exactly on the upper face of a non-periodic box joins the last cell
+        const bool in = fabs(t) < 2147483648.0 && kk >= 0;
+        if (!in || kk >= b.nc[d]) {
+            if (!in || b.periodic || !(v[d] - b.origin[d] <= b.size[d])) ok = false;
+            kk = in ? b.nc[d] - 1 : 0;
+        }
+        k[d] = kk;
+    }
+    const uint32_t id = (uint32_t)((k[2] * b.nc[1] + k[1]) * b.nc[0] + k[0]);
+    return (unsigned long long)id | (ok ? 1ull << 32 : 0ull);
+}
+
+template <int MODE>
+__device__ __forceinline__ bool cell_of_t(const BuildPlan &b, double a, double c1, double c2, uint32_t &id)
 {
     bool ok = true;
     int k[3] = {0, 0, 0};
-    if (b.mode == CUTE_GRID_BOX3D) {
-        double v[3] = {a, c1, c2};
-        for (int d = 0; d < 3; d++) {
-            double t = floor((v[d] - b.origin[d]) * b.inv_cell[d]);
-            if (!(t >= 0.0) || !(v[d] - b.origin[d] <= b.size[d]) || (b.periodic && !(v[d] < b.origin[d] + b.size[d]))) ok = false;
-            int kk = (t >= 0.0) ? (t < (double)b.nc[d] ? (int)t : b.nc[d] - 1) : 0;
-            k[d] = kk;
+    if (MODE == CUTE_GRID_BOX3D) {
+        const double t0 = (a - b.origin[0]) * b.inv_cell[0], t1 = (c1 - b.origin[1]) * b.inv_cell[1], t2 = (c2 - b.origin[2]) * b.inv_cell[2];
+        k[0] = floor_magic(t0); k[1] = floor_magic(t1); k[2] = floor_magic(t2);
+        const bool fine = fabs(t0) < 2147483648.0 && fabs(t1) < 2147483648.0 && fabs(t2) < 2147483648.0 &&
+                          (uint32_t)k[0] < (uint32_t)b.nc[0] && (uint32_t)k[1] < (uint32_t)b.nc[1] && (uint32_t)k[2] < (uint32_t)b.nc[2];
+        if (!fine) {
+            const unsigned long long r = cell_fix_box(b, a, c1, c2);
+            id = (uint32_t)r;
+            return (r >> 32) != 0;
         }
-    } else if (b.mode == CUTE_GRID_SPHERE) {
-        double al = fmod(a - b.origin[0], 360.0);
+    } else if (MODE == CUTE_GRID_SPHERE) {
+        double al = a - b.origin[0];
+        al -= 360.0 * (double)floor_magic(al * (1.0 / 360.0));          // RA modulo 360 relative to RA0
         if (al < 0.0) al += 360.0;
-        if (!(al >= 0.0) || !(al <= b.size[0])) ok = false;
-        double t = floor(al * b.inv_cell[0]);
-        k[0] = (t >= 0.0) ? (t < (double)b.nc[0] ? (int)t : b.nc[0] - 1) : 0;
+        if (al >= 360.0) al -= 360.0;
+        if (!(al >= 0.0) || !(al <= b.size[0]) || !(fabs(a) < 1.0e9) || !isfinite(c1) || !isfinite(c2)) ok = false;
+        double t = al * b.inv_cell[0];
+        k[0] = (t >= 0.0) ? (t < (double)b.nc[0] ? floor_magic(t) : b.nc[0] - 1) : 0;
         double u = sin(c1 * (kPi / 180.0)) - b.origin[1];
         if (!(u >= -1e-15) || !(u <= b.size[1] + 1e-15)) ok = false;
-        t = floor(u * b.inv_cell[1]);
-        k[1] = (t >= 0.0) ? (t < (double)b.nc[1] ? (int)t : b.nc[1] - 1) : 0;
+        t = u * b.inv_cell[1];
+        k[1] = (t >= 0.0) ? (t < (double)b.nc[1] ? floor_magic(t) : b.nc[1] - 1) : 0;
     }
     id = (uint32_t)((k[2] * b.nc[1] + k[1]) * b.nc[0] + k[0]);
     return ok;
+}
+
+__device__ __forceinline__ bool cell_of(const BuildPlan &b, double a, double c1, double c2, uint32_t &id)
+{
+    if (b.mode == CUTE_GRID_BOX3D) return cell_of_t<CUTE_GRID_BOX3D>(b, a, c1, c2, id);
+    if (b.mode == CUTE_GRID_SPHERE) return cell_of_t<CUTE_GRID_SPHERE>(b, a, c1, c2, id);
+    id = 0;
+    return true;
+}
+
+template <int DT>
+__device__ __forceinline__ double load_coord_t(const void *p, int64_t i)
+{
+    return DT == CUTE_F64 ? reinterpret_cast<const double *>(p)[i] : (double)reinterpret_cast<const float *>(p)[i];
 }
 
 // kPts points per thread, loads issued before their uses: these kernels are bound by the latency of dependent
@@ -219,6 +266,31 @@ static cudaError_t exclusive_scan(const uint32_t *in, int64_t n, uint32_t *out, 
 // sin d) in float64 ("projects all objects in the catalog into the unit sphere"),
 // then the same hi/lo split; w carries float32(z) for RADECZ.  p64 keeps the float64 values for
 // the refine path.
+__device__ __forceinline__ void emit_point(const BuildPlan &b, uint32_t slot, double a, double c1, double c2, uint32_t i)
+{
+    // XYZ: w carries |x|^2 split hi/lo, so that the (r,mu) kernel gets s.l = |x_i|^2 - |x_j|^2 without
+    // cancellation (l = x_i + x_j is the mid-point line of sight)
+    double v[4] = {a, c1, c2, a * a + c1 * c1 + c2 * c2};
+    if (b.coord != CUTE_COORD_XYZ) {
+        double al = a * (kPi / 180.0), de = c1 * (kPi / 180.0), sa, ca, sd, cd;
+        sincos(al, &sa, &ca);
+        sincos(de, &sd, &cd);
+        v[0] = cd * ca; v[1] = cd * sa; v[2] = sd; v[3] = c2;
+    }
+    float h[4], l[4];
+    for (int d = 0; d < 4; d++) { h[d] = (float)v[d]; l[d] = (float)(v[d] - (double)h[d]); }
+    if (b.weight) {   // integer weight: bit pattern in hi.w (the pair kernel multiplies integers), exact double in p64
+        const uint32_t w = b.weight[i];
+        h[3] = __uint_as_float(w); l[3] = 0.f; v[3] = (double)w;
+        if (w == 0u || w > 65535u) atomicExch(&b.status[0], 1u);
+        atomicMax(&b.status[2], w);
+    }
+    b.hi[slot] = make_float4(h[0], h[1], h[2], h[3]);
+    if (b.want_lo) b.lo[slot] = make_float4(l[0], l[1], l[2], l[3]);
+    if (b.want_f64) for (int d = 0; d < 4; d++) b.p64[(size_t)d * b.n_pad + slot] = v[d];
+    if (b.perm) b.perm[slot] = i;
+}
+
 __global__ void __launch_bounds__(256) k_scatter(BuildPlan b)
 {
     const int64_t base = (int64_t)blockIdx.x * (blockDim.x * kPts) + threadIdx.x;
@@ -251,28 +323,242 @@ __global__ void __launch_bounds__(256) k_scatter(BuildPlan b)
     for (int k = 0; k < kPts; k++) {
         const int64_t i = base + (int64_t)k * blockDim.x;
         if (i >= b.n) continue;
-        // XYZ: w carries |x|^2 split hi/lo, so that the (r,mu) kernel gets s.l = |x_i|^2 - |x_j|^2 without
-        // cancellation (l = x_i + x_j is the mid-point line of sight)
-        double v[4] = {a[k], c1[k], c2[k], a[k] * a[k] + c1[k] * c1[k] + c2[k] * c2[k]};
-        if (b.coord != CUTE_COORD_XYZ) {
-            double al = a[k] * (kPi / 180.0), de = c1[k] * (kPi / 180.0), sa, ca, sd, cd;
-            sincos(al, &sa, &ca);
-            sincos(de, &sd, &cd);
-            v[0] = cd * ca; v[1] = cd * sa; v[2] = sd; v[3] = c2[k];
-        }
-        float h[4], l[4];
-        for (int d = 0; d < 4; d++) { h[d] = (float)v[d]; l[d] = (float)(v[d] - (double)h[d]); }
-        if (b.weight) {   // integer weight: bit pattern in hi.w (the pair kernel multiplies integers), exact double in p64
-            const uint32_t w = b.weight[i];
-            h[3] = __uint_as_float(w); l[3] = 0.f; v[3] = (double)w;
-            if (w == 0u || w > 65535u) atomicExch(&b.status[0], 1u);
-            atomicMax(&b.status[2], w);
-        }
-        b.hi[slot[k]] = make_float4(h[0], h[1], h[2], h[3]);
-        if (b.want_lo) b.lo[slot[k]] = make_float4(l[0], l[1], l[2], l[3]);
-        if (b.want_f64) for (int d = 0; d < 4; d++) b.p64[(size_t)d * b.n_pad + slot[k]] = v[d];
-        if (b.perm) b.perm[slot[k]] = (uint32_t)i;
+        emit_point(b, slot[k], a[k], c1[k], c2[k], (uint32_t)i);
     }
+}
+
+
+// ---- large catalogues: two-level partition ------------------------------------------------------
+// The one-pass build above gives every point a random 16-byte store and a returning L2 atomic; at 10^7
+// points in random order that is half-used DRAM sectors and ~2x the algorithmic traffic (round-1 ncu).
+// Here instead: (1) a coarse pass groups the raw records into <= 1024 BUCKETS of consecutive cells -- each
+// CTA owns a contiguous slice of the input and, per bucket, a private output range found by a scan of the
+// per-(bucket, CTA) counts, so its shared-memory cursors hand out consecutive slots and L2 sees every line
+// filled before it is evicted; (2) one CTA per bucket counts, scans and scatters its few hundred cells
+// entirely in shared memory and writes cell_start itself.  No global atomics, every DRAM sector whole.
+struct Rec32 { double a, c1, c2; uint32_t idx, cell; };   // raw record of a float64 / RA-Dec catalogue (+ its cell)
+
+template <int DT>
+__device__ __forceinline__ void load_raw(const BuildPlan &b, uint32_t i, double &a, double &c1, double &c2)
+{
+    a = load_coord_t<DT>(b.c0, i); c1 = load_coord_t<DT>(b.c1, i);
+    c2 = b.coord != CUTE_COORD_RADEC ? load_coord_t<DT>(b.c2, i) : 0.0;
+}
+
+template <int MODE, int DT>
+__global__ void __launch_bounds__(512) k_part_hist(BuildPlan b)
+{
+    extern __shared__ uint32_t sh[];
+    const int B = b.part_B, G = b.part_G, g = blockIdx.x;
+    for (int k = threadIdx.x; k < B; k += blockDim.x) sh[k] = 0;
+    __syncthreads();
+    const uint32_t per = (uint32_t)((b.n + G - 1) / G), i0 = min((uint32_t)b.n, (uint32_t)g * per), i1 = min((uint32_t)b.n, i0 + per);
+    const uint32_t T = blockDim.x, shift = (uint32_t)b.part_shift;
+    bool bad = false;
+    uint32_t base = i0;
+    for (; base + T * kPts <= i1; base += T * kPts) {        // full trips: no bounds checks, all loads in flight first
+        double a[kPts], c1[kPts], c2[kPts];
+#pragma unroll
+        for (int k = 0; k < kPts; k++) load_raw<DT>(b, base + threadIdx.x + (uint32_t)k * T, a[k], c1[k], c2[k]);
+#pragma unroll
+        for (int k = 0; k < kPts; k++) {
+            uint32_t id;
+            bad = !cell_of_t<MODE>(b, a[k], c1[k], c2[k], id) || bad;   // (not finite => not ok)
+            atomicAdd(&sh[id >> shift], 1u);
+        }
+    }
+    for (uint32_t i = base + threadIdx.x; i < i1; i += T) {
+        double a, c1, c2;
+        load_raw<DT>(b, i, a, c1, c2);
+        uint32_t id;
+        bad = !cell_of_t<MODE>(b, a, c1, c2, id) || bad;
+        atomicAdd(&sh[id >> shift], 1u);
+    }
+    if (bad) atomicExch(&b.status[0], 1u);
+    __syncthreads();
+    for (int k = threadIdx.x; k < B; k += blockDim.x) b.part_table[(size_t)k * G + g] = sh[k];
+}
+
+template <bool F32REC>
+__device__ __forceinline__ void store_rec(const BuildPlan &b, uint32_t slot, double a, double c1, double c2, uint32_t i, uint32_t id)
+{
+    if (F32REC) reinterpret_cast<float4 *>(b.part_tmp)[slot] = make_float4((float)a, (float)c1, (float)c2, __uint_as_float(i));
+    else {
+        Rec32 r; r.a = a; r.c1 = c1; r.c2 = c2; r.idx = i; r.cell = id;
+        reinterpret_cast<Rec32 *>(b.part_tmp)[slot] = r;
+    }
+}
+
+template <int MODE, int DT, bool F32REC>
+__global__ void __launch_bounds__(512) k_part_scatter(BuildPlan b, const uint32_t *table_start)
+{
+    extern __shared__ uint32_t sh[];
+    const int B = b.part_B, G = b.part_G, g = blockIdx.x;
+    for (int k = threadIdx.x; k < B; k += blockDim.x) sh[k] = table_start[(size_t)k * G + g];
+    __syncthreads();
+    const uint32_t per = (uint32_t)((b.n + G - 1) / G), i0 = min((uint32_t)b.n, (uint32_t)g * per), i1 = min((uint32_t)b.n, i0 + per);
+    const uint32_t T = blockDim.x, shift = (uint32_t)b.part_shift;
+    uint32_t base = i0;
+    for (; base + T * kPts <= i1; base += T * kPts) {
+        double a[kPts], c1[kPts], c2[kPts];
+#pragma unroll
+        for (int k = 0; k < kPts; k++) load_raw<DT>(b, base + threadIdx.x + (uint32_t)k * T, a[k], c1[k], c2[k]);
+#pragma unroll
+        for (int k = 0; k < kPts; k++) {
+            uint32_t id;
+            cell_of_t<MODE>(b, a[k], c1[k], c2[k], id);
+            store_rec<F32REC>(b, atomicAdd(&sh[id >> shift], 1u), a[k], c1[k], c2[k], base + threadIdx.x + (uint32_t)k * T, id);
+        }
+    }
+    for (uint32_t i = base + threadIdx.x; i < i1; i += T) {
+        double a, c1, c2;
+        load_raw<DT>(b, i, a, c1, c2);
+        uint32_t id;
+        cell_of_t<MODE>(b, a, c1, c2, id);
+        store_rec<F32REC>(b, atomicAdd(&sh[id >> shift], 1u), a, c1, c2, i, id);
+    }
+}
+
+template <bool F32REC>
+__device__ __forceinline__ void load_rec(const BuildPlan &b, uint32_t s, double &a, double &c1, double &c2, uint32_t &idx, uint32_t &cell)
+{
+    if (F32REC) {   // float32 xyz: no room for the cell in 16 bytes, recomputed (three FP64 multiply-adds)
+        const float4 r = reinterpret_cast<const float4 *>(b.part_tmp)[s];
+        a = r.x; c1 = r.y; c2 = r.z; idx = __float_as_uint(r.w);
+        cell_of_t<CUTE_GRID_BOX3D>(b, a, c1, c2, cell);
+    } else {
+        const Rec32 r = reinterpret_cast<const Rec32 *>(b.part_tmp)[s];
+        a = r.a; c1 = r.c1; c2 = r.c2; idx = r.idx; cell = r.cell;
+    }
+}
+
+// One CTA per bucket.  The bucket's records are staged in shared memory (one coalesced read from HBM), its cells
+// counted and scanned there, and every record is then emitted to its final slot: scattered 16-byte stores, but inside a
+// window of a few hundred KB that L2 holds until its lines are whole.  A bucket too large for shared memory (a very
+// clustered catalogue) is swept twice from global memory instead (the second sweep hits L2).
+template <bool F32REC>
+__global__ void __launch_bounds__(1024) k_part_fine(BuildPlan b, const uint32_t *table_start, uint32_t cap)
+{
+    extern __shared__ __align__(16) unsigned char fsm[];
+    __shared__ uint32_t wsum[32];
+    const int bk = blockIdx.x, G = b.part_G, cpb = b.part_cpb;
+    uint32_t *cnt = reinterpret_cast<uint32_t *>(fsm);          // [cpb] counts, then starts, then cursors
+    unsigned char *stage = fsm + (((size_t)cpb * 4 + 15) & ~(size_t)15);
+    const uint32_t bs = table_start[(size_t)bk * G], be = table_start[(size_t)(bk + 1) * G];
+    const int64_t c0 = (int64_t)bk * cpb;
+    const int nc = (int)min((int64_t)cpb, b.ncells - c0);
+    const bool staged = be - bs <= cap;
+    const uint32_t T = blockDim.x;
+    for (int k = threadIdx.x; k < nc; k += T) cnt[k] = 0;
+    __syncthreads();
+    if (staged) {
+        if (F32REC) {
+            const float4 *src = reinterpret_cast<const float4 *>(b.part_tmp) + bs;
+            float4 *dst = reinterpret_cast<float4 *>(stage);
+            for (uint32_t s = threadIdx.x; s < be - bs; s += T) {
+                const float4 r = src[s];
+                dst[s] = r;
+                uint32_t id;
+                cell_of_t<CUTE_GRID_BOX3D>(b, (double)r.x, (double)r.y, (double)r.z, id);
+                atomicAdd(&cnt[id - (uint32_t)c0], 1u);
+            }
+        } else {
+            const Rec32 *src = reinterpret_cast<const Rec32 *>(b.part_tmp) + bs;
+            Rec32 *dst = reinterpret_cast<Rec32 *>(stage);
+            for (uint32_t s = threadIdx.x; s < be - bs; s += T) {
+                const Rec32 r = src[s];
+                dst[s] = r;
+                atomicAdd(&cnt[r.cell - (uint32_t)c0], 1u);
+            }
+        }
+    } else {
+        for (uint32_t s = bs + threadIdx.x; s < be; s += T) {
+            double a, c1, c2; uint32_t idx, id;
+            load_rec<F32REC>(b, s, a, c1, c2, idx, id);
+            atomicAdd(&cnt[id - (uint32_t)c0], 1u);
+        }
+    }
+    __syncthreads();
+    // exclusive scan of cnt[0..nc): each thread owns a run of consecutive cells
+    const int per = (nc + (int)T - 1) / (int)T;
+    const int k0 = min(nc, (int)threadIdx.x * per), k1 = min(nc, k0 + per);
+    uint32_t tsum = 0;
+    for (int k = k0; k < k1; k++) tsum += cnt[k];
+    uint32_t x = tsum;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+    if (lane == 31) wsum[wid] = x;
+    __syncthreads();
+    if (wid == 0) {
+        uint32_t v = lane < (int)(T >> 5) ? wsum[lane] : 0u;
+        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, v, o); if (lane >= o) v += y; }
+        wsum[lane] = v;
+    }
+    __syncthreads();
+    uint32_t run = (wid ? wsum[wid - 1] : 0u) + x - tsum;
+    for (int k = k0; k < k1; k++) {
+        const uint32_t c = cnt[k];
+        cnt[k] = run;                                           // local start = cursor
+        b.cell_start[c0 + k] = bs + run;
+        run += c;
+    }
+    if (bk == (int)gridDim.x - 1 && threadIdx.x == 0) b.cell_start[b.ncells] = (uint32_t)b.n;
+    __syncthreads();
+    if (staged) {
+        for (uint32_t s = threadIdx.x; s < be - bs; s += T) {
+            double a, c1, c2; uint32_t idx, id;
+            if (F32REC) {
+                const float4 r = reinterpret_cast<const float4 *>(stage)[s];
+                a = r.x; c1 = r.y; c2 = r.z; idx = __float_as_uint(r.w);
+                cell_of_t<CUTE_GRID_BOX3D>(b, a, c1, c2, id);
+            } else {
+                const Rec32 r = reinterpret_cast<const Rec32 *>(stage)[s];
+                a = r.a; c1 = r.c1; c2 = r.c2; idx = r.idx; id = r.cell;
+            }
+            emit_point(b, bs + atomicAdd(&cnt[id - (uint32_t)c0], 1u), a, c1, c2, idx);
+        }
+    } else {
+        for (uint32_t s = bs + threadIdx.x; s < be; s += T) {   // second sweep: the bucket is L2-resident
+            double a, c1, c2; uint32_t idx, id;
+            load_rec<F32REC>(b, s, a, c1, c2, idx, id);
+            emit_point(b, bs + atomicAdd(&cnt[id - (uint32_t)c0], 1u), a, c1, c2, idx);
+        }
+    }
+}
+
+static cudaError_t run_partition_build(const BuildPlan &b, cudaStream_t s)
+{
+    cudaError_t e;
+    const bool f32rec = b.dtype == CUTE_F32 && b.coord == CUTE_COORD_XYZ;
+    const size_t sh1 = (size_t)b.part_B * 4;
+    uint32_t *table_start = b.part_table + (((size_t)b.part_B * b.part_G + 63) / 64 * 64 + 64);
+    const bool box = b.mode == CUTE_GRID_BOX3D, f64 = b.dtype == CUTE_F64;
+    if (box && f64) k_part_hist<CUTE_GRID_BOX3D, CUTE_F64><<<b.part_G, 512, sh1, s>>>(b);
+    else if (box) k_part_hist<CUTE_GRID_BOX3D, CUTE_F32><<<b.part_G, 512, sh1, s>>>(b);
+    else if (f64) k_part_hist<CUTE_GRID_SPHERE, CUTE_F64><<<b.part_G, 512, sh1, s>>>(b);
+    else k_part_hist<CUTE_GRID_SPHERE, CUTE_F32><<<b.part_G, 512, sh1, s>>>(b);
+    if ((e = exclusive_scan(b.part_table, (int64_t)b.part_B * b.part_G, table_start, b.scan_tmp, s)) != cudaSuccess) return e;
+    // fine pass: shared memory = cell counters + staging for a bucket 1.5x the mean size (at least 64 KB, at most 200 KB)
+    const size_t cnt_b = ((size_t)b.part_cpb * 4 + 15) & ~(size_t)15, rec_b = f32rec ? 16 : 32;
+    size_t want = (size_t)(1.5 * (double)b.n / (double)b.part_B) * rec_b + 4096;
+    want = want < 64 * 1024 ? 64 * 1024 : want;
+    size_t sh2 = cnt_b + want;
+    if (sh2 > 200 * 1024) sh2 = 200 * 1024;
+    const uint32_t cap = sh2 > cnt_b ? (uint32_t)((sh2 - cnt_b) / rec_b) : 0u;
+    if (f32rec) {
+        if ((e = cudaFuncSetAttribute(k_part_fine<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh2)) != cudaSuccess) return e;
+        k_part_scatter<CUTE_GRID_BOX3D, CUTE_F32, true><<<b.part_G, 512, sh1, s>>>(b, table_start);
+        k_part_fine<true><<<b.part_B, 1024, sh2, s>>>(b, table_start, cap);
+    } else {
+        if ((e = cudaFuncSetAttribute(k_part_fine<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh2)) != cudaSuccess) return e;
+        if (box && f64) k_part_scatter<CUTE_GRID_BOX3D, CUTE_F64, false><<<b.part_G, 512, sh1, s>>>(b, table_start);
+        else if (box) k_part_scatter<CUTE_GRID_BOX3D, CUTE_F32, false><<<b.part_G, 512, sh1, s>>>(b, table_start);
+        else if (f64) k_part_scatter<CUTE_GRID_SPHERE, CUTE_F64, false><<<b.part_G, 512, sh1, s>>>(b, table_start);
+        else k_part_scatter<CUTE_GRID_SPHERE, CUTE_F32, false><<<b.part_G, 512, sh1, s>>>(b, table_start);
+        k_part_fine<false><<<b.part_B, 1024, sh2, s>>>(b, table_start, cap);
+    }
+    note_launches(3);
+    return cudaGetLastError();
 }
 
 // ---- G4: chunk table ---------------------------------------------------------------------------
@@ -283,6 +569,31 @@ __global__ void k_row_counts(BuildPlan b)
     uint32_t n = (b.mode == CUTE_GRID_NONE || b.order_only) ? (uint32_t)b.n
                                               : b.cell_start[(r + 1) * b.nc[0]] - b.cell_start[r * b.nc[0]];
     b.row_nchunks[r] = (n + kChunk - 1) / kChunk;
+}
+
+// rows <= 4096 * 1024 / ... : the common case (C5: 1600 rows, C4: ~3700) in ONE block instead of four launches
+__global__ void __launch_bounds__(1024) k_row_scan_small(BuildPlan b)
+{
+    __shared__ uint32_t sh[32];
+    __shared__ uint32_t carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    const bool one_row = (b.mode == CUTE_GRID_NONE || b.order_only);
+    for (int64_t r0 = 0; r0 < b.nrows; r0 += blockDim.x) {
+        const int64_t r = r0 + threadIdx.x;
+        uint32_t v = 0;
+        if (r < b.nrows) {
+            const uint32_t n = one_row ? (uint32_t)b.n : b.cell_start[(r + 1) * b.nc[0]] - b.cell_start[r * b.nc[0]];
+            v = (n + kChunk - 1) / kChunk;
+        }
+        uint32_t tot;
+        const uint32_t e = block_excl_scan(v, &tot, sh);
+        if (r < b.nrows) b.row_chunk_start[r] = e + carry;
+        __syncthreads();
+        if (threadIdx.x == 0) carry += tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) b.row_chunk_start[b.nrows] = carry;
 }
 
 __global__ void k_chunks(BuildPlan b, uint32_t max_chunks)
@@ -349,20 +660,26 @@ cudaError_t run_build(const BuildPlan &b, cudaStream_t s)
     const int T = 256;
     const int pblocks = (int)((b.n + (int64_t)T * kPts - 1) / ((int64_t)T * kPts));
     if ((e = cudaMemsetAsync(b.status, 0, 12, s)) != cudaSuccess) return e;
-    if (b.mode != CUTE_GRID_NONE) {
+    if (b.mode != CUTE_GRID_NONE && b.part_cpb > 0 && b.n > 0) {
+        if ((e = run_partition_build(b, s)) != cudaSuccess) return e;
+    } else if (b.mode != CUTE_GRID_NONE) {
         if ((e = cudaMemsetAsync(b.count, 0, (size_t)(b.ncells + 1) * 4, s)) != cudaSuccess) return e;
         if (b.n > 0) { k_cellid<<<pblocks, T, 0, s>>>(b); note_launches(1); }
         if ((e = exclusive_scan(b.count, b.ncells, b.cell_start, b.scan_tmp, s)) != cudaSuccess) return e;
         // the counters become the per-cell write cursors of the scatter
         if ((e = cudaMemcpyAsync(b.count, b.cell_start, (size_t)b.ncells * 4, cudaMemcpyDeviceToDevice, s)) != cudaSuccess) return e;
     }
-    if (b.n > 0) { k_scatter<<<pblocks, T, 0, s>>>(b); note_launches(1); }
-    k_row_counts<<<(int)((b.nrows + T - 1) / T), T, 0, s>>>(b);
-    if ((e = exclusive_scan(b.row_nchunks, b.nrows, b.row_chunk_start, b.scan_tmp, s)) != cudaSuccess) return e;
+    if (b.n > 0 && !(b.mode != CUTE_GRID_NONE && b.part_cpb > 0)) { k_scatter<<<pblocks, T, 0, s>>>(b); note_launches(1); }
+    if (b.nrows <= 65536) { k_row_scan_small<<<1, 1024, 0, s>>>(b); note_launches(1); }
+    else {
+        k_row_counts<<<(int)((b.nrows + T - 1) / T), T, 0, s>>>(b);
+        note_launches(1);
+        if ((e = exclusive_scan(b.row_nchunks, b.nrows, b.row_chunk_start, b.scan_tmp, s)) != cudaSuccess) return e;
+    }
     uint32_t max_chunks = (uint32_t)(b.n / kChunk + b.nrows + 1);
     k_chunks<<<(max_chunks + T - 1) / T, T, 0, s>>>(b, max_chunks);
     if (b.mode == CUTE_GRID_SPHERE && !b.order_only) { k_sphere_rows<<<(b.nc[1] + T - 1) / T, T, 0, s>>>(b); note_launches(1); }
-    note_launches(2);   // k_row_counts, k_chunks
+    note_launches(1);   // k_chunks
     return cudaGetLastError();
 }
 

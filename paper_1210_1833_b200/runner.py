@@ -62,7 +62,8 @@ class Job:
             inf = self.g_data.info()
             self.spec = api.grid_spec("box3d", periodic=bool(self.spec.periodic), origin=tuple(inf.origin),
                                       size=tuple(inf.size), ncell=tuple(inf.ncell),
-                                      rmax=self.spec.rmax, kind_mask=self.spec.kind_mask, no_perm=self.spec.no_perm)
+                                      rmax=self.spec.rmax, kind_mask=self.spec.kind_mask, no_perm=self.spec.no_perm,
+                                      build_path=self.spec.build_path)
         if self.d_rand is not None:
             if self.g_rand is not None:
                 self.g_rand.free()

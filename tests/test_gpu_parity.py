@@ -279,12 +279,15 @@ def test_permutation_invariance_and_sharding(rt):
     assert np.array_equal(acc, out["DR"][0])
 
 
-def test_cell_list_is_a_permutation(rt):
+@pytest.mark.parametrize("build_path", [1, 2])
+def test_cell_list_is_a_permutation(rt, build_path):
     """G1-G3 bit-exact: perm is a permutation, cell_start is the exclusive scan of the cell histogram,
-    and every sorted point lies in its cell."""
+    and every sorted point lies in its cell -- for the one-pass counting sort (1) and for the two-level
+    partition that large catalogues take (2)."""
     import torch
     api, runner, synth = rt
     w = synth.workload(5, 0.003)
+    w.grid = dict(w.grid, build_path=build_path)
     job = runner.job_for_workload(w).build()
     inf = job.g_data.info()
     n, nc = inf.n, inf.ncells
@@ -454,3 +457,99 @@ def test_monopole_log_bins_far_from_origin(rt, oracle):
     x = tuple(np.concatenate([c[:500], c[:500]]) for c in w.data)
     out2, _ = _run(runner, "monopole", x, None, bins, dict(mode="none"))
     _parity(oracle, out2["DD"][0], "monopole", x, None, bins)
+
+
+@pytest.mark.parametrize("cfg,scale", [(2, 0.02), (3, 0.02), (4, 0.02), (5, 0.002)])
+def test_partition_build_gives_the_same_histograms(rt, oracle, cfg, scale):
+    """the two-level partition build (build_path 2) and the one-pass build (1) are the same cell list up to the order
+    inside a cell: identical histograms for every kind, coordinate type and grid mode (float64 RA/Dec/z and xyz, float32
+    xyz; brute-force ordering cells, pixels, periodic and bounding-box cells)"""
+    api, runner, synth = rt
+    w = synth.workload(cfg, scale)
+    outs = []
+    for bp in (1, 2):
+        out, job = _run(runner, w.kind, w.data, w.rand, w.bins, dict(w.grid, build_path=bp), which=tuple(w.pairs))
+        outs.append(out)
+    for k in w.pairs:
+        assert np.array_equal(outs[0][k][0], outs[1][k][0])
+    c2 = w.rand if "DR" in w.pairs else None
+    which = "DR" if c2 is not None else "DD"
+    _parity(oracle, outs[1][which][0], w.kind, w.data, c2, w.bins, mode="celled" if w.grid.get("mode", "none") != "none" else "plain")
+
+
+@pytest.mark.parametrize("n,theta_deg,pix", [(20000, 10.0, 0.1), (3000, 20.0, 0.05), (9000, 3.0, 0.2)])
+def test_sphere_ring_rows_with_mixed_chunks(rt, n, theta_deg, pix):
+    """Regression (round-1 advisor): on a full ring, rows holding a little more than a multiple of 128 points mix a chunk
+    whose window covers the whole ring with one whose window does not; seam pairs of the row's own points were then
+    counted twice or dropped.  Full sky, fine pixels, 130-260 points per row, wide windows at high declination:
+    the pixel grid must equal brute force exactly."""
+    api, runner, synth = rt
+    rng = np.random.default_rng(77 + n)
+    ra = rng.random(n) * 360.0
+    dec = np.degrees(np.arcsin(rng.random(n) * 2 - 1))
+    th = math.radians(theta_deg)
+    bins = dict(n1=24, lo1=0.0, hi1=th, log1=0, n2=0, lo2=0.0, hi2=0.0, aperture=0.0, box_L=0.0)
+    out_g, job = _run(runner, "angular", (ra, dec), None, bins, dict(mode="sphere", thetamax=th, pix=pix))
+    assert job.spec.size[0] == 360.0
+    per_row = n / job.spec.ncell[1]
+    assert 10 < per_row < 400, per_row
+    out_b, _ = _run(runner, "angular", (ra, dec), None, bins, dict(mode="none"))
+    assert np.array_equal(out_g["DD"][0], out_b["DD"][0])
+    # and a second catalogue through the same grid (cross: every row window is met exactly once)
+    m = n // 2
+    ra2, dec2 = rng.random(m) * 360.0, np.degrees(np.arcsin(rng.random(m) * 2 - 1))
+    out_g, _ = _run(runner, "angular", (ra, dec), (ra2, dec2), bins, dict(mode="sphere", thetamax=th, pix=pix), which=("DR",))
+    out_b, _ = _run(runner, "angular", (ra, dec), (ra2, dec2), bins, dict(mode="none"), which=("DR",))
+    assert np.array_equal(out_g["DR"][0], out_b["DR"][0])
+
+
+def test_refine_path_against_enumeration_and_eq9(rt):
+    """The float64 refine path decides EVERY pair under force_refine.  It is compared here with counts that do not come
+    from the oracle: (i) the torus-lattice enumeration of integer vectors (Eq. 11 PAPER.md:85 with the periodic wrap of
+    PAPER.md:94) and (ii) r, mu from Eq. 9 for pairs built from (chi_1, chi_2, theta)."""
+    import itertools
+    api, runner, synth = rt
+    n, h = 6, 1.5
+    L = n * h
+    g = np.arange(n) * h + 0.25
+    x = np.array(list(itertools.product(g, g, g))).T
+    x = x[:, np.random.default_rng(5).permutation(x.shape[1])]
+    bins = dict(n1=29, lo1=0.05 * h, hi1=2.95 * h, log1=0, n2=0, lo2=0.0, hi2=0.0, aperture=0.0, box_L=L)
+    edges = bins["lo1"] + (bins["hi1"] - bins["lo1"]) * np.arange(30) / 29
+    want = np.zeros(29, dtype=np.int64)
+    rep = range(-n // 2, n // 2)
+    for v in itertools.product(rep, rep, rep):
+        m = v[0] ** 2 + v[1] ** 2 + v[2] ** 2
+        if m == 0:
+            continue
+        r = h * math.sqrt(m)
+        k = np.searchsorted(edges, r, side="right") - 1
+        if 0 <= k < 29 and r < edges[-1]:
+            want[k] += 1
+    want = want * n ** 3 // 2
+    for opts in (dict(force_refine=1), None):
+        out, _ = _run(runner, "monopole", tuple(x), None, bins, dict(mode="none"), opts)
+        assert np.array_equal(out["DD"][0].astype(np.int64), want)
+    # Eq. 9: one pair per catalogue, (r, mu) cell from the closed form
+    rng = np.random.default_rng(41)
+    nr, nm = 64, 64
+    b2 = dict(n1=nr, lo1=0.0, hi1=400.0, log1=0, n2=nm, lo2=0.0, hi2=1.0, aperture=0.0, box_L=0.0)
+    checked = 0
+    for _ in range(60):
+        c1, c2 = 1000.0 + 600.0 * rng.random(2)
+        th = 0.15 * rng.random()
+        r9 = math.sqrt(c1 * c1 + c2 * c2 - 2 * c1 * c2 * math.cos(th))
+        mu9 = abs(c1 * c1 - c2 * c2) / math.sqrt((c1 * c1 + c2 * c2) ** 2 - 4 * c1 * c1 * c2 * c2 * math.cos(th) ** 2)
+        u = rng.normal(size=3); u /= np.linalg.norm(u)
+        v = rng.normal(size=3); v -= v.dot(u) * u; v /= np.linalg.norm(v)
+        x1, x2 = c1 * u, c2 * (math.cos(th) * u + math.sin(th) * v)
+        tr, tm = r9 / 400.0 * nr, mu9 * nm
+        if r9 >= 399.0 or min(tr % 1, 1 - tr % 1, tm % 1, 1 - tm % 1) < 1e-6:
+            continue
+        cell = int(tr) * nm + min(int(tm), nm - 1)
+        for opts in (dict(force_refine=1), None):
+            out, _ = _run(runner, "rmu", tuple(np.array([x1, x2]).T), None, b2, dict(mode="none"), opts)
+            hh = out["DD"][0]
+            assert hh.sum() == 1 and hh[cell] == 1, (r9, mu9, opts)
+        checked += 1
+    assert checked > 40

@@ -465,3 +465,65 @@ def test_pixelised_counts_approach_the_exact_ones_above_the_pixel_scale(oracle):
     a = oracle.count("angular", (ra, dec), None, small)["hist"]
     b = oracle.count("angular", (pra, pdec), None, small, w1=pw)["hist"]
     assert b[0] == (pw.astype(np.int64) * (pw.astype(np.int64) - 1) // 2).sum() and b[1:].sum() == 0 and a[1:].sum() > 0
+
+
+# ---------------------------------------------------------------- 2-D ambiguity cells (parity rule)
+def _rmu_pair(r, mu, chi=1000.0):
+    """two points whose mid-point line of sight is the z axis exactly: s = r (sqrt(1-mu^2), 0, mu), l = 2 chi z"""
+    t = math.sqrt(max(0.0, 1.0 - mu * mu))
+    return (np.array([0.5 * r * t, -0.5 * r * t]), np.zeros(2), np.array([chi + 0.5 * r * mu, chi - 0.5 * r * mu]))
+
+
+def test_amb_cell_composition_two_axes(oracle):
+    """`amb_cell` of a 2-D histogram: every cell a flagged pair could land in when the flagged variable(s) cross their
+    edge -- the product of the candidate bins of both axes, out-of-range candidates going to the virtual cell.  Hand
+    cases on 10 x 10 bins of width 1 in r and 0.1 in mu (cell = 10 k_r + k_mu)."""
+    b = dict(n1=10, lo1=0.0, hi1=10.0, n2=10, lo2=0.0, hi2=1.0)
+    eps = 2.0 ** -21
+    # (a) only mu on an edge: mu = 0.4 (1 + 2^-21) is in mu-bin 4 and could be in 3; r = 2.5 is unflagged
+    res = oracle.count("rmu", _rmu_pair(2.5, 0.4 * (1 + eps)), None, b)
+    assert res["hist"][24] == 1 and res["hist"].sum() == 1
+    amb = res["amb_cell"]
+    assert amb[24] == 1 and amb[23] == 1 and amb.sum() == 2
+    assert res["amb_e2"][4] == 1 and res["amb_e1"].sum() == 0
+    # (b) r and mu both on an edge: r = 3 (1 - 2^-21) in r-bin 2 (could be 3), mu as above: four cells
+    res = oracle.count("rmu", _rmu_pair(3.0 * (1 - eps), 0.4 * (1 + eps)), None, b)
+    assert res["hist"][24] == 1
+    amb = res["amb_cell"]
+    assert sorted(np.nonzero(amb)[0].tolist()) == [23, 24, 33, 34] and amb.sum() == 4
+    assert res["amb_e1"][3] == 1 and res["amb_e2"][4] == 1
+    # (c) the outermost r edge: r = 10 (1 - 2^-21) is counted in r-bin 9 and could be out of range (virtual cell 100)
+    res = oracle.count("rmu", _rmu_pair(10.0 * (1 - eps), 0.55), None, b)
+    assert res["hist"][95] == 1
+    amb = res["amb_cell"]
+    assert amb[95] == 1 and amb[100] == 1 and amb.sum() == 2
+    # ... and from the other side: not counted, could be in cell 95
+    res = oracle.count("rmu", _rmu_pair(10.0 * (1 + eps), 0.55), None, b)
+    assert res["hist"].sum() == 0
+    amb = res["amb_cell"]
+    assert amb[95] == 1 and amb[100] == 1 and amb.sum() == 2
+    # (d) the parity rule accepts each allowed placement and nothing else
+    res = oracle.count("rmu", _rmu_pair(3.0 * (1 - eps), 0.4 * (1 + eps)), None, b)
+    for cell in (23, 24, 33, 34):
+        g = np.zeros(100, dtype=np.int64); g[cell] = 1
+        assert oracle.parity_ok(g, res)[0]
+    g = np.zeros(100, dtype=np.int64); g[25] = 1
+    assert not oracle.parity_ok(g, res)[0]
+
+
+def test_amb_cell_aperture_times_dz(oracle):
+    """RADIAL: the aperture is an edge in theta; a pair within 2^-20 of it AND of a dz edge could be in either dz cell or
+    not counted at all (virtual cell)."""
+    ap = math.radians(1.0 / 60)
+    b = dict(n1=2, lo1=0.0, hi1=2.0, n2=2, lo2=0.0, hi2=1.0, aperture=ap)
+    dz = 0.5 * (1 - 2.0 ** -21)                     # dz-bin 0, could be 1
+    def pair(sep_rad):
+        return oracle.count("radial", (np.array([10.0, 10.0]), np.array([0.0, math.degrees(sep_rad)]),
+                                       np.array([0.3, 0.3 + dz])), None, b)
+    out = pair(ap * (1 + 2.0 ** -22))               # just outside the aperture: not counted
+    assert out["hist"].sum() == 0
+    assert out["amb_cell"].tolist() == [1, 1, 0, 0, 1]
+    assert out["amb_e2"][1] == 1 and out["amb_e2"][3] == 1 and out["amb_e1"].sum() == 0
+    inn = pair(ap * (1 - 2.0 ** -22))               # just inside: counted in (zbar-bin 0, dz-bin 0)
+    assert inn["hist"].tolist() == [1, 0, 0, 0]
+    assert inn["amb_cell"].tolist() == [1, 1, 0, 0, 1]
