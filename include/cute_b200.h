@@ -74,9 +74,10 @@ typedef struct cute_catalog {
     int dtype;          /* CUTE_F32 | CUTE_F64     */
     const void *c0, *c1, *c2;
     const uint32_t *weight; /* optional integer weights, 1 <= w <= 65535 (objects per pixel of a pixel map,        */
-                            /* PAPER.md:233); NULL = unweighted.  CUTE_COORD_RADEC / CUTE_ANGULAR only.  A pair    */
-                            /* counts w_i w_j; in an auto-correlation the w_i objects of one pixel count as        */
-                            /* w_i (w_i - 1)/2 pairs at zero separation (exactly as w_i repeated objects would).   */
+                            /* PAPER.md:233; or any integer weight per object); NULL = unweighted.  RA/Dec and xyz */
+                            /* catalogues (ANGULAR, MONOPOLE, RMU, PISIGMA; not RADIAL).  A pair counts w_i w_j;   */
+                            /* in an auto-correlation the w_i objects of one point count as w_i (w_i - 1)/2 pairs  */
+                            /* at zero separation (exactly as w_i repeated objects would).                         */
 } cute_catalog;
 
 /* How to build the cell list.

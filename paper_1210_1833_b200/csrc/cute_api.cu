@@ -105,7 +105,7 @@ int check_catalog(const cute_catalog *c)
         if (!c->c0 || !c->c1) return CUTE_ERR_INVALID_ARG;
         if (c->coord != CUTE_COORD_RADEC && !c->c2) return CUTE_ERR_INVALID_ARG;
     }
-    if (c->weight && c->coord != CUTE_COORD_RADEC) return CUTE_ERR_UNSUPPORTED;   // weights: pixel maps of angular catalogues
+    if (c->weight && c->coord == CUTE_COORD_RADECZ) return CUTE_ERR_UNSUPPORTED;  // (the radial kind is unweighted)
     return CUTE_OK;
 }
 
@@ -142,7 +142,7 @@ void wants(const cute_catalog *c, const cute_grid_spec *s, int *want_lo, int *wa
 {
     int mask = s->kind_mask;
     if (c->coord == CUTE_COORD_XYZ) {
-        *want_lo = (mask == 0) || (mask & ((1 << CUTE_RMU) | (1 << CUTE_PISIGMA)));
+        *want_lo = (mask == 0) || (mask & ((1 << CUTE_RMU) | (1 << CUTE_PISIGMA))) || c->weight != nullptr;   // weights travel in lo.x
         *want_f64 = c->dtype == CUTE_F64;
     } else {
         *want_lo = 0;    // the angular fast path reads the float32 unit vectors only; tiny angles go to float64
@@ -795,12 +795,15 @@ static int count_impl(int kind, const cute_grid *g1, const cute_grid *g2, const 
         }
     }
     if (g1->weighted != g2->weighted) return CUTE_ERR_INVALID_ARG;
-    if (g1->weighted && kind != CUTE_ANGULAR) return CUTE_ERR_UNSUPPORTED;
+    if (g1->weighted && kind == CUTE_RADIAL) return CUTE_ERR_UNSUPPORTED;
+    if (g1->weighted && xyz && (!g1->has_lo || !g2->has_lo)) return CUTE_ERR_INVALID_ARG;
     PairParams p;
     memset(&p, 0, sizeof(p));
     p.g1 = g1->view; p.g2 = g2->view;
     p.weighted = g1->weighted;
-    p.self_bin = (p.weighted && is_auto && bins->lo1 == 0.0 && !bins->log1) ? 0 : -1;
+    p.weight_in_lo = (g1->weighted && xyz) ? 1 : 0;
+    // the w objects of one weighted point are w (w - 1) / 2 pairs at zero separation: cell (0 [, 0]) when the bins start at 0
+    p.self_bin = (p.weighted && is_auto && bins->lo1 == 0.0 && !bins->log1 && (bins->n2 == 0 || bins->lo2 == 0.0)) ? 0 : -1;
     p.epoch_j = kEpochJ;
     if (p.weighted) {
         // a uint32 counter receives at most 128 increments of w1max*w2max per j-point; the epoch is checked once

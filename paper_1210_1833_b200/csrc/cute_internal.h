@@ -80,7 +80,8 @@ struct PairParams {
     int logbins;                 // variable 1: 0 linear, 1 log
     int angpoly;                 // ANGULAR linear bins: theta = sqrt(q) * poly(q)
     int always_refine;           // 1: every pair passing the coarse test is recomputed in float64
-    int weighted;                // ANGULAR: pairs count w_i * w_j (uint32 bit patterns in hi.w)
+    int weighted;                // pairs count w_i * w_j (uint32 bit patterns in hi.w, or in lo.x when weight_in_lo)
+    int weight_in_lo;            // xyz catalogues: hi.w holds |x|^2, the weight travels in lo.x
     int self_bin;                // weighted auto-correlation: bin of zero separation (or -1)
     uint32_t epoch_j;            // flush a warp's uint32 histogram after this many j-points
     int n1, n2, n2eff, nhist;    // nhist = n1 * n2eff

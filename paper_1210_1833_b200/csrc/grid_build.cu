@@ -279,9 +279,11 @@ __device__ __forceinline__ void emit_point(const BuildPlan &b, uint32_t slot, do
     }
     float h[4], l[4];
     for (int d = 0; d < 4; d++) { h[d] = (float)v[d]; l[d] = (float)(v[d] - (double)h[d]); }
-    if (b.weight) {   // integer weight: bit pattern in hi.w (the pair kernel multiplies integers), exact double in p64
+    if (b.weight) {   // integer weight: a bit pattern (the pair kernel multiplies integers) in hi.w, or, for xyz
+                      // catalogues whose hi.w is |x|^2, in lo.x; RA/Dec: also as an exact double in p64
         const uint32_t w = b.weight[i];
-        h[3] = __uint_as_float(w); l[3] = 0.f; v[3] = (double)w;
+        if (b.coord == CUTE_COORD_XYZ) l[0] = __uint_as_float(w);
+        else { h[3] = __uint_as_float(w); l[3] = 0.f; v[3] = (double)w; }
         if (w == 0u || w > 65535u) atomicExch(&b.status[0], 1u);
         atomicMax(&b.status[2], w);
     }

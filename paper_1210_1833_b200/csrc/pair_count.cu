@@ -24,7 +24,7 @@ int plan_pair_kernel(PairParams &p, int want_warps, int want_cols)
     // Warps hide the latency of the dependent MUFU/FFMA chains and ncu shows throughput growing with the warp
     // count up to 16.  Default = 8 private histogram columns per warp, as many warps as fit.  A histogram too
     // large for 16 warps with private copies (the 2-D kinds) becomes ONE copy per CTA shared by all its warps.
-    const bool needlo = (p.kind == CUTE_RMU || p.kind == CUTE_PISIGMA);
+    const bool needlo = (p.kind == CUTE_RMU || p.kind == CUTE_PISIGMA || (p.weighted && p.kind != CUTE_ANGULAR));
     p.hist_shared = 0;
     const int clist[] = {3, 0, 5};
     for (int ci = 0; ci < 3; ci++) {

@@ -297,10 +297,13 @@ __device__ __forceinline__ void flush_hist(const PairParams &p, const WarpSmem &
     __syncwarp();
 }
 
-// weight of a pair: w_i * w_j for weighted catalogues (pixel maps; bit patterns in hi.w), else 1
+// weight of a pair: w_i * w_j for weighted catalogues (pixel maps), else 1.  The integer weight travels as
+// a bit pattern in hi.w (RA/Dec catalogues) or in lo.x (xyz catalogues, whose hi.w holds |x|^2)
 __device__ __forceinline__ uint32_t pair_weight(const PairParams &p, uint32_t i, uint32_t j)
 {
-    return p.weighted ? __float_as_uint(p.g1.hi[i].w) * __float_as_uint(p.g2.hi[j].w) : 1u;
+    if (!p.weighted) return 1u;
+    if (p.weight_in_lo) return __float_as_uint(p.g1.lo[i].x) * __float_as_uint(p.g2.lo[j].x);
+    return __float_as_uint(p.g1.hi[i].w) * __float_as_uint(p.g2.hi[j].w);
 }
 
 // deferred float64 recomputation of the queued pairs, one per lane
@@ -520,6 +523,7 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
     constexpr bool ALWAYS = (FLAGS & PK_ALWAYS) != 0, WEIGHTED = (FLAGS & PK_WEIGHTED) != 0;
     constexpr bool TWO_D = kind_is_2d(KIND);
     constexpr bool NEEDLW = (KIND == CUTE_RMU || KIND == CUTE_PISIGMA);
+    constexpr bool XYZW = WEIGHTED && KIND != CUTE_ANGULAR;   // weights of xyz catalogues: lo.x
     const uint32_t cs = FIXCS ? (uint32_t)fixed_colshift(KIND) : (uint32_t)p.colshift;
     const uint32_t sh = cs + 2u;
     const uint32_t hoff = (uint32_t)lane & ((1u << cs) - 1u);
@@ -534,11 +538,13 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
         float4 pj[2], pl[2];
         f32x2 q2[2][2];
         float q[2][R];
+        uint32_t wj[2];
 #pragma unroll
         for (int u = 0; u < 2; u++) {
             pj[u] = th[jj + u];
             pl[u] = make_float4(0.f, 0.f, 0.f, 0.f);
             if (NEEDLW) pl[u].w = tl[jj + u].w;
+            wj[u] = WEIGHTED ? __float_as_uint(XYZW ? tl[jj + u].x : pj[u].w) : 1u;
         }
 #pragma unroll
         for (int u = 0; u < 2; u++) {
@@ -588,7 +594,7 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
                             cell = cell * c.n2p + __float_as_uint(b);
                         }
                         addr[u][r] = hb + (cell << sh);
-                        if (WEIGHTED) red_shared_add(addr[u][r], __float_as_uint(ip.w[r]) * __float_as_uint(pj[u].w));
+                        if (WEIGHTED) red_shared_add(addr[u][r], __float_as_uint(ip.w[r]) * wj[u]);
                         else red_shared(addr[u][r]);
                     }
                 }
@@ -697,7 +703,8 @@ template <int KIND, bool MINIMG, bool LOGB, int FLAGS>
 __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_constant__ PairParams p)
 {
     const Consts cst = load_consts<KIND>(p);
-    constexpr bool NEEDLO = (KIND == CUTE_RMU || KIND == CUTE_PISIGMA);   // only the low part of |x|^2 (lo.w) is read
+    // lo.w = low part of |x|^2 (r-mu, pi-sigma); lo.x = integer weight of an xyz catalogue
+    constexpr bool NEEDLO = (KIND == CUTE_RMU || KIND == CUTE_PISIGMA || ((FLAGS & PK_WEIGHTED) && KIND != CUTE_ANGULAR));
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     WarpSmem s = carve<NEEDLO>(smem_raw + (size_t)warp * p.smem_per_warp);
@@ -743,11 +750,13 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
             const uint32_t k = lane + 32 * r;
             float4 h = make_float4(kSentinel, kSentinel, kSentinel, 0.f);
             lw[r] = 0.f;
+            float wbits = 0.f;
             if (k < ch.i_count) {
                 h = g1.hi[ch.i_begin + k];
-                if (NEEDLO) lw[r] = g1.lo[ch.i_begin + k].w;
+                if (NEEDLO) { const float4 l = g1.lo[ch.i_begin + k]; lw[r] = l.w; wbits = l.x; }
             }
-            bx[r] = h.x; by[r] = h.y; bz[r] = h.z; bw[r] = h.w; ip.w[r] = h.w;
+            bx[r] = h.x; by[r] = h.y; bz[r] = h.z; bw[r] = h.w;
+            ip.w[r] = ((FLAGS & PK_WEIGHTED) && KIND != CUTE_ANGULAR) ? wbits : h.w;
         }
 #pragma unroll
         for (int h = 0; h < 2; h++) {
@@ -919,8 +928,8 @@ static cudaError_t launch_k(const PairParams &p, int blocks, size_t smem, cudaSt
 template <int KIND, bool MINIMG, bool LOGB>
 static cudaError_t launch_t(const PairParams &p, int blocks, size_t smem, cudaStream_t s)
 {
-    if (p.weighted) {   // pixel maps: ANGULAR only
-        if constexpr (KIND == CUTE_ANGULAR) {
+    if (p.weighted) {   // integer weights (pixel maps PAPER.md:233, weighted objects): runtime column count
+        if constexpr (KIND != CUTE_RADIAL) {
             if (p.always_refine) return launch_k<KIND, MINIMG, LOGB, PK_ALWAYS | PK_WEIGHTED>(p, blocks, smem, s);
             return launch_k<KIND, MINIMG, LOGB, PK_WEIGHTED>(p, blocks, smem, s);
         }

@@ -553,3 +553,60 @@ def test_refine_path_against_enumeration_and_eq9(rt):
             assert hh.sum() == 1 and hh[cell] == 1, (r9, mu9, opts)
         checked += 1
     assert checked > 40
+
+
+@pytest.mark.parametrize("grid", ["none", "box3d"])
+def test_weighted_3d_kinds(rt, oracle, grid):
+    """integer weights per object for the 3-D kinds (PAPER.md:233 generalised): a pair counts w_i w_j,
+    the w objects of one point w(w-1)/2 pairs at zero separation -- weighted C5-like DD/DR (periodic box, float32), weighted
+    (r,mu) and (pi,sigma) on comoving float64 coordinates, brute force and cell lists, heavy weights, force_refine"""
+    api, runner, synth = rt
+    rng = np.random.default_rng(43)
+    w5 = synth.workload(5, 0.0008)
+    nd, nr = len(w5.data[0]), len(w5.rand[0])
+    wd, wr = rng.integers(1, 9, nd).astype(np.uint32), rng.integers(1, 4, nr).astype(np.uint32)
+    g5 = dict(mode="none") if grid == "none" else w5.grid
+    job = runner.Job("monopole", w5.data, w5.rand, w5.bins, g5, None, w_data=wd, w_rand=wr).build()
+    for which, a, b, wa, wb in (("DD", w5.data, None, wd, None), ("DR", w5.data, w5.rand, wd, wr)):
+        h, st = job.count(which)
+        orc = oracle.count("monopole", a, b, w5.bins, mode="celled", w1=wa, w2=wb)
+        ok, msg = oracle.parity_ok(h, orc)
+        assert ok, f"monopole {which}: {msg}"
+    job.opts = api.count_opts(force_refine=1)
+    h2, _ = job.count("DR")
+    job.opts = None
+    assert np.array_equal(h2, job.count("DR")[0])
+    # the weighted count of unit weights is the unweighted count
+    one = runner.Job("monopole", w5.data, None, w5.bins, g5, None, w_data=np.ones(nd, dtype=np.uint32)).build()
+    plain = runner.Job("monopole", w5.data, None, w5.bins, g5).build()
+    assert np.array_equal(one.count("DD")[0], plain.count("DD")[0])
+    # heavy weights: short uint32 epochs
+    wh = rng.integers(1, 300, nd).astype(np.uint32)
+    job = runner.Job("monopole", w5.data, None, w5.bins, g5, None, w_data=wh).build()
+    h, st = job.count("DD")
+    ok, msg = oracle.parity_ok(h, oracle.count("monopole", w5.data, None, w5.bins, mode="celled", w1=wh))
+    assert ok, msg
+    h_heavy = h
+    # (r, mu) and (pi, sigma) on C3-like comoving coordinates
+    w3 = synth.workload(3, 0.012)
+    n3d, n3r = len(w3.data[0]), len(w3.rand[0])
+    v1, v2 = rng.integers(1, 6, n3d).astype(np.uint32), rng.integers(1, 3, n3r).astype(np.uint32)
+    g3 = dict(mode="none") if grid == "none" else w3.grid
+    for kind, bins in (("rmu", w3.bins), ("pisigma", dict(w3.bins, n1=24, hi1=120.0, n2=24, lo2=0.0, hi2=120.0))):
+        g = dict(g3, rmax=math.hypot(bins["hi1"], bins["hi2"])) if (kind == "pisigma" and grid != "none") else g3
+        job = runner.Job(kind, w3.data, w3.rand, bins, g, None, w_data=v1, w_rand=v2).build()
+        for which, a, b, wa, wb in (("DD", w3.data, None, v1, None), ("DR", w3.data, w3.rand, v1, v2)):
+            h, st = job.count(which)
+            orc = oracle.count(kind, a, b, bins, mode="celled", w1=wa, w2=wb)
+            ok, msg = oracle.parity_ok(h, orc)
+            assert ok, f"{kind} {which}: {msg}"
+    # the end-to-end host entry point carries the weights too
+    hh, _ = api.cute_count_pairs_host(api.MONOPOLE, w5.data, None, api.COORD_XYZ, job_spec_for(api, w5, g5), w5.bins, w1=wh)
+    assert np.array_equal(hh, h_heavy)
+
+
+def job_spec_for(api, w, grid):
+    if grid.get("mode", "none") == "none":
+        return api.grid_spec("none")
+    L = w.bins["box_L"]
+    return api.grid_spec("box3d", periodic=True, size=(L, L, L), rmax=grid["rmax"])
