@@ -46,8 +46,8 @@
  * flags as lying within relative 2^-20 of a bin edge") is then
  *      |gpu[c] - oracle[c]| <= amb_cell[c]  for every c,   |sum gpu - sum oracle| <= amb_cell[ncell].
  *
- * Pins: tests/test_oracle_pins.py (V1..V10 of SURVEY.md 8(c)); no function here is "parity
- * unpinned".
+ * Pins: tests/test_oracle_pins.py (V1..V11 of SURVEY.md 8(c), the 2-D composition of amb_cell, the density-grid
+ * functions); no function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -672,6 +672,108 @@ int orc_multipoles(const double *xi, int n_r, int n_mu, double *out)
         out[2 * n_r + k] = 9.0 * a4 / (double)n_mu;
     }
     return ORC_OK;
+}
+
+/* ------------------------------------------------------------------ density-grid monopole (CUTE_box)
+ * "the particle content of the catalog is first interpolated to a grid and the overdensity field delta is estimated at
+ *  every grid point using a TSC algorithm.  Then pairs of grid points are correlated, and a weight delta_i delta_j is
+ *  given to each pair.  The correlation function is estimated as xi(r) = < delta(x) delta(x + r) >  (Eq. 17), where the
+ *  average is taken over all pairs of grid points separated by a distance r."
+ * Readings (the paper gives no formulas here):
+ *   D1  the grid points are the CENTRES of the ng^3 cubic cells of side h = L/ng: x_g = (g + 1/2) h, periodic;
+ *   D2  TSC = triangular-shaped cloud, the standard second-order B-spline per axis, s = |x - x_g| / h:
+ *           W(s) = 3/4 - s^2  (s <= 1/2),   (3/2 - s)^2 / 2  (1/2 < s <= 3/2),   0 otherwise;
+ *       a particle feeds the 3 x 3 x 3 grid points around its cell with the product of the three axis weights;
+ *   D3  delta_g = rho_g / rho_bar - 1 with rho_bar = N / ng^3 (the weights of one particle sum to 1);
+ *   D4  "pairs of grid points separated by a distance r": every ORDERED pair (g, g + v) with v != 0 an integer offset
+ *       taken with the minimum image, r = h |v|, binned half-open like every other separation (S1);
+ *       xi_k = sum over those pairs of delta_g delta_{g+v} / number of those pairs; a bin no offset falls in has
+ *       xi = 0 and is reported empty;  the offsets and their bins are found once, not per grid point.
+ * Plain float64 loops. */
+static double tsc_w(double s)
+{
+    s = fabs(s);
+    if (s <= 0.5) return 0.75 - s * s;
+    if (s <= 1.5) return 0.5 * (1.5 - s) * (1.5 - s);
+    return 0.0;
+}
+
+/* rho[ng^3] (z-major: index = (gz * ng + gy) * ng + gx) = TSC-assigned particle number per grid point */
+int orc_tsc_assign(int64_t n, const double *x, const double *y, const double *z, double L, int ng, double *rho)
+{
+    if (n < 0 || ng < 3 || !(L > 0.0)) return ORC_EINVAL;
+    const double h = L / (double)ng;
+    for (int64_t c = 0; c < (int64_t)ng * ng * ng; c++) rho[c] = 0.0;
+    for (int64_t i = 0; i < n; i++) {
+        const double p[3] = {x[i], y[i], z[i]};
+        int g0[3]; double w[3][3];
+        for (int d = 0; d < 3; d++) {
+            double u = p[d] / h;                       /* position in units of cells */
+            int c = (int)floor(u);                     /* the particle's own cell    */
+            g0[d] = c - 1;
+            for (int k = 0; k < 3; k++) w[d][k] = tsc_w(u - ((double)(c - 1 + k) + 0.5));
+        }
+        for (int a = 0; a < 3; a++)
+            for (int b = 0; b < 3; b++)
+                for (int c = 0; c < 3; c++) {
+                    int gx = ((g0[0] + c) % ng + ng) % ng, gy = ((g0[1] + b) % ng + ng) % ng, gz = ((g0[2] + a) % ng + ng) % ng;
+                    rho[((int64_t)gz * ng + gy) * ng + gx] += w[0][c] * w[1][b] * w[2][a];
+                }
+    }
+    return ORC_OK;
+}
+
+/* delta = rho / (n / ng^3) - 1 */
+int orc_overdensity(int64_t n, int ng, const double *rho, double *delta)
+{
+    if (n <= 0 || ng < 1) return ORC_EINVAL;
+    const double mean = (double)n / ((double)ng * ng * ng);
+    for (int64_t c = 0; c < (int64_t)ng * ng * ng; c++) delta[c] = rho[c] / mean - 1.0;
+    return ORC_OK;
+}
+
+/* Eq. 17 on a periodic grid: sum_dd[k] = sum of delta_g delta_{g+v} over ordered pairs with h|v| in bin k,
+ * npairs[k] = their number, xi[k] = sum_dd / npairs (0 when npairs = 0; the return value counts such bins) */
+int orc_grid_correlation(const double *delta, int ng, double L, const orc_bins *b, double *xi, double *sum_dd, uint64_t *npairs)
+{
+    if (ng < 3 || !(L > 0.0) || b->n1 < 1 || !(b->lo1 < b->hi1) || b->hi1 > 0.5 * L) return ORC_EINVAL;
+    double *e = (double *)malloc(((size_t)b->n1 + 1) * 8);
+    if (!e) return ORC_ENOMEM;
+    int rc = orc_edges(b, 0, e);
+    if (rc) { free(e); return rc; }
+    axis_t ax = {b->n1, b->log1, 0, b->lo1, b->hi1, e};
+    const double h = L / (double)ng;
+    int m = (int)floor(b->hi1 / h);
+    if (m > (ng - 1) / 2) m = (ng - 1) / 2;
+    for (int k = 0; k < b->n1; k++) { sum_dd[k] = 0.0; npairs[k] = 0; }
+    const int64_t ng3 = (int64_t)ng * ng * ng;
+    for (int dz = -m; dz <= m; dz++)
+        for (int dy = -m; dy <= m; dy++)
+            for (int dx = -m; dx <= m; dx++) {
+                if (dx == 0 && dy == 0 && dz == 0) continue;
+                const double r = h * sqrt((double)(dx * dx + dy * dy + dz * dz));
+                const int k = find_bin(&ax, r);
+                if (k < 0) continue;
+                double s = 0.0;
+#pragma omp parallel for reduction(+ : s) schedule(static)
+                for (int gz = 0; gz < ng; gz++) {
+                    const int hz = (gz + dz + ng) % ng;
+                    for (int gy = 0; gy < ng; gy++) {
+                        const int hy = (gy + dy + ng) % ng;
+                        const double *r0 = delta + ((int64_t)gz * ng + gy) * ng, *r1 = delta + ((int64_t)hz * ng + hy) * ng;
+                        for (int gx = 0; gx < ng; gx++) s += r0[gx] * r1[(gx + dx + ng) % ng];
+                    }
+                }
+                sum_dd[k] += s;
+                npairs[k] += (uint64_t)ng3;
+            }
+    int empty = 0;
+    for (int k = 0; k < b->n1; k++) {
+        if (npairs[k] == 0) { xi[k] = 0.0; empty++; }
+        else xi[k] = sum_dd[k] / (double)npairs[k];
+    }
+    free(e);
+    return empty;
 }
 
 int orc_max_threads(void) { return omp_get_max_threads(); }

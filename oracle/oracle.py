@@ -56,6 +56,9 @@ def _load():
         _lib.orc_natural.argtypes = [up, up, C.c_uint64, C.c_uint64, C.c_int, dp]
         _lib.orc_periodic_rr.argtypes = [C.c_uint64, C.c_double, C.POINTER(_Bins), dp]
         _lib.orc_multipoles.argtypes = [dp, C.c_int, C.c_int, dp]
+        _lib.orc_tsc_assign.argtypes = [C.c_int64, dp, dp, dp, C.c_double, C.c_int, dp]
+        _lib.orc_overdensity.argtypes = [C.c_int64, C.c_int, dp, dp]
+        _lib.orc_grid_correlation.argtypes = [dp, C.c_int, C.c_double, C.POINTER(_Bins), dp, dp, up]
     return _lib
 
 
@@ -176,6 +179,47 @@ def multipoles(xi_rmu, n_r: int, n_mu: int) -> np.ndarray:
     rc = _load().orc_multipoles(_dp(xi), int(n_r), int(n_mu), _dp(out))
     if rc:
         raise ValueError(f"orc_multipoles failed ({rc})")
+    return out
+
+
+def tsc_assign(cat, L: float, ng: int) -> np.ndarray:
+    """TSC particle number per grid point, shape (ng, ng, ng) indexed [gz, gy, gx]."""
+    c = [np.ascontiguousarray(np.asarray(a, dtype=np.float64)) for a in cat[:3]]
+    rho = np.zeros(ng * ng * ng)
+    rc = _load().orc_tsc_assign(c[0].size, _dp(c[0]), _dp(c[1]), _dp(c[2]), float(L), int(ng), _dp(rho))
+    if rc:
+        raise ValueError(f"orc_tsc_assign failed ({rc})")
+    return rho.reshape(ng, ng, ng)
+
+
+def overdensity(rho: np.ndarray, n: int) -> np.ndarray:
+    ng = rho.shape[0]
+    r = np.ascontiguousarray(rho, dtype=np.float64).ravel()
+    d = np.zeros_like(r)
+    rc = _load().orc_overdensity(int(n), int(ng), _dp(r), _dp(d))
+    if rc:
+        raise ValueError(f"orc_overdensity failed ({rc})")
+    return d.reshape(ng, ng, ng)
+
+
+def grid_correlation(delta: np.ndarray, L: float, bins: dict):
+    """Eq. 17 on a periodic grid: dict(xi, sum_dd, npairs, empty)."""
+    ng = delta.shape[0]
+    d = np.ascontiguousarray(delta, dtype=np.float64).ravel()
+    b = _bins(bins)
+    xi, sdd, npr = np.zeros(b.n1), np.zeros(b.n1), np.zeros(b.n1, dtype=np.uint64)
+    rc = _load().orc_grid_correlation(_dp(d), int(ng), float(L), C.byref(b), _dp(xi), _dp(sdd), _up(npr))
+    if rc < 0:
+        raise ValueError(f"orc_grid_correlation failed ({rc})")
+    return dict(xi=xi, sum_dd=sdd, npairs=npr, empty=int(rc))
+
+
+def density_grid_xi(cat, L: float, ng: int, bins: dict):
+    """the whole density-grid monopole: TSC -> delta -> Eq. 17"""
+    rho = tsc_assign(cat, L, ng)
+    delta = overdensity(rho, len(cat[0]))
+    out = grid_correlation(delta, L, bins)
+    out["delta"] = delta
     return out
 
 

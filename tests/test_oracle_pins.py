@@ -527,3 +527,76 @@ def test_amb_cell_aperture_times_dz(oracle):
     inn = pair(ap * (1 - 2.0 ** -22))               # just inside: counted in (zbar-bin 0, dz-bin 0)
     assert inn["hist"].tolist() == [1, 0, 0, 0]
     assert inn["amb_cell"].tolist() == [1, 1, 0, 0, 1]
+
+
+# ---------------------------------------------------------------- N4 density-grid monopole (Eq. 17)
+def test_tsc_weights_closed_forms(oracle):
+    """TSC (reading D2): a particle at a cell centre feeds (1/8, 3/4, 1/8) per axis; one on a cell face (1/2, 1/2, 0);
+    the weights of any particle sum to 1 (mass conservation); a particle per cell centre gives rho = 1, delta = 0."""
+    L, ng = 8.0, 8
+    rho = oracle.tsc_assign((np.array([3.5]), np.array([3.5]), np.array([3.5])), L, ng)      # centre of cell (3,3,3)
+    w = np.array([0.125, 0.75, 0.125])
+    want = np.zeros((ng, ng, ng))
+    want[2:5, 2:5, 2:5] = w[:, None, None] * w[None, :, None] * w[None, None, :]
+    assert np.allclose(rho, want, atol=1e-15)
+    rho = oracle.tsc_assign((np.array([4.0]), np.array([3.5]), np.array([3.5])), L, ng)      # on the face between x-cells 3 and 4
+    assert np.allclose(rho[3, 3, 2:6], 0.75 * 0.75 * np.array([0.0, 0.5, 0.5, 0.0]), atol=1e-15)
+    # periodic wrap: a particle in cell 0 reaches cell ng - 1
+    rho = oracle.tsc_assign((np.array([0.5]), np.array([0.5]), np.array([0.5])), L, ng)
+    assert abs(rho[0, 0, ng - 1] - 0.125 * 0.75 * 0.75) < 1e-15 and abs(rho.sum() - 1.0) < 1e-14
+    rng = np.random.default_rng(7)
+    x = rng.random((3, 5000)) * L
+    rho = oracle.tsc_assign(tuple(x), L, ng)
+    assert abs(rho.sum() - 5000.0) < 1e-9 and rho.min() >= 0.0
+    g = (np.arange(ng) + 0.5) * (L / ng)
+    lat = np.array(list(itertools.product(g, g, g))).T
+    rho = oracle.tsc_assign(tuple(lat), L, ng)
+    assert np.allclose(rho, 1.0, atol=1e-14)
+    assert np.allclose(oracle.overdensity(rho, ng ** 3), 0.0, atol=1e-14)
+    assert np.allclose(oracle.overdensity(2.0 * np.ones((4, 4, 4)), 128), 0.0)            # rho_bar = N / ng^3
+
+
+def test_grid_correlation_of_a_plane_wave(oracle):
+    """Eq. 17 on delta = A cos(k.x): (1/N) sum_g delta_g delta_{g+v} = A^2/2 cos(k.v) for a grid wave vector, so
+    xi_k = A^2/2 * mean over the offsets of the shell of cos(k.v) -- the offsets are enumerated here, not by the oracle."""
+    ng, L, A = 16, 32.0, 0.3
+    h = L / ng
+    kv = np.array([2, 1, 3])                                   # wave vector in units of 2 pi / L
+    gz, gy, gx = np.meshgrid(np.arange(ng), np.arange(ng), np.arange(ng), indexing="ij")
+    delta = A * np.cos(2 * np.pi * (kv[0] * gx + kv[1] * gy + kv[2] * gz) / ng)
+    bins = dict(n1=6, lo1=0.0, hi1=12.0)
+    e = np.linspace(0.0, 12.0, 7)
+    want_s, want_n = np.zeros(6), np.zeros(6)
+    m = int(12.0 // h)
+    for dz, dy, dx in itertools.product(range(-m, m + 1), repeat=3):
+        if dx == dy == dz == 0:
+            continue
+        r = h * math.sqrt(dx * dx + dy * dy + dz * dz)
+        k = np.searchsorted(e, r, side="right") - 1
+        if 0 <= k < 6 and r < e[-1]:
+            want_s[k] += 0.5 * A * A * math.cos(2 * np.pi * (kv[0] * dx + kv[1] * dy + kv[2] * dz) / ng)
+            want_n[k] += 1
+    out = oracle.grid_correlation(delta, L, bins)
+    assert np.array_equal(out["npairs"], (want_n * ng ** 3).astype(np.uint64))
+    ok = want_n > 0
+    assert ok.sum() == 5 and out["empty"] == 1 and out["xi"][0] == 0.0          # no offset is shorter than h = 2
+    assert np.allclose(out["xi"][ok], want_s[ok] / want_n[ok], atol=1e-13)
+    assert np.allclose(out["sum_dd"], want_s * ng ** 3, atol=1e-9)
+    # a constant field correlates with itself everywhere; bins no offset reaches are reported empty
+    out = oracle.grid_correlation(np.full((ng, ng, ng), 0.5), L, dict(n1=40, lo1=0.0, hi1=4.0))
+    assert out["empty"] > 0 and np.all(out["xi"][out["npairs"] > 0] == 0.25) and np.all(out["xi"][out["npairs"] == 0] == 0.0)
+
+
+def test_density_grid_agrees_with_pair_counts_above_the_grid_scale(oracle):
+    """"it will only yield reliable results down to the scale of the grid": on a clustered periodic box
+    (Thomas process, sigma = 3) the density-grid xi equals the pair-count xi of Eq. 13 at r >> h and is smoothed (lower)
+    at r ~ h."""
+    L, n, ng = 200.0, 30000, 64                                  # h = 3.125
+    x = synth.thomas_box(n, L, 3.0, 10.0, 99)
+    bins = dict(n1=10, lo1=0.0, hi1=50.0, box_L=L)
+    dd = oracle.count("monopole", tuple(x), None, bins, mode="celled")["hist"].astype(float)
+    xi_pairs = dd / oracle.periodic_rr(n, L, bins) - 1.0
+    xi_grid = oracle.density_grid_xi(tuple(x), L, ng, dict(n1=10, lo1=0.0, hi1=50.0))["xi"]
+    assert np.all(np.abs(xi_grid[3:] - xi_pairs[3:]) < 2e-3)                       # r > 15 = 5 h: the same function
+    assert xi_pairs[0] > 1.0 and 0.9 * xi_pairs[0] < xi_grid[0] < xi_pairs[0]      # r < 5: the signal, a little smoothed
+    assert 0.85 * xi_pairs[1] < xi_grid[1] < xi_pairs[1]
