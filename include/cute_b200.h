@@ -240,6 +240,21 @@ int cute_count_pairs_host(int kind, const cute_catalog *cat1, const cute_catalog
                           const cute_bin_spec *bins, const cute_count_opts *opts, uint64_t *h_hist, void *d_workspace,
                           size_t bytes, void *stream);
 
+/* Density-grid monopole of a periodic box (the second algorithm of CUTE_box): "the particle content of
+ * the catalog is first interpolated to a grid and the overdensity field delta is estimated at every grid point using a TSC
+ * algorithm.  Then pairs of grid points are correlated, and a weight delta_i delta_j is given to each pair", xi(r) =
+ * <delta(x) delta(x + r)> (Eq. 17); the relative offsets and their bins are found once.  Readings (N4): grid
+ * points = centres (g + 1/2) L/ng of the ng^3 cells; TSC = second-order B-spline per axis; delta = rho ng^3 / N - 1; every
+ * ordered pair of distinct grid points with the minimum image, r = (L/ng) |v|, half-open bins (variable 1 of `bins`,
+ * linear or log, hi1 <= L/2; the other fields are ignored).  cat: DEVICE, CUTE_COORD_XYZ in [0, L) (taken modulo L),
+ * float32 or float64, unweighted.  Outputs (HOST, n1 entries; h_sum_dd and h_npairs may be NULL): xi, the sums of
+ * delta delta and the numbers of grid-point pairs per bin; d_delta (DEVICE, ng^3 doubles, index (gz ng + gy) ng + gx, may
+ * be NULL) receives the overdensity field.  Float64 throughout: equal to a serial float64 evaluation up to the order of
+ * the additions.  A bin no offset falls in gets xi = 0 and CUTE_WARN_EMPTY_BIN.  Synchronises the stream. */
+int cute_density_grid_workspace_bytes(int ng, const cute_bin_spec *bins, double L, size_t *bytes);
+int cute_density_grid_xi(const cute_catalog *cat, double L, int ng, const cute_bin_spec *bins, double *h_xi, double *h_sum_dd,
+                         uint64_t *h_npairs, double *d_delta, void *d_workspace, size_t bytes, void *stream);
+
 /* Microbenchmarks of the units the pair kernel's roofline is made of (FP32 / packed FP32x2 /
  * integer issue rates, MUFU, shared-memory atomics versus same-address multiplicity, broadcast LDS, and mixes that
  * show which instructions share an issue port).  One persistent 512-thread CTA per SM, timed with clock64() inside the

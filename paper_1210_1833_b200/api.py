@@ -59,7 +59,8 @@ SYMBOLS = ["cute_version", "cute_strerror", "cute_launch_count", "cute_catalog_b
            "cute_grid_get_info", "cute_count_scratch_bytes", "cute_count_pairs", "cute_count_items",
            "cute_count_status", "cute_host_workspace_bytes", "cute_count_pairs_host", "cute_bin_edges",
            "cute_landy_szalay", "cute_natural_estimator", "cute_multipoles", "cute_periodic_rr", "cute_periodic_xi",
-           "cute_peak_count", "cute_peak_name", "cute_measure_peaks", "cute_shard_items", "cute_auto_grid_spec"]
+           "cute_peak_count", "cute_peak_name", "cute_measure_peaks", "cute_shard_items", "cute_auto_grid_spec",
+           "cute_density_grid_workspace_bytes", "cute_density_grid_xi"]
 
 
 def _load() -> C.CDLL:
@@ -93,6 +94,9 @@ def _load() -> C.CDLL:
     lib.cute_shard_items.argtypes = [C.c_int64, C.c_int64, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     lib.cute_auto_grid_spec.argtypes = [C.c_int, C.c_int, C.POINTER(C.POINTER(cute_catalog)), C.c_int, C.c_double, C.c_double,
                                         C.c_double, C.POINTER(C.c_int), C.c_int, vp, vp, C.POINTER(cute_grid_spec)]
+    lib.cute_density_grid_workspace_bytes.argtypes = [C.c_int, C.POINTER(cute_bin_spec), C.c_double, C.POINTER(C.c_size_t)]
+    lib.cute_density_grid_xi.argtypes = [C.POINTER(cute_catalog), C.c_double, C.c_int, C.POINTER(cute_bin_spec), dp, dp, up, vp, vp,
+                                         C.c_size_t, vp]
     lib.cute_peak_count.restype = C.c_int
     lib.cute_peak_name.restype = C.c_char_p
     lib.cute_peak_name.argtypes = [C.c_int]
@@ -390,6 +394,28 @@ def cute_periodic_xi(dd, n: int, L: float, bins: dict):
     xi = np.zeros(b.n1)
     rc = _check(lib.cute_periodic_xi(_up(dd), int(n), float(L), C.byref(b), _dp(xi)), "cute_periodic_xi")
     return xi, rc
+
+
+def cute_density_grid_xi(cols, L: float, ng: int, bins: dict, want_delta: bool = False, workspace=None, stream=None):
+    """Density-grid monopole (Eq. 17) of device xyz columns: dict(xi, sum_dd, npairs, status[, delta])."""
+    torch = _torch()
+    cat, keep = _catalog(cols, COORD_XYZ, True)
+    b = bin_spec(bins)
+    nb = C.c_size_t(0)
+    _check(lib.cute_density_grid_workspace_bytes(int(ng), C.byref(b), float(L), C.byref(nb)), "cute_density_grid_workspace_bytes")
+    if workspace is None or workspace.numel() < nb.value + 256:
+        workspace = torch.empty(nb.value + 256, dtype=torch.uint8, device=keep[0].device)
+    off = (-workspace.data_ptr()) % 256
+    xi, sdd, npr = np.zeros(b.n1), np.zeros(b.n1), np.zeros(b.n1, dtype=np.uint64)
+    delta = torch.empty(ng * ng * ng, dtype=torch.float64, device=keep[0].device) if want_delta else None
+    rc = _check(lib.cute_density_grid_xi(C.byref(cat), float(L), int(ng), C.byref(b), _dp(xi), _dp(sdd), _up(npr),
+                                         C.c_void_p(delta.data_ptr()) if delta is not None else None,
+                                         C.c_void_p(workspace.data_ptr() + off), workspace.numel() - off, C.c_void_p(_stream_ptr(stream))),
+                "cute_density_grid_xi")
+    out = dict(xi=xi, sum_dd=sdd, npairs=npr, status=rc, workspace=workspace)
+    if delta is not None:
+        out["delta"] = delta.view(ng, ng, ng)
+    return out
 
 
 def cute_measure_peaks(stream=None) -> dict:

@@ -610,3 +610,29 @@ def job_spec_for(api, w, grid):
         return api.grid_spec("none")
     L = w.bins["box_L"]
     return api.grid_spec("box3d", periodic=True, size=(L, L, L), rmax=grid["rmax"])
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_density_grid_monopole(rt, oracle, dtype):
+    """N4 (Eq. 17): TSC overdensity field and grid-point correlation against the float64 oracle.
+    Float64 on both sides, so the tolerance is the order of the additions: 1e-12 on delta, 1e-10 (absolute, in units of
+    <delta^2>) on xi; the numbers of grid-point pairs per bin are integers and must be equal."""
+    import torch
+    api, runner, synth = rt
+    L, n, ng = 200.0, 30000, 48
+    x = synth.thomas_box(n, L, 3.0, 10.0, 99, dtype)
+    cols = [torch.from_numpy(np.ascontiguousarray(c)).cuda() for c in x]
+    for bins in (dict(n1=12, lo1=0.0, hi1=60.0), dict(n1=9, lo1=3.0, hi1=80.0, log1=1), dict(n1=40, lo1=0.0, hi1=10.0)):
+        out = api.cute_density_grid_xi(cols, L, ng, bins, want_delta=True)
+        orc = oracle.density_grid_xi(tuple(np.asarray(c, dtype=np.float64) for c in x), L, ng, bins)
+        d = out["delta"].cpu().numpy()
+        assert np.max(np.abs(d - orc["delta"])) < 1e-12 * max(1.0, np.abs(orc["delta"]).max())
+        assert np.array_equal(out["npairs"], orc["npairs"])
+        var = float((orc["delta"] ** 2).mean())
+        assert np.max(np.abs(out["xi"] - orc["xi"])) < 1e-10 * max(1.0, var)
+        assert (out["status"] == api.WARN_EMPTY_BIN) == (orc["empty"] > 0)
+    # mass conservation on the device: <delta> = 0
+    assert abs(float(out["delta"].mean())) < 1e-12
+    # validation: r_max beyond L/2, a non-xyz catalogue
+    with pytest.raises(api.CuteError):
+        api.cute_density_grid_xi(cols, L, ng, dict(n1=4, lo1=0.0, hi1=120.0))
