@@ -285,7 +285,11 @@ __device__ __forceinline__ void flush_hist(const PairParams &p, const WarpSmem &
         for (int k = 0; k < C; k++) {
             int col = (k + lane) & (C - 1);
             if (p.hist_shared) sum += atomicExch(row + col, 0u);   // other warps keep adding: read-and-clear in one step
-            else { sum += row[col]; row[col] = 0; }
+            else {
+                // the epoch bound keeps every private counter far below 2^31: one above it means increments were lost
+                if (row[col] >= 0x80000000u) atomicOr(p.status, 2u);
+                sum += row[col]; row[col] = 0;
+            }
         }
         // border cells hold the clamped out-of-range pairs: dropped
         const bool real = k1p >= 1u && k1p <= (uint32_t)p.n1 && k2p >= 1u && (p.n2 == 0 || k2p <= (uint32_t)p.n2);
@@ -532,7 +536,13 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
     constexpr uint32_t MB1 = CUTE_MAGIC_BITS - 1u;
     const uint32_t hb = smem_u32(s.hist + hoff) - ((TWO_D ? MB1 * (c.n2p + 1u) : MB1) << sh);
     const float bot = CUTE_MAGIC_F - 1.0f;
-#pragma unroll 2
+    // Measured (C5): reading the NEXT block's j-points before this block's guarded bin path and four copies of the body
+    // are worth 4 % on the short monopole body and cost as much on the longer angular / r-mu bodies (registers).
+    constexpr bool PREFETCH = KIND == 1 /* CUTE_MONOPOLE */ && !WEIGHTED;
+    constexpr int kUnroll = PREFETCH ? 4 : 2;
+    float4 nx[2];
+    if (PREFETCH) { nx[0] = th[0]; nx[1] = th[1]; }
+#pragma unroll kUnroll
     for (uint32_t jp = 0; jp < cnt2; jp++) {
         const uint32_t jj = 2u * jp;
         float4 pj[2], pl[2];
@@ -541,10 +551,14 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
         uint32_t wj[2];
 #pragma unroll
         for (int u = 0; u < 2; u++) {
-            pj[u] = th[jj + u];
+            pj[u] = PREFETCH ? nx[u] : th[jj + u];
             pl[u] = make_float4(0.f, 0.f, 0.f, 0.f);
             if (NEEDLW) pl[u].w = tl[jj + u].w;
             wj[u] = WEIGHTED ? __float_as_uint(XYZW ? tl[jj + u].x : pj[u].w) : 1u;
+        }
+        if (PREFETCH) {
+            const uint32_t jn = min(jj + 2u, (uint32_t)kTile - 2u);   // (the last block re-reads inside the tile buffer)
+            nx[0] = th[jn]; nx[1] = th[jn + 1];
         }
 #pragma unroll
         for (int u = 0; u < 2; u++) {

@@ -107,3 +107,47 @@ def test_c5_full_sampled(rt, oracle):
     w = synth.workload(5)
     nd = len(w.data[0])
     _cross_block_check(rt, oracle, w, "DR", w.data, w.rand, _blocks(nd, 500, (0, 9999, 19999)), "celled")
+
+
+def _perm_of(job, torch):
+    """sorted slot -> input index of the data grid (cute_grid_info.d_perm)"""
+    inf = job.g_data.info()
+    ws = job.g_data.workspace
+    off = inf.d_perm - ws.data_ptr()
+    return ws[off:off + inf.n * 4].view(torch.int32).cpu().numpy().astype(np.int64)
+
+
+@pytest.mark.parametrize("cfg", [2, 5])
+def test_auto_path_at_full_size(rt, oracle, cfg):
+    """The auto-correlation path (j > i mask, own-row segments) at BASELINE.json's full sizes, tied to the oracle two ways:
+    (i) the exact identity cross(A, A)[k] = 2 auto(A)[k] + N [k = 0 and lo = 0] -- the cross side is oracle-checked on
+    blocks by the tests above; (ii) the auto count of ~2e4 CONSECUTIVE cell-sorted points (a dense block of the real
+    catalogue, through the same grid spec, so the same cells, chunks and own-row logic) against the oracle."""
+    import torch
+    api, runner, synth = rt
+    w = synth.workload(cfg)
+    n = len(w.data[0])
+    grid = dict(w.grid)                                     # (keeps the permutation: no_perm is not set)
+    job = runner.Job(w.kind, w.data, w.data, w.bins, grid).build()   # the same catalogue twice: two grids
+    h_auto, st_auto = job.count("DD")
+    h_cross, st_cross = job.count("DR")
+    want = 2 * h_auto.astype(np.int64)
+    if w.bins["lo1"] == 0.0 and not w.bins.get("log1", 0):
+        want[0] += n                                        # the N pairs (i, i) at zero separation
+    assert np.array_equal(h_cross.astype(np.int64), want)
+    if w.grid.get("mode", "none") == "none":
+        assert st_auto["evaluated"] == n * (n - 1) // 2 and st_cross["evaluated"] == n * n
+    # (ii) a block of consecutive sorted points
+    perm = _perm_of(job, torch)
+    assert np.array_equal(np.sort(perm), np.arange(n))
+    for s0 in (0, n // 2 + 12345):
+        idx = perm[s0:s0 + 20000]
+        sub = tuple(np.ascontiguousarray(c[idx]) for c in w.data)
+        jb = runner.Job(w.kind, sub, None, w.bins, grid)
+        jb.spec = job.spec
+        jb.build()
+        h, st = jb.count("DD")
+        orc = oracle.count(w.kind, sub, None, w.bins, mode="celled" if cfg == 5 else "plain")
+        ok, msg = oracle.parity_ok(h, orc)
+        assert ok, f"sorted block at {s0}: {msg}"
+        assert h.sum() > 1000
