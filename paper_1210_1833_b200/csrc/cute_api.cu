@@ -669,19 +669,30 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
                 const double se = (double)A.c1 + q * ((double)A.c2 + q * ((double)A.c3 + q * (double)A.c4));
                 series_err = fmax(series_err, 0.5 * sc * fabs(log(toc * toc / se)));
             }
-            // The absolute chord error is a RELATIVE error e_abs / c of theta: pairs closer than c_min always go to
-            // float64 (kernel: q < q_small), the others carry tau ~ sc e_abs / c_min.  For a uniform density the number
-            // of always-refined pairs grows as c_min^2 and the number of near-edge pairs as 1 / c_min: the total is
-            // least at c_min^3 = sc e_abs c_hi^2.  Below lo nothing can be mis-binned INTO range as long as lo >> e_abs.
+            // The absolute chord error is a RELATIVE error e_abs / c of theta, so tau = tau_a + tau_b / c depends on the pair.
+            // The kernel's one threshold (a1.tau) is sized for chords >= c_mid, which is nearly every pair (the number of
+            // pairs grows as theta^2); a block holding a closer pair is tested with tau_mid (sized for the closest chord
+            // that is still decided in float32, c_min) and its pairs are then decided one by one with their own tau.
+            // Pairs closer than c_min always go to float64; c_min is where tau reaches 0.1 bin (or lo, if that is larger).
+            // Below lo nothing can be mis-binned INTO range as long as lo >> e_abs.
             if (c_lo < 16.0 * e_abs) p.always_refine = 1;          // (bins finer than the float32 unit vectors resolve)
-            double c_min = cbrt(sc * stretch * e_abs * c_hi * c_hi);
+            const double lgmax = fabs(log2(fmax(c_lo * c_lo * 0.25, 1e-37))) + 2.0;
+            const double ks = 1.25 * tau_scale;
+            const double tau_a = ks * (sc * stretch * rel + (double)A.S * (1.0 / 2097152.0 + 2.0 * kU * lgmax) +
+                                       4.0 * kU * ((double)A.S * lgmax + fabs((double)A.O) + n1 + 1.0) + 1.5 * series_err);
+            const double tau_b = ks * sc * stretch * e_abs;
+            double c_min = fmax(c_lo, tau_b / 0.1);
             c_min = fmin(c_min, 0.5 * c_hi);
-            if (c_min <= c_lo) { c_min = c_lo; p.q_small = 0.f; }
+            double c_mid = fmax(c_min, fmin(0.1 * c_hi, 64.0 * cbrt(sc * stretch * e_abs * c_hi * c_hi)));
+            c_mid = fmin(c_mid, 0.5 * c_hi);
+            if (c_min <= c_lo) p.q_small = 0.f;
             else { const double cs = c_min * 1.001 + 2.0 * e_abs; p.q_small = (float)(cs * cs * (1.0 + 16.0 * kU)); }
-            const double lgmax = fabs(log2(fmax(c_min * c_min * 0.25, 1e-37))) + 2.0;
-            tau1 = sc * stretch * (e_abs / fmax(c_min, 1e-18) + rel) + (double)A.S * (1.0 / 2097152.0 + 2.0 * kU * lgmax) +
-                   4.0 * kU * ((double)A.S * lgmax + fabs((double)A.O) + n1 + 1.0) + 1.5 * series_err;
-            tau1 *= 1.25 * tau_scale;
+            { const double cs = c_mid * 1.001 + 2.0 * e_abs; p.q_mid = (float)(cs * cs * (1.0 + 16.0 * kU)); }
+            // (the float32 chord is within e_abs of the true one: 1 / c_true <= (1 + 2 e_abs / c) / c_float32, c >= c_lo)
+            p.tau_a = (float)(tau_a * 1.0001);
+            p.tau_b = (float)(tau_b * (1.0 + 2.0 * e_abs / fmax(c_min, 1e-18)) * 1.001);
+            p.tau_mid = (float)(tau_a + tau_b / fmax(c_min, 1e-18));
+            tau1 = tau_a + tau_b / c_mid;
             const double cp = chord_of(fmin(kPi, b->hi1 * (1.0 + 2.0 * tau1 / sc))) * (1.0 + 32.0 * kU) + e_abs;
             p.q_hi = (float)(fmin(4.0, cp * cp) * (1.0 + 8.0 * kU));
         } else {

@@ -91,6 +91,8 @@ struct PairParams {
     int hist_shared;             // 1: one histogram copy per CTA (large 2-D histograms), flushed with atomicExch
     float q_hi;                  // coarse float32 range test on q (padded)
     float q_small;               // ANGULAR: pairs with q below this are always recomputed in float64 (theta < theta_min)
+    float q_mid, tau_mid;        // ANGULAR log bins: a1.tau holds for chord^2 >= q_mid, tau_mid for q_small <= chord^2 < q_mid
+    float tau_a, tau_b;          // ... and a pair's own bound is tau_a + tau_b / chord
     float dz_hi;                 // RADIAL: coarse test on |dz|
     FastAxis a1, a2;
     // float64 side (refine path): exact definition

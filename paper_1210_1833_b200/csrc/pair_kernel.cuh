@@ -340,6 +340,7 @@ struct IPoints {           // the R = 4 i-points of this lane as two packed pair
 
 struct Consts {            // loop constants held in registers (not re-read from the constant bank)
     float q_hi, q_small, dz_hi, Lf, invL;   // q_small: ANGULAR, pairs closer than theta_min always go to float64
+    float q_mid, thr_mid, tau_a, tau_b;     // ANGULAR log bins: tau = tau_a + tau_b / chord; thr1 holds for q >= q_mid
     float S1, O1h, thr1, top1, tauw1, c1, c2, c3, c4;   // O1h = O - 1/2, thr1 = 1/2 - tau, top1 = MAGIC + n1
     float S2, O2h, top2, tv2, tauw2, cc2;               // tv2 = tau2 - 1/2
     uint32_t n2p;
@@ -349,7 +350,8 @@ template <int KIND>
 __device__ __forceinline__ Consts load_consts(const PairParams &p)
 {
     Consts c;
-    c.q_hi = p.q_hi; c.q_small = p.q_small; c.dz_hi = p.dz_hi; c.Lf = p.Lf; c.invL = p.Lf > 0.f ? 1.0f / p.Lf : 0.f;
+    c.q_hi = p.q_hi; c.q_small = p.q_small; c.dz_hi = p.dz_hi;
+    c.q_mid = p.q_mid; c.thr_mid = 0.5f - p.tau_mid; c.tau_a = p.tau_a; c.tau_b = p.tau_b; c.Lf = p.Lf; c.invL = p.Lf > 0.f ? 1.0f / p.Lf : 0.f;
     c.S1 = p.a1.S; c.O1h = p.a1.O - 0.5f; c.thr1 = 0.5f - p.a1.tau; c.top1 = CUTE_MAGIC_F + (float)p.n1; c.tauw1 = p.a1.tau_w;
     c.c1 = p.a1.c1; c.c2 = p.a1.c2; c.c3 = p.a1.c3; c.c4 = p.a1.c4;
     c.S2 = p.a2.S; c.O2h = p.a2.O - 0.5f; c.top2 = CUTE_MAGIC_F + (float)p.n2; c.tv2 = p.a2.tau - 0.5f; c.tauw2 = p.a2.tau_w;
@@ -612,14 +614,30 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
                         else red_shared(addr[u][r]);
                     }
                 }
-                if (flag[0] || flag[1] || (KIND == CUTE_ANGULAR && qm < c.q_small)) {   // rare: undo and queue the uncertain pairs for float64
+                // ANGULAR, log bins: the error of log(theta) grows as 1 / theta.  thr1 is sized for chords above sqrt(q_mid)
+                // (nearly every pair); a block that holds a closer pair is examined with the loose threshold of the
+                // closest allowed chord, and the pairs are then decided one by one with their own tau = a + b / chord.
+                bool near_flag = false;
+                if (KIND == CUTE_ANGULAR && LOGB && qm < c.q_mid) {
+                    float am = 0.f;
+#pragma unroll
+                    for (int u = 0; u < 2; u++)
+#pragma unroll
+                        for (int r = 0; r < R; r++) am = fmaxf(am, va[u][r]);
+                    near_flag = am > c.thr_mid;
+                }
+                if (flag[0] || flag[1] || near_flag || (KIND == CUTE_ANGULAR && qm < c.q_small)) {   // rare: undo and queue the uncertain pairs for float64
 #pragma unroll
                     for (int u = 0; u < 2; u++) {
                         uint32_t need = 0;
 #pragma unroll
                         for (int r = 0; r < R; r++)
-                            if ((va[u][r] > c.thr1 || vb[u][r] > 0.f || (KIND == CUTE_ANGULAR && q[u][r] < c.q_small)) && q[u][r] < c.q_hi)
-                                need |= 1u << r;
+                        {
+                            bool unc = va[u][r] > c.thr1 || vb[u][r] > 0.f || (KIND == CUTE_ANGULAR && q[u][r] < c.q_small);
+                            if (KIND == CUTE_ANGULAR && LOGB)   // the pair's own tau (q_mid > 0 only for log bins)
+                                unc = q[u][r] < c.q_small || va[u][r] > 0.5f - fmaf(c.tau_b, fast_rsqrt(fmaxf(q[u][r], 1.0e-30f)), c.tau_a);
+                            if (unc && q[u][r] < c.q_hi) need |= 1u << r;
+                        }
                         if (need) push_refine<KIND>(p, s, need, ip.idx0, j0 + jj + u, hoff, refined_inline,
                                                     make_uint4(addr[u][0], addr[u][1], addr[u][2], addr[u][3]), 1);
                     }
