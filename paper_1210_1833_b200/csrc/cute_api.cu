@@ -580,7 +580,16 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
         // error of one separation component: input rounding, subtraction rounding, periodic image
         // (minimum image by d - L rint(d/L): a d within rounding of L/2 may take the other image, |d'| off by <= 2uL)
         double e_d = (f64in ? 2.0 * kU * M : 0.0) + kU * (minimg ? 3.0 * b->box_L : b->hi1 * 1.01);
-        if (p.periodic && !minimg) e_d += 2.0 * kU * 2.0 * b->box_L;
+        if (p.periodic && !minimg) {
+            // the periodic image is taken by subtracting L from the larger coordinate: exact (Sterbenz) when the wrapped
+            // cells lie in the upper half of the box, i.e. nc >= 2k + 2 on every axis; else one rounding at ulp(2L)
+            bool exact = true;
+            for (int d = 0; d < 3; d++) {
+                const int k = (int)ceil(g1->spec.rmax / g1->cell[d] * (1.0 - 1e-12));
+                if (g1->spec.ncell[d] < 2 * k + 2) exact = false;
+            }
+            if (!exact) e_d += 2.0 * kU * 2.0 * b->box_L;
+        }
         const double e_r = sqrt(3.0) * e_d;                    // | |d+e| - |d| | <= |e|
         const double rel = 8.0 * kU;                           // q accumulation + MUFU sqrt/lg2
         if (b->log1) {

@@ -648,12 +648,18 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
 }
 
 // ------------------------------------------------------------------------------- G4: neighbour schedule
-// Segment code: bits 0-1 / 2-3 / 4-5 = periodic image of the i-points along x / y / z
-// (0: none, 1: +L, 2: -L); bit 8: same cell row in an auto-correlation (count j > i only).
-__device__ __forceinline__ float image_shift(uint32_t code, int axis, float L)
+// Segment code: bits 0-1 / 2-3 / 4-5 = periodic image along x / y / z (0: none, 1: the i-points are one box length BELOW
+// the j-points, 2: above); bit 8: same cell row in an auto-correlation (count j > i only).
+// The image is applied by subtracting L from the LARGER coordinate, which is exact in float32 (Sterbenz: L/2 <= x <= 2L for a
+// point in the top cells of the box): code 2 shifts the i-points (registers, once per segment), code 1 shifts the j-points
+// (in the shared-memory tile, once per tile).  Adding L to the smaller coordinate would round at ulp(2L).
+__device__ __forceinline__ float image_shift_i(uint32_t code, int axis, float L)
 {
-    uint32_t c = (code >> (2 * axis)) & 3u;
-    return c == 1u ? L : (c == 2u ? -L : 0.f);
+    return ((code >> (2 * axis)) & 3u) == 2u ? -L : 0.f;
+}
+__device__ __forceinline__ float image_shift_j(uint32_t code, int axis, float L)
+{
+    return ((code >> (2 * axis)) & 3u) == 1u ? -L : 0.f;
 }
 
 // Lane `nb` expands neighbour row number nb of the chunk into <= 3 contiguous ranges of the
@@ -869,6 +875,7 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
             if (have) issue(stage, t_j0, t_cnt);
             int active_slot = -1;
             bool seg_mask = false;
+            float jsx = 0.f, jsy = 0.f, jsz = 0.f;   // image shift of this segment's j-points
             while (have) {
                 uint32_t n_j0 = 0, n_cnt = 0; int n_slot = 0;
                 const bool have_next = next_tile(n_j0, n_cnt, n_slot);
@@ -880,7 +887,8 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
                     const uint32_t code = s.segs[t_slot].z;
                     seg_mask = (code & 0x100u) != 0;
                     if (KIND == CUTE_MONOPOLE && !MINIMG && p.periodic) {
-                        const float sx = image_shift(code, 0, p.Lf), sy = image_shift(code, 1, p.Lf), sz = image_shift(code, 2, p.Lf);
+                        const float sx = image_shift_i(code, 0, p.Lf), sy = image_shift_i(code, 1, p.Lf), sz = image_shift_i(code, 2, p.Lf);
+                        jsx = image_shift_j(code, 0, p.Lf); jsy = image_shift_j(code, 1, p.Lf); jsz = image_shift_j(code, 2, p.Lf);
 #pragma unroll
                         for (int h = 0; h < 2; h++) {
                             ip.X[h] = pk(bx[2 * h] + sx, bx[2 * h + 1] + sx);
@@ -890,6 +898,14 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
                     }
                 }
                 float4 *th = s.thi + stage * kTile, *tl = s.tlo + stage * kTile;
+                if (KIND == CUTE_MONOPOLE && !MINIMG && (jsx != 0.f || jsy != 0.f || jsz != 0.f)) {
+                    for (uint32_t k = lane; k < t_cnt; k += 32) {   // this tile's j-points take the image (exact, see above)
+                        float4 v = th[k];
+                        v.x += jsx; v.y += jsy; v.z += jsz;
+                        th[k] = v;
+                    }
+                    __syncwarp();
+                }
                 if (t_cnt & 1u) {   // odd tile: pad with a sentinel j-point (never in range); the tile has room (t_cnt < kTile)
                     if (lane == 0) {
                         // (-kSentinel: the padding I-points sit at +kSentinel and must not meet the padding j at distance 0)
