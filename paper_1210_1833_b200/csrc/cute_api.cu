@@ -336,13 +336,20 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
         int64_t cap = mc;
         for (int d = 0; d < 3; d++) {
             if (spec->ncell[d] > 0) nc[d] = spec->ncell[d];
-            else {   // cell side ~ rmax/4  =>  k = ceil(rmax/a) = 4: with the corners of the 9^3 cube trimmed, ~45 % of
-                     // the evaluated pairs are in range (measured on C5: 1.35x faster than rmax/2); periodic needs nc >= 2k+1
-                // ... but not so small that a cell holds fewer than ~150 points on average: a 128-point work item
-                // should come from one or two cells, else its j-ranges widen again (measured on C3)
+            else {   // cell side a = rmax / k with an INTEGER k (k cells reach exactly rmax: a side just below rmax / k
+                     // costs a whole extra layer of cells).  Measured (profiles/r02_cells.md): k = 4 or 5 is the optimum for
+                     // both C3 (sparse, 50 Mpc/h: -16 % time against rmax / 2) and C5 (dense, 40 Mpc/h: -5 % against
+                     // rmax / 4) -- smaller cells trim the searched volume closer to the sphere, until a 128-point work item
+                     // spans too many of them.  k = 5 when a cell then still holds >= 64 points on average, else 4, falling
+                     // back to 3 and 2 for catalogues so sparse that a cell would hold < 8.
                 const double vol = g->spec.size[0] * g->spec.size[1] * g->spec.size[2];
-                const double a_dens = cat->n > 0 ? cbrt(150.0 * vol / (double)cat->n) : 0.0;
-                const double a_want = fmax(0.25 * spec->rmax, fmin(a_dens, 0.5 * spec->rmax));
+                const double dens = cat->n > 0 && vol > 0.0 ? (double)cat->n / vol : 0.0;
+                auto per_cell = [&](int k) { const double a = spec->rmax / k; return dens * a * a * a; };
+                int kk = 2;
+                if (per_cell(5) >= 64.0) kk = 5;
+                else if (per_cell(4) >= 8.0) kk = 4;
+                else if (per_cell(3) >= 8.0) kk = 3;
+                const double a_want = spec->rmax / kk;
                 double t = floor(g->spec.size[d] / a_want * (1.0 + 1e-12));
                 nc[d] = t < 1 ? 1 : (t > 1024 ? 1024 : (int)t);
                 if (spec->periodic) {   // nearest cell count with nc >= 2 ceil(rmax/a) + 1
