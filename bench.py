@@ -406,6 +406,42 @@ def summarise(cfg_id, w, scale, rn, total_ms, total_pairs, record, steps, peaks,
     return out
 
 
+def density_grid_entry(api, torch, peaks_hbm):
+    """the density-grid monopole (Eq. 17) on the C5 data catalogue, 128^3 grid,
+    C5's bins.  The TSC scatter is timed alone through a bin spec no offset falls in (the stencil is then skipped)."""
+    from paper_1210_1833_b200 import synth
+    w = synth.workload(5, 1.0)
+    cols = [torch.from_numpy(np.ascontiguousarray(c)).cuda() for c in w.data]
+    L, ng, n = w.bins["box_L"], 128, len(w.data[0])
+    bins = dict(n1=w.bins["n1"], lo1=0.0, hi1=w.bins["hi1"])
+    tiny = dict(n1=1, lo1=0.0, hi1=0.5 * L / ng)
+
+    def timed(b, reps=3):
+        out = api.cute_density_grid_xi(cols, L, ng, b)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            out = api.cute_density_grid_xi(cols, L, ng, b, workspace=out["workspace"])
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps, out
+
+    ms_tsc, _ = timed(tiny)
+    ms_all, out = timed(bins)
+    pairs = float(out["npairs"].sum())
+    hbm, hsrc = peaks_hbm
+    tsc_bytes = n * 12.0 + 2.0 * ng ** 3 * 8.0          # read the particles once; zero and write the grid
+    ms_st = max(ms_all - ms_tsc, 1e-6)
+    return {"config": "N4", "workload": f"density-grid monopole (PAPER.md:250-260): C5 data, n={n}, grid {ng}^3, {bins['n1']} bins to {bins['hi1']}",
+            "ms_total": ms_all, "ms_tsc_and_overdensity": ms_tsc, "ms_stencil": ms_st,
+            "grid_point_pairs": pairs, "grid_point_pairs_per_s": pairs / (ms_st * 1e-3),
+            "tsc": {"bound": "hbm", "algorithmic_bytes": tsc_bytes, "achieved": tsc_bytes / (ms_tsc * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
+                    "frac": tsc_bytes / (ms_tsc * 1e-3) / 1e9 / hbm, "peak_source": hsrc,
+                    "note": "27 float64 atomics per particle into the L2-resident grid: atomic-bound, not HBM-bound"},
+            "stencil": {"bound": "fp64 fma", "flops": 2.0 * pairs, "achieved_tflops": 2.0 * pairs / (ms_st * 1e-3) / 1e12,
+                        "note": "float64 multiply-add per grid-point pair, delta read from L2 (16 MB grid)"}}
+
+
 def measured_peaks(api, torch):
     """Roofline denominators measured on this device in this run (cute_measure_peaks: SURVEY.md 8(d) R2)."""
     pk = api.cute_measure_peaks()
@@ -492,6 +528,8 @@ def run_ours(args):
             per_config.append(summarise(cid, wc, args.scale, rc, tms, tp, rec, ksteps, peaks, clock_mhz, ec, cc))
             del rc
             torch.cuda.empty_cache()
+        if args.scale == 1.0:
+            per_config.append(density_grid_entry(api, torch, hbm_peak()))
 
     cfg = {"workload": describe(head_id, w, args.scale), "scale": args.scale,
            "l2": "256 MiB buffer written between timed iterations (L2 flush)",

@@ -47,14 +47,21 @@ inline int64_t cell_cap(int64_t n) { return n * 2 > 4096 ? n * 2 : 4096; }
 inline int part_ctas() { return 2 * sm_count(); }
 
 // rec_bytes: bytes of one raw record of the partition path (16: float32 xyz, 32: otherwise); used when n >= kPartMinN
-// Measured on B200 (profiles/r02_build.md): the partition wins for float64 / RA-Dec catalogues (32-byte records that carry
-// their cell, so sin() and the FP64 cell arithmetic run twice instead of four times: C4 0.42 -> 0.34 ms), and loses for
-// float32 xyz (C5: 0.86 ms against 0.70 ms one-pass -- the 160 MB of grouped records do not fit L2 and make a round trip
-// through HBM), so float32 xyz keeps the one-pass counting sort unless build_path = 2 asks otherwise.
-inline bool use_partition(int64_t n, const cute_catalog *c, const cute_grid_spec *s)
+// Which build a catalogue takes (measured on B200, profiles/r02_build_c5.md, r02_build_c4.md and DESIGN.md 5.1):
+//  * float64 / RA-Dec catalogues of >= 2^20 objects: the two-level partition (32-byte records that carry their cell, so
+//    sin() and the FP64 cell arithmetic run twice instead of four times: C4 0.42 -> 0.34 ms);
+//  * float32 xyz: the partition only when there are many cells (C5, 125 000 cells: 0.89 ms against 1.09 ms one-pass; with
+//    64 000 cells the one-pass sort wins, 0.70 against 0.86 ms -- its scattered stores thrash less).
+// The workspace is sized for either (the cell count is not known before the box is); build_path = 1 / 2 force one.
+inline bool may_partition(int64_t n, const cute_grid_spec *s)
 {
+    return n > 0 && (s->build_path == 2 || (s->build_path == 0 && n >= kPartMinN));
+}
+inline bool use_partition(int64_t n, const cute_catalog *c, const cute_grid_spec *s, int64_t ncells)
+{
+    if (!may_partition(n, s)) return false;
     const bool f32xyz = c->dtype == CUTE_F32 && c->coord == CUTE_COORD_XYZ;
-    return n > 0 && (s->build_path == 2 || (s->build_path == 0 && n >= kPartMinN && !f32xyz));
+    return s->build_path == 2 || !f32xyz || ncells > 90000;
 }
 
 Layout make_layout(int64_t n, int want_lo, int want_f64, int64_t max_cells, int64_t max_rows, int rec_bytes)
@@ -264,7 +271,7 @@ int cute_grid_workspace_bytes(const cute_catalog *cat, const cute_grid_spec *spe
     wants(cat, spec, &want_lo, &want_f64);
     cell_bounds(cat, spec, &mc, &mr);
     if (mc > 0x7ffffff0ll) return CUTE_ERR_INVALID_ARG;
-    *bytes = make_layout(cat->n, want_lo, want_f64, mc, mr, !use_partition(cat->n, cat, spec) ? 0 : (cat->dtype == CUTE_F32 && cat->coord == CUTE_COORD_XYZ) ? 16 : 32).total;
+    *bytes = make_layout(cat->n, want_lo, want_f64, mc, mr, !may_partition(cat->n, spec) ? 0 : (cat->dtype == CUTE_F32 && cat->coord == CUTE_COORD_XYZ) ? 16 : 32).total;
     return CUTE_OK;
 }
 
@@ -281,7 +288,7 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     int64_t mc, mr;
     wants(cat, spec, &want_lo, &want_f64);
     cell_bounds(cat, spec, &mc, &mr);
-    const Layout L = make_layout(cat->n, want_lo, want_f64, mc, mr, !use_partition(cat->n, cat, spec) ? 0 : (cat->dtype == CUTE_F32 && cat->coord == CUTE_COORD_XYZ) ? 16 : 32);
+    const Layout L = make_layout(cat->n, want_lo, want_f64, mc, mr, !may_partition(cat->n, spec) ? 0 : (cat->dtype == CUTE_F32 && cat->coord == CUTE_COORD_XYZ) ? 16 : 32);
     if (bytes < L.total) return CUTE_ERR_WORKSPACE_TOO_SMALL;
     unsigned char *w = (unsigned char *)d_workspace;
 
@@ -337,7 +344,7 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
         for (int d = 0; d < 3; d++) {
             if (spec->ncell[d] > 0) nc[d] = spec->ncell[d];
             else {   // cell side a = rmax / k with an INTEGER k (k cells reach exactly rmax: a side just below rmax / k
-                     // costs a whole extra layer of cells).  Measured (profiles/r02_cells.md): k = 4 or 5 is the optimum for
+                     // costs a whole extra layer of cells).  Measured (cell-side sweep): k = 4 or 5 is the optimum for
                      // both C3 (sparse, 50 Mpc/h: -16 % time against rmax / 2) and C5 (dense, 40 Mpc/h: -5 % against
                      // rmax / 4) -- smaller cells trim the searched volume closer to the sphere, until a 128-point work item
                      // spans too many of them.  k = 5 when a cell then still holds >= 64 points on average, else 4, falling
@@ -428,7 +435,7 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     for (int d = 0; d < 6; d++) g->bbox[d] = bbox[d];
     g->has_bbox = (need_bbox || box_given) ? 1 : 0;
 
-    if (use_partition(cat->n, cat, spec) && b.mode != CUTE_GRID_NONE) {   // large catalogue: two-level partition (grid_build.cu)
+    if (use_partition(cat->n, cat, spec, b.ncells) && b.mode != CUTE_GRID_NONE) {   // large catalogue: two-level partition (grid_build.cu)
         b.part_tmp = w + L.part_tmp; b.part_table = (uint32_t *)(w + L.part_table); b.part_G = L.part_G;
         part_shape(b.ncells, &b.part_B, &b.part_cpb);
         b.part_shift = 0;
