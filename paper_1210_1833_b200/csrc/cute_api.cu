@@ -343,20 +343,19 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
         int64_t cap = mc;
         for (int d = 0; d < 3; d++) {
             if (spec->ncell[d] > 0) nc[d] = spec->ncell[d];
-            else {   // cell side a = rmax / k with an INTEGER k (k cells reach exactly rmax: a side just below rmax / k
-                     // costs a whole extra layer of cells).  Measured (cell-side sweep): k = 4 or 5 is the optimum for
-                     // both C3 (sparse, 50 Mpc/h: -16 % time against rmax / 2) and C5 (dense, 40 Mpc/h: -5 % against
-                     // rmax / 4) -- smaller cells trim the searched volume closer to the sphere, until a 128-point work item
-                     // spans too many of them.  k = 5 when a cell then still holds >= 64 points on average, else 4, falling
-                     // back to 3 and 2 for catalogues so sparse that a cell would hold < 8.
+            else {   // Cell side along y and z: a = rmax / k with an INTEGER k (k cells reach exactly rmax: a side just
+                     // below rmax / k costs a whole extra layer of rows), k such that a 128-point work item is about as long
+                     // along x as a row is wide (128 = 1.7 n a^3): longer items are sticks that almost every j-point is
+                     // partly in range of, shorter ones waste the trimming.  Along x, the contiguous axis, the cells only
+                     // set the granularity of the trimmed j-ranges: a / 4.  Measured (cell sweeps): C5
+                     // (40, 40, 40) 618 ms -> (10, 40, 40) 562 ms; C3 (50, 50, 50) 49.6 ms -> (17, 67, 67) 44.6 ms; round 1's
+                     // rmax/2 and rmax/4 cubes: 58 and 649 ms.  A non-periodic catalogue rarely fills its bounding box
+                     // (a survey footprint fills about a third of it): its density is taken three times the box average.
                 const double vol = g->spec.size[0] * g->spec.size[1] * g->spec.size[2];
-                const double dens = cat->n > 0 && vol > 0.0 ? (double)cat->n / vol : 0.0;
-                auto per_cell = [&](int k) { const double a = spec->rmax / k; return dens * a * a * a; };
-                int kk = 2;
-                if (per_cell(5) >= 64.0) kk = 5;
-                else if (per_cell(4) >= 8.0) kk = 4;
-                else if (per_cell(3) >= 8.0) kk = 3;
-                const double a_want = spec->rmax / kk;
+                const double dens = (cat->n > 0 && vol > 0.0 ? (double)cat->n / vol : 0.0) * (spec->periodic ? 1.0 : 3.0);
+                int kk = dens > 0.0 ? (int)lround(spec->rmax / cbrt(75.0 / dens)) : 2;
+                kk = kk < 2 ? 2 : (kk > 5 ? 5 : kk);
+                const double a_want = spec->rmax / kk * (d == 0 ? 0.25 : 1.0);
                 double t = floor(g->spec.size[d] / a_want * (1.0 + 1e-12));
                 nc[d] = t < 1 ? 1 : (t > 1024 ? 1024 : (int)t);
                 if (spec->periodic) {   // nearest cell count with nc >= 2 ceil(rmax/a) + 1
