@@ -798,9 +798,13 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
         }
 #pragma unroll
         for (int h = 0; h < 2; h++) {
-            ip.X[h] = pk(bx[2 * h], bx[2 * h + 1]); ip.Y[h] = pk(by[2 * h], by[2 * h + 1]); ip.Z[h] = pk(bz[2 * h], bz[2 * h + 1]);
-            ip.W[h] = pk(bw[2 * h], bw[2 * h + 1]);
-            ip.LW[h] = pk(lw[2 * h], lw[2 * h + 1]);
+            // (the packed pairs are BORN in an aligned register pair by a packed add of +0: ptxas otherwise keeps the scalars
+            // of the LDG.128 results and re-assembles every pair with two MOVs before each use inside the loop)
+            const f32x2 z2 = bc(0.f);
+            ip.X[h] = add2(pk(bx[2 * h], bx[2 * h + 1]), z2); ip.Y[h] = add2(pk(by[2 * h], by[2 * h + 1]), z2);
+            ip.Z[h] = add2(pk(bz[2 * h], bz[2 * h + 1]), z2);
+            ip.W[h] = add2(pk(bw[2 * h], bw[2 * h + 1]), z2);
+            ip.LW[h] = add2(pk(lw[2 * h], lw[2 * h + 1]), z2);
         }
 
         if ((FLAGS & PK_WEIGHTED) && p.is_auto && p.self_bin >= 0 && sp == 0) {
