@@ -15,10 +15,11 @@ constexpr int kTile = 128;                        // j-points per shared-memory 
 constexpr int kStages = 2;                        // double buffering
 constexpr int kSegBatch = 32;                     // neighbour rows expanded per batch (one per lane)
 constexpr int kSegSlots = 3 * kSegBatch;          // <= 3 contiguous j-segments per neighbour row
-constexpr int kRefineCap = 64;                    // deferred float64 recomputations queued per warp
+constexpr int kRefineCap = 64;                    // flagged blocks queued per warp for re-examination (pair_kernel.cuh)
 #ifndef CUTE_MAX_WARPS
 #define CUTE_MAX_WARPS 16                         // warps per CTA = per SM (registers: 65536 / (32 * warps) per thread)
 #endif
+constexpr int kPairCap = 96;                      // uncertain pairs queued per warp for float64 (settled 32 at a time)
 constexpr int kMaxWarps = CUTE_MAX_WARPS;
 constexpr float kSentinel = 1.0e18f;              // coordinate of a padding i-point (never in range)
 constexpr uint32_t kEpochJ = 1u << 22;            // flush a warp's uint32 histogram after this many j

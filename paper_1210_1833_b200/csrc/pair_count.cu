@@ -14,7 +14,7 @@ static inline uint32_t hist_bytes(int nhist_pad, int colshift)
 
 static inline uint32_t warp_smem_bytes(bool needlo, int nhist_pad, int colshift, bool shared_hist)
 {
-    uint32_t b = kStages * kTileBytesHost * (needlo ? 2 : 1) + kSegSlots * 16 + kRefineCap * 8 + 32;
+    uint32_t b = kStages * kTileBytesHost * (needlo ? 2 : 1) + kSegSlots * 16 + kRefineCap * 16 + kPairCap * 16 + 32;
     if (!shared_hist) b += hist_bytes(nhist_pad, colshift);
     return (b + 127) & ~127u;
 }

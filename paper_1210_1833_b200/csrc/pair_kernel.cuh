@@ -239,8 +239,9 @@ constexpr uint32_t kTileBytes = kTile * 16;
 struct WarpSmem {          // pointers into this warp's slice of dynamic shared memory
     float4 *thi, *tlo;     // [kStages][kTile]
     uint4 *segs;           // [kSegSlots] {j_begin, j_end, code, -}
-    uint2 *rq;             // [kRefineCap] deferred (i, j)
-    uint32_t *rq_count;
+    uint4 *rq;             // [kRefineCap] flagged blocks {idx0, j, meta, i_last} (see flag_block)
+    uint4 *pq;             // [kPairCap] uncertain pairs {i, j, provisional address, weight}
+    uint32_t *rq_count, *pq_count;
     uint32_t *hist;        // [nhist_pad << colshift]
     uint32_t bar[kStages]; // shared-space addresses of the mbarriers
 };
@@ -255,10 +256,13 @@ __device__ __forceinline__ WarpSmem carve(unsigned char *ws)
     if (NEEDLO) ws += kStages * kTileBytes;
     s.segs = reinterpret_cast<uint4 *>(ws);
     ws += kSegSlots * 16;
-    s.rq = reinterpret_cast<uint2 *>(ws);
-    ws += kRefineCap * 8;
+    s.rq = reinterpret_cast<uint4 *>(ws);
+    ws += kRefineCap * 16;
+    s.pq = reinterpret_cast<uint4 *>(ws);
+    ws += kPairCap * 16;
     for (int k = 0; k < kStages; k++) s.bar[k] = smem_u32(ws + 8 * k);
     s.rq_count = reinterpret_cast<uint32_t *>(ws + 8 * kStages);
+    s.pq_count = s.rq_count + 1;
     ws += 32;
     s.hist = reinterpret_cast<uint32_t *>(ws);
     return s;
@@ -310,29 +314,10 @@ __device__ __forceinline__ uint32_t pair_weight(const PairParams &p, uint32_t i,
     return __float_as_uint(p.g1.hi[i].w) * __float_as_uint(p.g2.hi[j].w);
 }
 
-// deferred float64 recomputation of the queued pairs, one per lane
-template <int KIND>
-__device__ __forceinline__ uint32_t drain_refine(const PairParams &p, const WarpSmem &s, int lane)
-{
-    __syncwarp();
-    uint32_t n = *s.rq_count;
-    n = n < (uint32_t)kRefineCap ? n : (uint32_t)kRefineCap;
-    uint32_t done = 0;
-    for (uint32_t e = lane; e < n; e += 32) {
-        uint2 ij = s.rq[e];
-        int cell = refine_cell<KIND>(p, ij.x, ij.y);
-        if (cell >= 0) atomicAdd(s.hist + ((pad_cell(p, (uint32_t)cell) << p.colshift) + (lane & ((1 << p.colshift) - 1))), pair_weight(p, ij.x, ij.y));
-        done++;
-    }
-    __syncwarp();
-    if (lane == 0) *s.rq_count = 0;
-    __syncwarp();
-    return done;
-}
-
 // ------------------------------------------------------------------------------- the per-pair body
 struct IPoints {           // the R = 4 i-points of this lane as two packed pairs (points 0,1 and 2,3)
     f32x2 X[2], Y[2], Z[2];      // hi (already shifted by the segment's periodic image)
+    f32x2 X0[2], Y0[2], Z0[2];   // hi, unshifted (periodic cell lists re-derive X, Y, Z per segment)
     f32x2 W[2], LW[2];           // RMU / PISIGMA: |x|^2 hi, |x|^2 lo
     float w[R];                  // RADIAL: z; WEIGHTED: weight bit patterns
     uint32_t idx0;               // cell-sorted index of i-point 0 (point r is idx0 + 32 r)
@@ -362,27 +347,6 @@ __device__ __forceinline__ Consts load_consts(const PairParams &p)
     }
     c.n2p = (uint32_t)p.n2p;
     return c;
-}
-
-// rare path: the pairs of this lane whose float32 bin is not certain (bit r of `need`).  Their provisional increment
-// (already made at addr[r], in this lane's column) is undone and the pair is queued for float64.
-template <int KIND>
-__device__ __noinline__ void push_refine(const PairParams &p, const WarpSmem &s, uint32_t need, uint32_t idx0, uint32_t j,
-                                         uint32_t hoff, uint32_t &refined_inline, uint4 addr, int undo)
-{
-    const uint32_t a[R] = {addr.x, addr.y, addr.z, addr.w};
-    for (int r = 0; r < R; r++) {
-        if (!(need & (1u << r))) continue;
-        const uint32_t i = idx0 + 32u * r;
-        if (undo) red_shared_add(a[r], 0u - pair_weight(p, i, j));
-        const uint32_t slot = atomicAdd(s.rq_count, 1u);
-        if (slot < (uint32_t)kRefineCap) s.rq[slot] = make_uint2(i, j);
-        else {
-            const int cell = refine_cell<KIND>(p, i, j);
-            refined_inline++;
-            if (cell >= 0) atomicAdd(s.hist + ((pad_cell(p, (uint32_t)cell) << p.colshift) + hoff), pair_weight(p, i, j));
-        }
-    }
 }
 
 // rint and distance from it, two pairs at a time: r = MAGIC + rint(t), d = t - rint(t) in [-1/2, 1/2]  (t = S g + Oh)
@@ -517,27 +481,311 @@ __device__ __forceinline__ bool bin_map(const PairParams &p, const Consts &c, co
     return flag;
 }
 
+// ------------------------------------------------------------------------------- one guarded block
+// A BLOCK is two j-points against the lane's four i-points (eight pairs per lane, 256 per warp).  The same three
+// functions serve the hot loop (compute_tile) and the deferred re-examination of a flagged block (process_entry),
+// so that both see bit-identical float32 results.
+
+// Segment code: bits 0-1 / 2-3 / 4-5 = periodic image along x / y / z (0: none, 1: the i-points are one box length BELOW
+// the j-points, 2: above); bit 8: same cell row in an auto-correlation (count j > i only).
+// The image is applied by subtracting L from the LARGER coordinate, which is exact in float32 (Sterbenz: L/2 <= x <= 2L for a
+// point in the top cells of the box): code 2 shifts the i-points (registers, once per segment), code 1 shifts the j-points
+// (in the shared-memory tile, once per tile).  Adding L to the smaller coordinate would round at ulp(2L).
+__device__ __forceinline__ float image_shift_i(uint32_t code, int axis, float L)
+{
+    return ((code >> (2 * axis)) & 3u) == 2u ? -L : 0.f;
+}
+__device__ __forceinline__ float image_shift_j(uint32_t code, int axis, float L)
+{
+    return ((code >> (2 * axis)) & 3u) == 1u ? -L : 0.f;
+}
+
+// The lane's i-points: cell-sorted indices idx0 + 32 r (r < 4) up to i_last, padding points beyond it.  The packed pairs
+// are BORN in an aligned register pair by a packed add (of the segment's image shift, or of +0): ptxas otherwise keeps the
+// scalars of the LDG.128 results and re-assembles every pair with two MOVs before each packed use inside the loop
+// (measured: 18 % of C3's issue slots).
+template <int KIND, int FLAGS>
+__device__ __forceinline__ void load_ipoints(const GridView &g1, uint32_t idx0, uint32_t i_last, float sx, float sy, float sz,
+                                             IPoints &ip, float &xmin, float &xmax)
+{
+    constexpr bool NEEDLO = (KIND == CUTE_RMU || KIND == CUTE_PISIGMA || ((FLAGS & PK_WEIGHTED) && KIND != CUTE_ANGULAR));
+    float bx[R], by[R], bz[R], bw[R], lw[R];
+    ip.idx0 = idx0;
+    xmin = 3.0e38f; xmax = -3.0e38f;
+#pragma unroll
+    for (int r = 0; r < R; r++) {
+        const uint32_t k = idx0 + 32u * r;
+        float4 h = make_float4(kSentinel, kSentinel, kSentinel, 0.f);
+        lw[r] = 0.f;
+        float wbits = 0.f;
+        if (k <= i_last) {
+            h = g1.hi[k];
+            if (NEEDLO) { const float4 l = g1.lo[k]; lw[r] = l.w; wbits = l.x; }
+            xmin = fminf(xmin, h.x); xmax = fmaxf(xmax, h.x);
+        }
+        bx[r] = h.x; by[r] = h.y; bz[r] = h.z; bw[r] = h.w;
+        ip.w[r] = ((FLAGS & PK_WEIGHTED) && KIND != CUTE_ANGULAR) ? wbits : h.w;
+    }
+    const f32x2 z2 = bc(0.f);
+#pragma unroll
+    for (int h = 0; h < 2; h++) {
+        ip.X0[h] = add2(pk(bx[2 * h], bx[2 * h + 1]), z2); ip.Y0[h] = add2(pk(by[2 * h], by[2 * h + 1]), z2);
+        ip.Z0[h] = add2(pk(bz[2 * h], bz[2 * h + 1]), z2);
+        ip.W[h] = add2(pk(bw[2 * h], bw[2 * h + 1]), z2);
+        ip.LW[h] = add2(pk(lw[2 * h], lw[2 * h + 1]), z2);
+        ip.X[h] = add2(ip.X0[h], bc(sx)); ip.Y[h] = add2(ip.Y0[h], bc(sy)); ip.Z[h] = add2(ip.Z0[h], bc(sz));
+    }
+}
+
+// P2 for a block; returns the lane's smallest q.  masked: auto-correlation, only j > i counts (j = index of the first j-point)
+template <int KIND, bool MINIMG>
+__device__ __forceinline__ float block_separations(const Consts &c, const IPoints &ip, const float4 pj[2], bool masked, uint32_t j,
+                                                   f32x2 q2[2][2], float q[2][R])
+{
+#pragma unroll
+    for (int u = 0; u < 2; u++) {
+        separations<KIND, MINIMG>(c, ip, pj[u], q2[u]);
+        unpk(q2[u][0], q[u][0], q[u][1]);
+        unpk(q2[u][1], q[u][2], q[u][3]);
+        if (masked) {
+#pragma unroll
+            for (int r = 0; r < R; r++) q[u][r] = (j + u > ip.idx0 + 32u * r) ? q[u][r] : 3.0e38f;
+            q2[u][0] = pk(q[u][0], q[u][1]);
+            q2[u][1] = pk(q[u][2], q[u][3]);
+        }
+    }
+    return fminf(fminf(fminf(q[0][0], q[0][1]), fminf(q[0][2], q[0][3])), fminf(fminf(q[1][0], q[1][1]), fminf(q[1][2], q[1][3])));
+}
+
+// RADIAL / always-refine: the pairs that pass the coarse float32 test (bit 4 u + r)
+template <int KIND>
+__device__ __forceinline__ uint32_t block_candidates(const Consts &c, const IPoints &ip, const float4 pj[2], const float q[2][R])
+{
+    uint32_t need = 0;
+#pragma unroll
+    for (int u = 0; u < 2; u++)
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            bool in = q[u][r] < c.q_hi;
+            if (KIND == CUTE_RADIAL) in = in && (fabsf(ip.w[r] - pj[u].w) < c.dz_hi);
+            if (in) need |= 1u << (4 * u + r);
+        }
+    return need;
+}
+
+// P3 + the addresses of P4 for a block: addr = shared-memory address of the pair's (clamped) padded histogram cell in
+// column hoff; returns "some pair of this lane may be uncertain" (then block_uncertain says which).
+// Padded cell (k1 + 1) [* n2p + (k2 + 1)] of column hoff lives at hb + ((bits(r1) [* n2p + bits(r2)]) << sh): the
+// magic-number bits are folded into the base (all arithmetic modulo 2^32).
+template <int KIND>
+__device__ __forceinline__ uint32_t hist_base(const WarpSmem &s, const Consts &c, uint32_t hoff, uint32_t sh)
+{
+    constexpr uint32_t MB1 = CUTE_MAGIC_BITS - 1u;
+    return smem_u32(s.hist + hoff) - ((kind_is_2d(KIND) ? MB1 * (c.n2p + 1u) : MB1) << sh);
+}
+
+template <int KIND, bool LOGB, int FLAGS>
+__device__ __forceinline__ bool block_bins(const PairParams &p, const Consts &c, const IPoints &ip, const f32x2 q2[2][2], const float q[2][R],
+                                           float qm, const float4 pj[2], const float4 pl[2], uint32_t hb, uint32_t sh,
+                                           uint32_t addr[2][R], float va[2][R], float vb[2][R])
+{
+    constexpr bool SIMPLE = (FLAGS & PK_SIMPLE) != 0;
+    constexpr bool TWO_D = kind_is_2d(KIND);
+    const float bot = CUTE_MAGIC_F - 1.0f;
+    float r1[2][R], r2[2][R];
+    bool flag[2];
+#pragma unroll
+    for (int u = 0; u < 2; u++)
+        flag[u] = bin_map<KIND, LOGB, SIMPLE>(p, c, ip, q2[u], q[u], pj[u].w, pl[u].w, r1[u], r2[u], va[u], vb[u]);
+    // clamp into the padded histogram (no compare, no select)
+#pragma unroll
+    for (int u = 0; u < 2; u++) {
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            float a = fminf(r1[u][r], c.top1);
+            if (!SIMPLE) a = fmaxf(a, bot);
+            uint32_t cell = __float_as_uint(a);
+            if (TWO_D) {
+                float b = fminf(r2[u][r], c.top2);
+                if (!SIMPLE) b = fmaxf(b, bot);
+                cell = cell * c.n2p + __float_as_uint(b);
+            }
+            addr[u][r] = hb + (cell << sh);
+        }
+    }
+    // ANGULAR, log bins: the error of log(theta) grows as 1 / theta.  thr1 is sized for chords above sqrt(q_mid)
+    // (nearly every pair); a block that holds a closer pair is examined with the loose threshold of the
+    // closest allowed chord, and the pairs are then decided one by one with their own tau = a + b / chord.
+    bool near_flag = false;
+    if (KIND == CUTE_ANGULAR && LOGB && qm < c.q_mid) {
+        float am = 0.f;
+#pragma unroll
+        for (int u = 0; u < 2; u++)
+#pragma unroll
+            for (int r = 0; r < R; r++) am = fmaxf(am, va[u][r]);
+        near_flag = am > c.thr_mid;
+    }
+    return flag[0] || flag[1] || near_flag || (KIND == CUTE_ANGULAR && qm < c.q_small);
+}
+
+// the in-range pairs of a flagged block whose float32 bin is not certain (bit 4 u + r)
+template <int KIND, bool LOGB>
+__device__ __forceinline__ uint32_t block_uncertain(const Consts &c, const float q[2][R], const float va[2][R], const float vb[2][R])
+{
+    uint32_t need = 0;
+#pragma unroll
+    for (int u = 0; u < 2; u++)
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            bool unc = va[u][r] > c.thr1 || vb[u][r] > 0.f || (KIND == CUTE_ANGULAR && q[u][r] < c.q_small);
+            if (KIND == CUTE_ANGULAR && LOGB)   // the pair's own tau (q_mid > 0 only for log bins)
+                unc = q[u][r] < c.q_small || va[u][r] > 0.5f - fmaf(c.tau_b, fast_rsqrt(fmaxf(q[u][r], 1.0e-30f)), c.tau_a);
+            if (unc && q[u][r] < c.q_hi) need |= 1u << (4 * u + r);
+        }
+    return need;
+}
+
+// ------------------------------------------------------------------------------- the rare path
+// A lane whose block holds a pair that float32 cannot decide does NOT deal with it in the hot loop (measured on C3: the
+// per-pair undo-and-queue code ran with one lane of 32 active and took 28 % of all issue slots).  It queues the BLOCK:
+// {idx0, first j, meta, i_last}, meta = lane | masked << 5 | (second j is padding) << 6 | image code << 8.  When 32 blocks
+// are queued (and before every flush) the warp re-examines them one per lane (examine_entry): the same float32 arithmetic
+// on the same inputs gives the same bins and the same uncertain pairs, which go to a second queue {i, j, provisional
+// address, weight}.  That queue is emptied 32 pairs at a time, one per lane, all lanes busy (settle_pair): the pair is
+// recomputed in float64 with the paper's definition (refine_cell), and if the float64 cell is not the provisional one the
+// count is moved.
+__device__ __forceinline__ void settle_pair(const PairParams &p, const WarpSmem &s, uint32_t cs, int cell, uint4 pe, int lane)
+{
+    const uint32_t hb = smem_u32(s.hist);
+    const uint32_t col = pe.z ? ((pe.z - hb) >> 2) & ((1u << cs) - 1u) : (uint32_t)lane & ((1u << cs) - 1u);
+    const uint32_t na = cell >= 0 ? hb + 4u * ((pad_cell(p, (uint32_t)cell) << cs) + col) : 0u;
+    if (na != pe.z) {                      // move the provisional count (same column: exact)
+        if (pe.z) red_shared_add(pe.z, 0u - pe.w);
+        if (na) red_shared_add(na, pe.w);
+    }
+}
+
+template <int KIND, bool MINIMG, bool LOGB, int FLAGS>
+__device__ __forceinline__ uint32_t examine_entry(const PairParams &p, const WarpSmem &s, const Consts &c, uint4 en, int lane)
+{
+    constexpr bool ALWAYS = (FLAGS & PK_ALWAYS) != 0 || KIND == CUTE_RADIAL, WEIGHTED = (FLAGS & PK_WEIGHTED) != 0;
+    constexpr bool FIXCS = (FLAGS & PK_FIXCS) != 0;
+    constexpr bool NEEDLW = (KIND == CUTE_RMU || KIND == CUTE_PISIGMA);
+    constexpr bool XYZW = WEIGHTED && KIND != CUTE_ANGULAR;
+    const uint32_t idx0 = en.x, j = en.y, meta = en.z, i_last = en.w, code = meta >> 8;
+    const bool masked = (meta & 32u) != 0, pad2 = (meta & 64u) != 0;
+    const uint32_t cs = FIXCS ? (uint32_t)fixed_colshift(KIND) : (uint32_t)p.colshift, sh = cs + 2u;
+    const uint32_t hoff = (meta & 31u) & ((1u << cs) - 1u);
+    float sx = 0.f, sy = 0.f, sz = 0.f, jsx = 0.f, jsy = 0.f, jsz = 0.f;
+    if (KIND == CUTE_MONOPOLE && !MINIMG && p.periodic) {
+        sx = image_shift_i(code, 0, p.Lf); sy = image_shift_i(code, 1, p.Lf); sz = image_shift_i(code, 2, p.Lf);
+        jsx = image_shift_j(code, 0, p.Lf); jsy = image_shift_j(code, 1, p.Lf); jsz = image_shift_j(code, 2, p.Lf);
+    }
+    IPoints ip;
+    float xmin, xmax;
+    load_ipoints<KIND, FLAGS>(p.g1, idx0, i_last, sx, sy, sz, ip, xmin, xmax);
+    float4 pj[2], pl[2];
+    uint32_t wj[2];
+#pragma unroll
+    for (int u = 0; u < 2; u++) {
+        pl[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (u == 1 && pad2) pj[u] = make_float4(-kSentinel, -kSentinel, -kSentinel, 0.f);
+        else {
+            pj[u] = p.g2.hi[j + u];
+            if (jsx != 0.f || jsy != 0.f || jsz != 0.f) { pj[u].x += jsx; pj[u].y += jsy; pj[u].z += jsz; }
+            if (NEEDLW || XYZW) pl[u] = p.g2.lo[j + u];
+        }
+        wj[u] = WEIGHTED ? __float_as_uint(XYZW ? pl[u].x : pj[u].w) : 1u;
+    }
+    f32x2 q2[2][2];
+    float q[2][R];
+    const float qm = block_separations<KIND, MINIMG>(c, ip, pj, masked, j, q2, q);
+    uint32_t need, addr[2][R];
+    if (ALWAYS) {
+        need = block_candidates<KIND>(c, ip, pj, q);
+#pragma unroll
+        for (int u = 0; u < 2; u++)
+#pragma unroll
+            for (int r = 0; r < R; r++) addr[u][r] = 0u;
+    } else {
+        float va[2][R], vb[2][R];
+        block_bins<KIND, LOGB, FLAGS>(p, c, ip, q2, q, qm, pj, pl, hist_base<KIND>(s, c, hoff, sh), sh, addr, va, vb);
+        need = block_uncertain<KIND, LOGB>(c, q, va, vb);
+    }
+    uint32_t inline_done = 0;
+#pragma unroll
+    for (int u = 0; u < 2; u++)
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            if (!(need & (1u << (4 * u + r)))) continue;
+            const uint4 pe = make_uint4(idx0 + 32u * r, j + u, addr[u][r], WEIGHTED ? __float_as_uint(ip.w[r]) * wj[u] : 1u);
+            const uint32_t slot = atomicAdd(s.pq_count, 1u);
+            if (slot < (uint32_t)kPairCap) s.pq[slot] = pe;
+            else {   // queue full (only the test modes that send every pair to float64 get here)
+                settle_pair(p, s, cs, refine_cell<KIND>(p, pe.x, pe.y), pe, lane);
+                inline_done++;
+            }
+        }
+    return inline_done;
+}
+
+// empties the block queue; the pair queue is emptied in groups of 32 (all of it when `all`)
+template <int KIND, bool MINIMG, bool LOGB, int FLAGS>
+__device__ __noinline__ uint32_t drain_flagged(const PairParams &p, const WarpSmem &s, const Consts &c, int lane, bool all)
+{
+    const uint32_t cs = (FLAGS & PK_FIXCS) ? (uint32_t)fixed_colshift(KIND) : (uint32_t)p.colshift;
+    __syncwarp();
+    uint32_t n = *s.rq_count;
+    n = n < (uint32_t)kRefineCap ? n : (uint32_t)kRefineCap;
+    uint32_t done = 0;
+    for (uint32_t e0 = 0; e0 < n || all; e0 += 32) {
+        if (e0 + lane < n) done += examine_entry<KIND, MINIMG, LOGB, FLAGS>(p, s, c, s.rq[e0 + lane], lane);
+        __syncwarp();
+        uint32_t m = *s.pq_count;
+        m = m < (uint32_t)kPairCap ? m : (uint32_t)kPairCap;
+        const bool last = e0 + 32 >= n;
+        while (m >= 32u || (all && last && m > 0u)) {
+            const uint32_t take = m < 32u ? m : 32u;
+            if ((uint32_t)lane < take) {
+                const uint4 pe = s.pq[m - take + lane];
+                settle_pair(p, s, cs, refine_cell<KIND>(p, pe.x, pe.y), pe, lane);
+            }
+            m -= take; done += (uint32_t)lane < take ? 1u : 0u;
+        }
+        __syncwarp();
+        if (lane == 0) *s.pq_count = m;
+        __syncwarp();
+        if (last) break;
+    }
+    if (lane == 0) *s.rq_count = 0;
+    __syncwarp();
+    return done;
+}
+
+// block queue full (test modes only): the lane examines its block at once
+template <int KIND, bool MINIMG, bool LOGB, int FLAGS>
+__device__ __noinline__ uint32_t examine_overflow(const PairParams &p, const WarpSmem &s, const Consts &c, uint4 en, int lane)
+{
+    return examine_entry<KIND, MINIMG, LOGB, FLAGS>(p, s, c, en, lane);
+}
+
 // One tile of j-points against the lane's i-points, two j-points (eight pairs per lane) per guarded block: the pair
 // of independent chains is what hides the LDS / MUFU / packed-FMA latencies with four warps per scheduler.
-// An odd tile is padded with a sentinel j-point (never in range) by the caller; cnt2 = number of j-PAIRS.
+// An odd tile is padded with a sentinel j-point (never in range) by the caller.  meta0 = lane | masked << 5 | code << 8.
 template <int KIND, bool MINIMG, bool LOGB, int FLAGS, bool MASK>
 __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem &s, const Consts &c, const IPoints &ip,
-                                             const float4 *th, const float4 *tl, uint32_t cnt2, uint32_t j0,
-                                             int lane, uint32_t &refined_inline)
+                                             const float4 *th, const float4 *tl, uint32_t t_cnt, uint32_t j0, uint32_t meta0,
+                                             uint32_t i_last, int lane, uint32_t &refined_inline)
 {
-    constexpr bool FIXCS = (FLAGS & PK_FIXCS) != 0, SIMPLE = (FLAGS & PK_SIMPLE) != 0;
-    constexpr bool ALWAYS = (FLAGS & PK_ALWAYS) != 0, WEIGHTED = (FLAGS & PK_WEIGHTED) != 0;
-    constexpr bool TWO_D = kind_is_2d(KIND);
+    constexpr bool FIXCS = (FLAGS & PK_FIXCS) != 0;
+    constexpr bool ALWAYS = (FLAGS & PK_ALWAYS) != 0 || KIND == CUTE_RADIAL, WEIGHTED = (FLAGS & PK_WEIGHTED) != 0;
     constexpr bool NEEDLW = (KIND == CUTE_RMU || KIND == CUTE_PISIGMA);
     constexpr bool XYZW = WEIGHTED && KIND != CUTE_ANGULAR;   // weights of xyz catalogues: lo.x
     const uint32_t cs = FIXCS ? (uint32_t)fixed_colshift(KIND) : (uint32_t)p.colshift;
     const uint32_t sh = cs + 2u;
     const uint32_t hoff = (uint32_t)lane & ((1u << cs) - 1u);
-    // padded cell (k1 + 1) [* n2p + (k2 + 1)] of column hoff lives at hb + ((bits(r1) [* n2p + bits(r2)]) << sh):
-    // the magic-number bits are folded into the base (all arithmetic modulo 2^32)
-    constexpr uint32_t MB1 = CUTE_MAGIC_BITS - 1u;
-    const uint32_t hb = smem_u32(s.hist + hoff) - ((TWO_D ? MB1 * (c.n2p + 1u) : MB1) << sh);
-    const float bot = CUTE_MAGIC_F - 1.0f;
+    const uint32_t hb = hist_base<KIND>(s, c, hoff, sh);
+    const uint32_t cnt2 = (t_cnt + 1u) >> 1;
     // Measured (C5): reading the NEXT block's j-points before this block's guarded bin path and four copies of the body
     // are worth 4 % on the short monopole body and cost as much on the longer angular / r-mu bodies (registers).
     constexpr bool PREFETCH = KIND == 1 /* CUTE_MONOPOLE */ && !WEIGHTED;
@@ -562,106 +810,34 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
             const uint32_t jn = min(jj + 2u, (uint32_t)kTile - 2u);   // (the last block re-reads inside the tile buffer)
             nx[0] = th[jn]; nx[1] = th[jn + 1];
         }
-#pragma unroll
-        for (int u = 0; u < 2; u++) {
-            separations<KIND, MINIMG>(c, ip, pj[u], q2[u]);
-            unpk(q2[u][0], q[u][0], q[u][1]);
-            unpk(q2[u][1], q[u][2], q[u][3]);
-            if (MASK) {                          // auto-correlation: j > i only
-#pragma unroll
-                for (int r = 0; r < R; r++) q[u][r] = (j0 + jj + u > ip.idx0 + 32u * r) ? q[u][r] : 3.0e38f;
-                q2[u][0] = pk(q[u][0], q[u][1]);
-                q2[u][1] = pk(q[u][2], q[u][3]);
-            }
-        }
-        const float qm = fminf(fminf(fminf(q[0][0], q[0][1]), fminf(q[0][2], q[0][3])),
-                               fminf(fminf(q[1][0], q[1][1]), fminf(q[1][2], q[1][3])));
+        const float qm = block_separations<KIND, MINIMG>(c, ip, pj, MASK, j0 + jj, q2, q);
         if (qm < c.q_hi) {
-            if (ALWAYS || KIND == CUTE_RADIAL) {
-#pragma unroll
-                for (int u = 0; u < 2; u++) {
-                    uint32_t need = 0;
-#pragma unroll
-                    for (int r = 0; r < R; r++) {
-                        bool in = q[u][r] < c.q_hi;
-                        if (KIND == CUTE_RADIAL) in = in && (fabsf(ip.w[r] - pj[u].w) < c.dz_hi);
-                        if (in) need |= 1u << r;
-                    }
-                    if (need) push_refine<KIND>(p, s, need, ip.idx0, j0 + jj + u, hoff, refined_inline, make_uint4(0u, 0u, 0u, 0u), 0);
-                }
-            } else {
-                float r1[2][R], r2[2][R], va[2][R], vb[2][R];
-                bool flag[2];
+            bool flagged;
+            if (ALWAYS) flagged = block_candidates<KIND>(c, ip, pj, q) != 0u;
+            else {
+                uint32_t addr[2][R];
+                float va[2][R], vb[2][R];
+                flagged = block_bins<KIND, LOGB, FLAGS>(p, c, ip, q2, q, qm, pj, pl, hb, sh, addr, va, vb);
+                // ---- P4: increment (an uncertain pair is counted provisionally like any other)
 #pragma unroll
                 for (int u = 0; u < 2; u++)
-                    flag[u] = bin_map<KIND, LOGB, SIMPLE>(p, c, ip, q2[u], q[u], pj[u].w, pl[u].w, r1[u], r2[u], va[u], vb[u]);
-                // ---- P4: clamp into the padded histogram and increment (no compare, no select)
-                uint32_t addr[2][R];
-#pragma unroll
-                for (int u = 0; u < 2; u++) {
 #pragma unroll
                     for (int r = 0; r < R; r++) {
-                        float a = fminf(r1[u][r], c.top1);
-                        if (!SIMPLE) a = fmaxf(a, bot);
-                        uint32_t cell = __float_as_uint(a);
-                        if (TWO_D) {
-                            float b = fminf(r2[u][r], c.top2);
-                            if (!SIMPLE) b = fmaxf(b, bot);
-                            cell = cell * c.n2p + __float_as_uint(b);
-                        }
-                        addr[u][r] = hb + (cell << sh);
                         if (WEIGHTED) red_shared_add(addr[u][r], __float_as_uint(ip.w[r]) * wj[u]);
                         else red_shared(addr[u][r]);
                     }
-                }
-                // ANGULAR, log bins: the error of log(theta) grows as 1 / theta.  thr1 is sized for chords above sqrt(q_mid)
-                // (nearly every pair); a block that holds a closer pair is examined with the loose threshold of the
-                // closest allowed chord, and the pairs are then decided one by one with their own tau = a + b / chord.
-                bool near_flag = false;
-                if (KIND == CUTE_ANGULAR && LOGB && qm < c.q_mid) {
-                    float am = 0.f;
-#pragma unroll
-                    for (int u = 0; u < 2; u++)
-#pragma unroll
-                        for (int r = 0; r < R; r++) am = fmaxf(am, va[u][r]);
-                    near_flag = am > c.thr_mid;
-                }
-                if (flag[0] || flag[1] || near_flag || (KIND == CUTE_ANGULAR && qm < c.q_small)) {   // rare: undo and queue the uncertain pairs for float64
-#pragma unroll
-                    for (int u = 0; u < 2; u++) {
-                        uint32_t need = 0;
-#pragma unroll
-                        for (int r = 0; r < R; r++)
-                        {
-                            bool unc = va[u][r] > c.thr1 || vb[u][r] > 0.f || (KIND == CUTE_ANGULAR && q[u][r] < c.q_small);
-                            if (KIND == CUTE_ANGULAR && LOGB)   // the pair's own tau (q_mid > 0 only for log bins)
-                                unc = q[u][r] < c.q_small || va[u][r] > 0.5f - fmaf(c.tau_b, fast_rsqrt(fmaxf(q[u][r], 1.0e-30f)), c.tau_a);
-                            if (unc && q[u][r] < c.q_hi) need |= 1u << r;
-                        }
-                        if (need) push_refine<KIND>(p, s, need, ip.idx0, j0 + jj + u, hoff, refined_inline,
-                                                    make_uint4(addr[u][0], addr[u][1], addr[u][2], addr[u][3]), 1);
-                    }
-                }
+            }
+            if (flagged) {   // rare: queue the block for re-examination (process_entry)
+                const uint4 en = make_uint4(ip.idx0, j0 + jj, meta0 | (jj + 1u >= t_cnt ? 64u : 0u), i_last);
+                const uint32_t slot = atomicAdd(s.rq_count, 1u);
+                if (slot < (uint32_t)kRefineCap) s.rq[slot] = en;
+                else refined_inline += examine_overflow<KIND, MINIMG, LOGB, FLAGS>(p, s, c, en, lane);
             }
         }
     }
 }
 
 // ------------------------------------------------------------------------------- G4: neighbour schedule
-// Segment code: bits 0-1 / 2-3 / 4-5 = periodic image along x / y / z (0: none, 1: the i-points are one box length BELOW
-// the j-points, 2: above); bit 8: same cell row in an auto-correlation (count j > i only).
-// The image is applied by subtracting L from the LARGER coordinate, which is exact in float32 (Sterbenz: L/2 <= x <= 2L for a
-// point in the top cells of the box): code 2 shifts the i-points (registers, once per segment), code 1 shifts the j-points
-// (in the shared-memory tile, once per tile).  Adding L to the smaller coordinate would round at ulp(2L).
-__device__ __forceinline__ float image_shift_i(uint32_t code, int axis, float L)
-{
-    return ((code >> (2 * axis)) & 3u) == 2u ? -L : 0.f;
-}
-__device__ __forceinline__ float image_shift_j(uint32_t code, int axis, float L)
-{
-    return ((code >> (2 * axis)) & 3u) == 1u ? -L : 0.f;
-}
-
 // Lane `nb` expands neighbour row number nb of the chunk into <= 3 contiguous ranges of the
 // cell-sorted j array ("we only correlate C_i with the cells inside a cube of 2k+1 cells per side
 // around it", with k = ceil(Rmax/a) -- DESIGN.md reading G3; on the sphere the rows
@@ -756,7 +932,7 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
         for (uint32_t k = lane; k < ((uint32_t)p.nhist_pad << p.colshift); k += 32) s.hist[k] = 0;
     if (lane == 0) {
         for (int k = 0; k < kStages; k++) mbar_init(s.bar[k], 1);
-        *s.rq_count = 0;
+        *s.rq_count = 0; *s.pq_count = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
@@ -779,32 +955,13 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
         const Chunk ch = g1.chunks[c];
         const uint32_t i_last = ch.i_begin + ch.i_count - 1;
 
-        // ---- i-points into registers
+        // ---- i-points into registers; x-extent of the chunk (the j-ranges are trimmed to it)
         IPoints ip;
-        ip.idx0 = ch.i_begin + lane;
-        float bx[R], by[R], bz[R], bw[R], lw[R];
-#pragma unroll
-        for (int r = 0; r < R; r++) {
-            const uint32_t k = lane + 32 * r;
-            float4 h = make_float4(kSentinel, kSentinel, kSentinel, 0.f);
-            lw[r] = 0.f;
-            float wbits = 0.f;
-            if (k < ch.i_count) {
-                h = g1.hi[ch.i_begin + k];
-                if (NEEDLO) { const float4 l = g1.lo[ch.i_begin + k]; lw[r] = l.w; wbits = l.x; }
-            }
-            bx[r] = h.x; by[r] = h.y; bz[r] = h.z; bw[r] = h.w;
-            ip.w[r] = ((FLAGS & PK_WEIGHTED) && KIND != CUTE_ANGULAR) ? wbits : h.w;
-        }
-#pragma unroll
-        for (int h = 0; h < 2; h++) {
-            // (the packed pairs are BORN in an aligned register pair by a packed add of +0: ptxas otherwise keeps the scalars
-            // of the LDG.128 results and re-assembles every pair with two MOVs before each use inside the loop)
-            const f32x2 z2 = bc(0.f);
-            ip.X[h] = add2(pk(bx[2 * h], bx[2 * h + 1]), z2); ip.Y[h] = add2(pk(by[2 * h], by[2 * h + 1]), z2);
-            ip.Z[h] = add2(pk(bz[2 * h], bz[2 * h + 1]), z2);
-            ip.W[h] = add2(pk(bw[2 * h], bw[2 * h + 1]), z2);
-            ip.LW[h] = add2(pk(lw[2 * h], lw[2 * h + 1]), z2);
+        float xmin, xmax;
+        load_ipoints<KIND, FLAGS>(g1, ch.i_begin + lane, i_last, 0.f, 0.f, 0.f, ip, xmin, xmax);
+        for (int o = 16; o; o >>= 1) {
+            xmin = fminf(xmin, __shfl_xor_sync(0xffffffffu, xmin, o));
+            xmax = fmaxf(xmax, __shfl_xor_sync(0xffffffffu, xmax, o));
         }
 
         if ((FLAGS & PK_WEIGHTED) && p.is_auto && p.self_bin >= 0 && sp == 0) {
@@ -819,16 +976,6 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
             for (int o = 16; o; o >>= 1) self += __shfl_xor_sync(0xffffffffu, self, o);
             if (lane == 0 && self) atomicAdd(p.hist + p.self_bin, self);
         }
-        // x-extent of the chunk (the j-ranges are trimmed to it)
-        float xmin = 3.0e38f, xmax = -3.0e38f;
-#pragma unroll
-        for (int r = 0; r < R; r++)
-            if ((uint32_t)(lane + 32 * r) < ch.i_count) { xmin = fminf(xmin, bx[r]); xmax = fmaxf(xmax, bx[r]); }
-        for (int o = 16; o; o >>= 1) {
-            xmin = fminf(xmin, __shfl_xor_sync(0xffffffffu, xmin, o));
-            xmax = fmaxf(xmax, __shfl_xor_sync(0xffffffffu, xmax, o));
-        }
-
         // ---- neighbour rows, 32 at a time
         int nrows_nb = 1;
         if (p.mode == CUTE_GRID_BOX3D) nrows_nb = (2 * p.ky + 1) * (2 * p.kz + 1);
@@ -895,9 +1042,7 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
                         jsx = image_shift_j(code, 0, p.Lf); jsy = image_shift_j(code, 1, p.Lf); jsz = image_shift_j(code, 2, p.Lf);
 #pragma unroll
                         for (int h = 0; h < 2; h++) {
-                            ip.X[h] = pk(bx[2 * h] + sx, bx[2 * h + 1] + sx);
-                            ip.Y[h] = pk(by[2 * h] + sy, by[2 * h + 1] + sy);
-                            ip.Z[h] = pk(bz[2 * h] + sz, bz[2 * h + 1] + sz);
+                            ip.X[h] = add2(ip.X0[h], bc(sx)); ip.Y[h] = add2(ip.Y0[h], bc(sy)); ip.Z[h] = add2(ip.Z0[h], bc(sz));
                         }
                     }
                 }
@@ -918,9 +1063,9 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
                     }
                     __syncwarp();
                 }
-                const uint32_t t_cnt2 = (t_cnt + 1u) >> 1;
+                const uint32_t meta0 = (uint32_t)lane | ((s.segs[t_slot].z & 0x3fu) << 8);
                 if (seg_mask && t_j0 <= i_last) {
-                    compute_tile<KIND, MINIMG, LOGB, FLAGS, true>(p, s, cst, ip, th, tl, t_cnt2, t_j0, lane, refined_inline);
+                    compute_tile<KIND, MINIMG, LOGB, FLAGS, true>(p, s, cst, ip, th, tl, t_cnt, t_j0, meta0 | 32u, i_last, lane, refined_inline);
 #pragma unroll
                     for (int r = 0; r < R; r++) {
                         if (ip.idx0 + 32u * r <= i_last) {
@@ -929,14 +1074,14 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
                         }
                     }
                 } else {
-                    compute_tile<KIND, MINIMG, LOGB, FLAGS, false>(p, s, cst, ip, th, tl, t_cnt2, t_j0, lane, refined_inline);
+                    compute_tile<KIND, MINIMG, LOGB, FLAGS, false>(p, s, cst, ip, th, tl, t_cnt, t_j0, meta0, i_last, lane, refined_inline);
                     if (lane == 0) evaluated += (unsigned long long)ch.i_count * t_cnt;
                 }
                 __syncwarp();
-                if (*s.rq_count >= 32u) refined += drain_refine<KIND>(p, s, lane);
+                if (*s.rq_count >= 32u) refined += drain_flagged<KIND, MINIMG, LOGB, FLAGS>(p, s, cst, lane, false);
                 jepoch += t_cnt;
                 if (jepoch >= p.epoch_j) {
-                    refined += drain_refine<KIND>(p, s, lane);   // (an undone increment and its recount stay in one epoch)
+                    refined += drain_flagged<KIND, MINIMG, LOGB, FLAGS>(p, s, cst, lane, true);   // (a provisional increment and its correction stay in one epoch)
                     flush_hist(p, s, lane); flushes++; jepoch = 0;
                 }
                 stage ^= 1u;
@@ -945,11 +1090,11 @@ __global__ void __launch_bounds__(32 * kMaxWarps, 1) pair_kernel(const __grid_co
             if (p.mode == CUTE_GRID_NONE) break;
         }
         if (p.flush_items && (items % p.flush_items) == 0) {
-            refined += drain_refine<KIND>(p, s, lane);
+            refined += drain_flagged<KIND, MINIMG, LOGB, FLAGS>(p, s, cst, lane, true);
             flush_hist(p, s, lane); flushes++; jepoch = 0;
         }
     }
-    refined += drain_refine<KIND>(p, s, lane);
+    refined += drain_flagged<KIND, MINIMG, LOGB, FLAGS>(p, s, cst, lane, true);
     flush_hist(p, s, lane);
     flushes++;
     refined += refined_inline;
