@@ -8,10 +8,12 @@
 // Readings D1-D4: grid points = cell centres (g + 1/2) h; TSC = second-order B-spline per axis;
 // delta = rho / (N / ng^3) - 1; every ordered pair (g, g + v), v != 0 with the minimum image, r = h |v|, half-open bins.
 // Three kernels: TSC scatter (float64 atomics into the L2-resident grid; HBM-bound on the particle read),
-// overdensity (elementwise), and the offset-stencil correlation: the offsets are found, binned and sorted by bin ONCE on
-// the host; every thread owns one grid point and sweeps the offsets of a bin with one float64 accumulator, the block
-// reduces it and adds it to the bin's global sum.  All arithmetic float64 (the grid fits L2; this path is not the
-// float32 pair kernel), so the result differs from a serial float64 loop only by the order of the additions.
+// overdensity (elementwise), and the offset-stencil correlation.  The offsets are found and binned ONCE on the host.
+// k_grid_corr_rows (offsets of at most 16 cells per axis) treats each (vy, vz) as a 1-D cross-correlation of x-rows for all
+// vx at once, register-tiled, rows staged in shared memory by cp.async, half of the offsets swept (xi is even);
+// k_grid_corr (anything else) gives every thread one grid point and sweeps the offsets of a bin.
+// All arithmetic float64 (the grid fits L2; this path is not the float32 pair kernel), so the result differs from a
+// serial float64 loop only by the order of the additions.
 #include "cute_internal.h"
 #include <math.h>
 #include <vector>
@@ -111,6 +113,176 @@ __global__ void __launch_bounds__(kCorrThreads) k_grid_corr(const double *__rest
     }
 }
 
+// The fast stencil (offsets of at most 16 cells per axis).  xi(v) = <delta(g) delta(g + v)> is even in v, so only the
+// half-space vz > 0 | (vz = 0, vy > 0) | (vz = vy = 0, vx > 0) is swept and every sum counts twice.  A CTA owns one
+// (vy, vz) and a slab of z; a group of LPR lanes takes one x-row A = delta[gz][gy][.] and the shifted row
+// B = delta[gz+vz][gy+vy][.] at a time: B goes to shared memory with a circular halo of M cells, each lane keeps XT = 8
+// consecutive points of A in registers, reads its window of 8 + 2M points of B once (LDS.128) and feeds 8 (2M + 1) float64
+// multiply-adds into 2M + 1 register accumulators, one per vx -- a 1-D cross-correlation of the two rows for all lags at
+// once.  Row pairs reach shared memory by cp.async, three of them in flight per lane group while one is computed.
+constexpr int kXT = 8, kStagesDG = 4;
+template <int M>
+__global__ void __launch_bounds__(256, 1) k_grid_corr_rows(const double *__restrict__ delta, int ng, int m, const int2 *__restrict__ vyz,
+                                                           int zsplit, const int *__restrict__ binidx, double *sum_dd, int lpr_log2)
+{
+    constexpr int W = 2 * M + 1, WIN = kXT + 2 * M;
+    extern __shared__ __align__(16) double rows_sm[];
+    __shared__ double red[8][W];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int2 v = vyz[blockIdx.x / zsplit];
+    const int zs = blockIdx.x % zsplit;
+    const int zper = (ng + zsplit - 1) / zsplit, z0 = min(ng, zs * zper), z1 = min(ng, z0 + zper);
+    const int r0 = z0 * ng, r1 = z1 * ng;                  // rows (gz * ng + gy) of this slab
+    double acc[W];
+#pragma unroll
+    for (int k = 0; k < W; k++) acc[k] = 0.0;
+    auto stage_index = [&](int i) {                        // staged row: buf[i] = B[(i - M) mod ng]
+        int x = (i - M) % ng;
+        return x < 0 ? x + ng : x;
+    };
+
+    if (lpr_log2 >= 0) {
+        // ---- LPR lanes per row (kXT * LPR >= ng, ng a multiple of kXT), 32 / LPR rows per warp and trip:
+        //      register-resident, software-pipelined, no guards in the loop
+        const int LPR = 1 << lpr_log2, RPW = 32 >> lpr_log2;
+        const int sub = lane >> lpr_log2, lr = lane & (LPR - 1);
+        const int blen = ng + 2 * M;                       // (even: 16-byte aligned rows)
+        // 16-byte pieces are stored swizzled inside aligned groups of 8 (piece p at p ^ ((p >> 3) & 7)): the lanes of a
+        // quarter-warp read pieces 4 apart, which would otherwise share two bank groups (4-way conflicts, measured)
+        auto swz = [](int p) { return p ^ ((p >> 3) & 7); };
+        const int blen_pad = (blen + 15) & ~15, slot = blen_pad + ((ng + 15) & ~15);   // one staged row pair: B with its halo, then A
+        // B is staged in 16-byte pieces (M and ng are even, so a pair of slots never straddles the wrap): per lane
+        // ceil((ng + 2M) / 2 / LPR) <= kXT / 2 + ceil(M / 8) of them
+        constexpr int NST = kXT / 2 + (M + 7) / 8;
+        int xs[NST], xg[NST];                              // first slot of each piece this lane fills, and the x of B it holds
+#pragma unroll                                             // (the same for every row; pieces past the halo re-stage the last one)
+        for (int t = 0; t < NST; t++) { xs[t] = min(2 * (lr + LPR * t), blen - 2); xg[t] = stage_index(xs[t]); xs[t] = 2 * swz(xs[t] / 2); }
+        // the lane's window: pieces xa / 2 + j of B and of A, at their swizzled places (byte offsets inside a staged row pair)
+        uint32_t ob[WIN / 2], oa[kXT / 2];
+        const bool live = kXT * lr < ng;
+        const int xa = live ? kXT * lr : 0;
+#pragma unroll
+        for (int j = 0; j < WIN / 2; j++) ob[j] = 16u * (uint32_t)swz(xa / 2 + j);
+#pragma unroll
+        for (int k = 0; k < kXT / 2; k++) oa[k] = 8u * (uint32_t)blen_pad + 16u * (uint32_t)swz(xa / 2 + k);
+        // stage s of this lane's row group: rows_sm[((s * 8 + wid) * RPW + sub) * slot]
+        auto stage_ptr = [&](int st) { return rows_sm + (((size_t)st * 8 + wid) * RPW + sub) * slot; };
+        // rows r0 + wid * RPW + sub + 8 RPW it: (gz, gy) advanced without a division; the slab is a whole number of trips
+        int gz = z0, gy = wid * RPW + sub;
+        while (gy >= ng) { gy -= ng; gz++; }
+        auto issue = [&](int st) {                         // cp.async: the row pair goes to shared memory without passing registers
+            const int gzc = min(gz, ng - 1);               // (a row past the end of the slab is fetched and never used)
+            int hy = gy + v.x, hz = gzc + v.y;
+            hy += hy < 0 ? ng : (hy >= ng ? -ng : 0);
+            hz += hz < 0 ? ng : (hz >= ng ? -ng : 0);
+            const double *A = delta + ((size_t)gzc * ng + gy) * ng + xa, *B = delta + ((size_t)hz * ng + hy) * ng;
+            double *sb = stage_ptr(st);
+            const uint32_t sa = (uint32_t)__cvta_generic_to_shared(sb);
+#pragma unroll
+            for (int t = 0; t < NST; t++)
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(sa + 8u * (uint32_t)xs[t]), "l"(B + xg[t]) : "memory");
+#pragma unroll
+            for (int k = 0; k < kXT / 2; k++)
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(sa + oa[k]), "l"(A + 2 * k) : "memory");
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            gy += 8 * RPW;
+            while (gy >= ng) { gy -= ng; gz++; }
+        };
+        for (int st = 0; st < kStagesDG - 1; st++) issue(st);
+        const int ntrips = (r1 - r0) / (8 * RPW);
+        int st = 0;
+        for (int it = 0; it < ntrips; it++) {
+            issue((st + kStagesDG - 1) % kStagesDG);       // kStagesDG - 1 row pairs in flight while this one is computed
+            asm volatile("cp.async.wait_group %0;" ::"n"(kStagesDG - 1) : "memory");
+            __syncwarp();
+            const unsigned char *sb = reinterpret_cast<const unsigned char *>(stage_ptr(st));
+            double a[kXT], w[WIN];
+#pragma unroll
+            for (int k = 0; k < kXT / 2; k++) {
+                const double2 t = *reinterpret_cast<const double2 *>(sb + oa[k]);
+                a[2 * k] = live ? t.x : 0.0; a[2 * k + 1] = live ? t.y : 0.0;
+            }
+#pragma unroll
+            for (int j = 0; j < WIN / 2; j++) { const double2 t = *reinterpret_cast<const double2 *>(sb + ob[j]); w[2 * j] = t.x; w[2 * j + 1] = t.y; }
+#pragma unroll
+            for (int i = 0; i < kXT; i++)                  // (i outermost: 2M + 1 independent multiply-adds between dependent ones)
+#pragma unroll
+                for (int k = 0; k < W; k++) acc[k] = fma(a[i], w[i + k], acc[k]);
+            __syncwarp();
+            st = st + 1 == kStagesDG ? 0 : st + 1;
+        }
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+    } else {
+        // ---- any other row length: the same scheme with 4 points per lane, segment by segment, without the register pipeline
+        const int ngp = (ng + 3) & ~3, blen = ngp + 2 * M;
+        double *buf = rows_sm + (size_t)wid * blen;
+        for (int r = r0 + wid; r < r1; r += 8) {
+            const int gz = r / ng, gy = r - gz * ng;
+            int hy = gy + v.x, hz = gz + v.y;
+            hy += hy < 0 ? ng : (hy >= ng ? -ng : 0);
+            hz += hz < 0 ? ng : (hz >= ng ? -ng : 0);
+            const double *A = delta + ((size_t)gz * ng + gy) * ng, *B = delta + ((size_t)hz * ng + hy) * ng;
+            for (int i = lane; i < blen; i += 32) buf[i] = i < ng + 2 * M ? B[stage_index(i)] : 0.0;
+            __syncwarp();
+            for (int x0 = 4 * lane; x0 < ngp; x0 += 128) {
+                double a[4], w[4 + 2 * M];
+#pragma unroll
+                for (int k = 0; k < 4; k++) a[k] = (x0 + k < ng) ? A[x0 + k] : 0.0;
+                const double2 *b2 = reinterpret_cast<const double2 *>(buf + x0);
+#pragma unroll
+                for (int j = 0; j < 2 + M; j++) { const double2 t = b2[j]; w[2 * j] = t.x; w[2 * j + 1] = t.y; }
+#pragma unroll
+                for (int i = 0; i < 4; i++)
+#pragma unroll
+                    for (int k = 0; k < W; k++) acc[k] = fma(a[i], w[i + k], acc[k]);
+            }
+            __syncwarp();
+        }
+    }
+    // ---- reduce the accumulators over the CTA and add them to their bins (acc[k]: vx = k - M)
+#pragma unroll
+    for (int k = 0; k < W; k++) {
+        double t = acc[k];
+        for (int o = 16; o; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        if (lane == 0) red[wid][k] = t;
+    }
+    __syncthreads();
+    if (threadIdx.x < W) {
+        const int vx = (int)threadIdx.x - M, Wm = 2 * m + 1;
+        const bool half = v.y > 0 || v.x > 0 || vx > 0;    // the mirrored offset is met through this one
+        if (abs(vx) <= m && half) {
+            const int bin = binidx[((v.y + m) * Wm + (v.x + m)) * Wm + (vx + m)];
+            if (bin >= 0) {
+                double t = 0.0;
+                for (int w8 = 0; w8 < 8; w8++) t += red[w8][threadIdx.x];
+                atomicAdd(&sum_dd[bin], 2.0 * t);
+            }
+        }
+    }
+}
+
+template <int M>
+static cudaError_t launch_rows(const double *delta, int ng, int m, const int2 *vyz, int npairs, const int *binidx, double *sum_dd, cudaStream_t s)
+{
+    int zsplit = (8 * 148 + npairs - 1) / npairs;
+    zsplit = zsplit < 1 ? 1 : (zsplit > ng ? ng : zsplit);
+    // fast path: ng a multiple of 8, at most 256, and every slab a whole number of trips of 8 warps x (32 / LPR) rows
+    int lpr_log2 = -1;
+    if (ng % kXT == 0 && ng <= 32 * kXT && ng > 4 * kXT) {   // (8, 16 or 32 lanes per row: the staging below assumes >= 8)
+        int l2 = 0;
+        while ((kXT << l2) < ng) l2++;
+        const int trip = 8 * (32 >> l2);
+        while (zsplit > 1 && (ng % zsplit != 0 || ((ng / zsplit) * ng) % trip != 0)) zsplit--;
+        if (ng % zsplit == 0 && ((ng / zsplit) * ng) % trip == 0) lpr_log2 = l2;
+    }
+    const size_t smem = lpr_log2 >= 0 ? (size_t)kStagesDG * 8 * (size_t)(32 >> lpr_log2) * ((size_t)((ng + 2 * M + 15) & ~15) + (size_t)((ng + 15) & ~15)) * sizeof(double)
+                                      : (size_t)8 * ((size_t)((ng + 3) & ~3) + 2 * M) * sizeof(double);
+    cudaError_t e = cudaFuncSetAttribute(k_grid_corr_rows<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_grid_corr_rows<M><<<npairs * zsplit, 256, smem, s>>>(delta, ng, m, vyz, zsplit, binidx, sum_dd, lpr_log2);
+    return cudaGetLastError();
+}
+
 // host: the offsets of Eq. 17 and their bins, once
 static int find_bin_host(const std::vector<double> &e, int n, double lo, double hi, int lg, double v)
 {
@@ -195,12 +367,34 @@ int cute_density_grid_xi(const cute_catalog *cat, double L, int ng, const cute_b
     if (cudaMemsetAsync(d_status, 0, 256, s) != cudaSuccess || cudaMemsetAsync(rho, 0, ng3 * 8, s) != cudaSuccess ||
         cudaMemsetAsync(d_sum, 0, (size_t)nb * 8, s) != cudaSuccess)
         return CUTE_ERR_CUDA;
-    if (!offs.empty() && cudaMemcpyAsync(d_offs, offs.data(), offs.size() * 16, cudaMemcpyHostToDevice, s) != cudaSuccess) return CUTE_ERR_CUDA;
+    const bool fast = m <= 16 && m >= 1 && (size_t)8 * (((ng + 3) & ~3) + 32) * 8 <= 200 * 1024;
+    if (!offs.empty() && !fast && cudaMemcpyAsync(d_offs, offs.data(), offs.size() * 16, cudaMemcpyHostToDevice, s) != cudaSuccess) return CUTE_ERR_CUDA;
     if (cudaMemcpyAsync(d_bstart, bstart.data(), bstart.size() * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) return CUTE_ERR_CUDA;
     k_tsc<<<(unsigned)((cat->n + 255) / 256), 256, 0, s>>>(cat->c0, cat->c1, cat->c2, cat->dtype, cat->n, (double)ng / L, ng, rho, d_status);
     k_overdensity<<<(unsigned)((ng3 + 255) / 256), 256, 0, s>>>(rho, (int64_t)ng3, (double)ng3 / (double)cat->n);
     if (d_delta && cudaMemcpyAsync(d_delta, rho, ng3 * 8, cudaMemcpyDeviceToDevice, s) != cudaSuccess) return CUTE_ERR_CUDA;
-    if (!offs.empty()) k_grid_corr<<<(unsigned)((ng3 + kCorrThreads - 1) / kCorrThreads), kCorrThreads, 0, s>>>(rho, ng, d_offs, d_bstart, nb, d_sum);
+    if (!offs.empty() && fast) {
+        // fast stencil: the table offset -> bin and the list of (vy, vz) of the half-space live where the sorted offsets were
+        const int Wm = 2 * m + 1;
+        std::vector<int> binidx((size_t)Wm * Wm * Wm, -1);
+        for (const int4 &o : offs) binidx[((size_t)(o.z + m) * Wm + (size_t)(o.y + m)) * Wm + (size_t)(o.x + m)] = o.w;
+        std::vector<int2> vyz;
+        for (int vz = 0; vz <= m; vz++)
+            for (int vy = (vz == 0 ? 0 : -m); vy <= m; vy++) vyz.push_back(make_int2(vy, vz));
+        int *d_binidx = (int *)d_offs;
+        int2 *d_vyz = (int2 *)((unsigned char *)d_offs + dg_align(binidx.size() * 4));
+        if (cudaMemcpyAsync(d_binidx, binidx.data(), binidx.size() * 4, cudaMemcpyHostToDevice, s) != cudaSuccess ||
+            cudaMemcpyAsync(d_vyz, vyz.data(), vyz.size() * 8, cudaMemcpyHostToDevice, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
+            return CUTE_ERR_CUDA;   // (the host vectors go out of scope below: the copies must have left them)
+        cudaError_t e;
+        const int np = (int)vyz.size();
+        if (m <= 4) e = launch_rows<4>(rho, ng, m, d_vyz, np, d_binidx, d_sum, s);
+        else if (m <= 8) e = launch_rows<8>(rho, ng, m, d_vyz, np, d_binidx, d_sum, s);
+        else if (m <= 12) e = launch_rows<12>(rho, ng, m, d_vyz, np, d_binidx, d_sum, s);
+        else e = launch_rows<16>(rho, ng, m, d_vyz, np, d_binidx, d_sum, s);
+        if (e != cudaSuccess) return CUTE_ERR_CUDA;
+    } else if (!offs.empty())
+        k_grid_corr<<<(unsigned)((ng3 + kCorrThreads - 1) / kCorrThreads), kCorrThreads, 0, s>>>(rho, ng, d_offs, d_bstart, nb, d_sum);
     note_launches(3);
     if (cudaGetLastError() != cudaSuccess) return CUTE_ERR_CUDA;
     std::vector<double> sums((size_t)nb);

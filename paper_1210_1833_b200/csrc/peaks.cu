@@ -14,6 +14,7 @@ enum PeakOp {
     P_ATOMS_INC_M1, P_ATOMS_INC_M2, P_ATOMS_INC_M4, P_ATOMS_INC_M8, P_ATOMS_INC_M32, P_ATOMS_ADD_M1,
     P_ATOMS_COLS8, P_ATOMS_COLS32, P_LDS128_BCAST,
     P_MIX_FFMA_FMNMX, P_MIX_FFMA2_FMNMX, P_MIX_FFMA2_MUFU_FMNMX, P_MIX_FFMA_IADD, P_MIX_FFMA2_FFMA,
+    P_DFMA,      // float64 multiply-add: the density-grid stencil's roofline (density_grid.cu)
     P_COUNT
 };
 
@@ -22,7 +23,8 @@ static const char *kPeakNames[P_COUNT] = {
     "mufu_sqrt", "mufu_lg2", "mufu_rsq",
     "atoms_inc_same1", "atoms_inc_same2", "atoms_inc_same4", "atoms_inc_same8", "atoms_inc_same32", "atoms_add_same1",
     "atoms_inc_cols8_random_bins", "atoms_inc_cols32_random_bins", "lds128_broadcast",
-    "mix_ffma+fmnmx", "mix_ffma2+fmnmx", "mix_2ffma2+mufu+fmnmx", "mix_ffma+iadd", "mix_ffma2+ffma"
+    "mix_ffma+fmnmx", "mix_ffma2+fmnmx", "mix_2ffma2+mufu+fmnmx", "mix_ffma+iadd", "mix_ffma2+ffma",
+    "dfma"
 };
 
 constexpr int kPeakThreads = 512;
@@ -58,6 +60,8 @@ __global__ void __launch_bounds__(kPeakThreads, 1) k_peak(unsigned long long *cy
     float a[kChains];
     unsigned long long a2[kChains];
     uint32_t u[kChains];
+    double d[kChains];
+    const double db = 1.0 + 1e-9 * (double)threadIdx.x, dc = 1e-12 * (double)(threadIdx.x & 31);
     const float b = 1.0f + 1e-7f * (float)threadIdx.x, c = 1e-9f * (float)lane;
     unsigned long long b2, c2;
     asm volatile("mov.b64 %0, {%1, %1};" : "=l"(b2) : "f"(b));
@@ -67,6 +71,7 @@ __global__ void __launch_bounds__(kPeakThreads, 1) k_peak(unsigned long long *cy
         a[k] = 1.0f + 0.01f * (float)(k + lane);
         asm volatile("mov.b64 %0, {%1, %1};" : "=l"(a2[k]) : "f"(a[k]));
         u[k] = (uint32_t)(k * 7 + threadIdx.x);
+        d[k] = 1.0 + 0.01 * (double)(k + lane);
     }
     // shared-atomic address patterns
     uint32_t base = (uint32_t)__cvta_generic_to_shared(sh);
@@ -87,6 +92,7 @@ __global__ void __launch_bounds__(kPeakThreads, 1) k_peak(unsigned long long *cy
 #pragma unroll
         for (int k = 0; k < kChains; k++) {
             if (OP == P_FFMA) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(a[k]) : "f"(b), "f"(c));
+            else if (OP == P_DFMA) asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(d[k]) : "d"(db), "d"(dc));
             else if (OP == P_FADD) asm volatile("add.rn.f32 %0, %0, %1;" : "+f"(a[k]) : "f"(c));
             else if (OP == P_FFMA2) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(a2[k]) : "l"(b2), "l"(c2));
             else if (OP == P_FADD2) asm volatile("add.rn.f32x2 %0, %0, %1;" : "+l"(a2[k]) : "l"(c2));
@@ -134,7 +140,7 @@ __global__ void __launch_bounds__(kPeakThreads, 1) k_peak(unsigned long long *cy
     atomicMax(&tmax, (unsigned long long)(t1 - t0));
     float s = 0.f;
 #pragma unroll
-    for (int k = 0; k < kChains; k++) s += a[k] + (float)(a2[k] & 0xffu) + (float)(u[k] & 0xffu);
+    for (int k = 0; k < kChains; k++) s += a[k] + (float)(a2[k] & 0xffu) + (float)(u[k] & 0xffu) + (float)d[k];
     __syncthreads();
     if (threadIdx.x == 0) cyc[blockIdx.x] = tmax;
     if (s == 12345.678f) sink[threadIdx.x] = s + (float)sh[lane];   // never true: keeps the chains alive

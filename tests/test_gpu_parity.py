@@ -633,6 +633,14 @@ def test_density_grid_monopole(rt, oracle, dtype):
         assert (out["status"] == api.WARN_EMPTY_BIN) == (orc["empty"] > 0)
     # mass conservation on the device: <delta> = 0
     assert abs(float(out["delta"].mean())) < 1e-12
+    # grids whose rows are whole 8-point lane segments take the register-tiled stencil (16, 8 and 4 lanes per row)
+    for ng2, hi in ((64, 30.0), (32, 40.0), (128, 10.0)):
+        bins = dict(n1=10, lo1=0.0, hi1=hi)
+        out = api.cute_density_grid_xi(cols, L, ng2, bins)
+        orc = oracle.density_grid_xi(tuple(np.asarray(c, dtype=np.float64) for c in x), L, ng2, bins)
+        assert np.array_equal(out["npairs"], orc["npairs"])
+        var = float((orc["delta"] ** 2).mean())
+        assert np.max(np.abs(out["xi"] - orc["xi"])) < 1e-10 * max(1.0, var)
     # validation: r_max beyond L/2, a non-xyz catalogue
     with pytest.raises(api.CuteError):
         api.cute_density_grid_xi(cols, L, ng, dict(n1=4, lo1=0.0, hi1=120.0))
