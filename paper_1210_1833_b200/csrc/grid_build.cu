@@ -421,6 +421,31 @@ __global__ void __launch_bounds__(512) k_part_scatter(BuildPlan b, const uint32_
     }
 }
 
+// 1-D TMA bulk copy global -> shared with an mbarrier (the bucket's records reach shared memory in one instruction,
+// issued by one thread: per-thread loads of ~10 records each would expose their latency one after the other)
+__device__ __forceinline__ void fine_stage_bulk(void *dst, const void *src, uint32_t bytes, unsigned long long *bar)
+{
+    const uint32_t b = (uint32_t)__cvta_generic_to_shared(bar), d = (uint32_t)__cvta_generic_to_shared(dst);
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(b) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(b), "r"(bytes) : "memory");
+        const uint32_t piece = 1u << 16;                       // pieces of 64 KB
+        for (uint32_t o = 0; o < bytes; o += piece) {
+            const uint32_t n = bytes - o < piece ? bytes - o : piece;
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(d + o), "l"(reinterpret_cast<const unsigned char *>(src) + o), "r"(n), "r"(b) : "memory");
+        }
+    }
+    __syncthreads();                                           // the barrier is initialised before anybody polls it
+    uint32_t ok;
+    do {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\nselp.u32 %0, 1, 0, p;\n}\n"
+                     : "=r"(ok) : "r"(b) : "memory");
+    } while (!ok);
+}
+
 template <bool F32REC>
 __device__ __forceinline__ void load_rec(const BuildPlan &b, uint32_t s, double &a, double &c1, double &c2, uint32_t &idx, uint32_t &cell)
 {
@@ -454,24 +479,20 @@ __global__ void __launch_bounds__(1024) k_part_fine(BuildPlan b, const uint32_t 
     for (int k = threadIdx.x; k < nc; k += T) cnt[k] = 0;
     __syncthreads();
     if (staged) {
+        __shared__ unsigned long long stage_bar;
         if (F32REC) {
-            const float4 *src = reinterpret_cast<const float4 *>(b.part_tmp) + bs;
-            float4 *dst = reinterpret_cast<float4 *>(stage);
+            if (be > bs) fine_stage_bulk(stage, reinterpret_cast<const float4 *>(b.part_tmp) + bs, (be - bs) * 16u, &stage_bar);
+            const float4 *dst = reinterpret_cast<const float4 *>(stage);
             for (uint32_t s = threadIdx.x; s < be - bs; s += T) {
-                const float4 r = src[s];
-                dst[s] = r;
+                const float4 r = dst[s];
                 uint32_t id;
                 cell_of_t<CUTE_GRID_BOX3D>(b, (double)r.x, (double)r.y, (double)r.z, id);
                 atomicAdd(&cnt[id - (uint32_t)c0], 1u);
             }
         } else {
-            const Rec32 *src = reinterpret_cast<const Rec32 *>(b.part_tmp) + bs;
-            Rec32 *dst = reinterpret_cast<Rec32 *>(stage);
-            for (uint32_t s = threadIdx.x; s < be - bs; s += T) {
-                const Rec32 r = src[s];
-                dst[s] = r;
-                atomicAdd(&cnt[r.cell - (uint32_t)c0], 1u);
-            }
+            if (be > bs) fine_stage_bulk(stage, reinterpret_cast<const Rec32 *>(b.part_tmp) + bs, (be - bs) * 32u, &stage_bar);
+            const Rec32 *dst = reinterpret_cast<const Rec32 *>(stage);
+            for (uint32_t s = threadIdx.x; s < be - bs; s += T) atomicAdd(&cnt[dst[s].cell - (uint32_t)c0], 1u);
         }
     } else {
         for (uint32_t s = bs + threadIdx.x; s < be; s += T) {
