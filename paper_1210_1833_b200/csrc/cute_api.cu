@@ -892,7 +892,7 @@ static int count_impl(int kind, const cute_grid *g1, const cute_grid *g2, const 
         // all warps feed one counter, and each of them may overshoot its share by one tile before it checks
         if (p.weighted) {
             const uint64_t per_j = 128ull * g1->wmax * g2->wmax;
-            const uint64_t e = 0x7fffffffull / per_j;   // (the shared copy is read as a signed 32-bit number: undone increments)
+            const uint64_t e = 0x7fffffffull / per_j;   // (the shared copy is read as a signed 32-bit number: moved counts)
             if (e < (uint64_t)kTile * (uint64_t)p.warps + (uint64_t)p.warps) return CUTE_ERR_OVERFLOW;
             const uint64_t share = (e - (uint64_t)kTile * (uint64_t)p.warps) / (uint64_t)p.warps;
             p.epoch_j = (uint32_t)(share < (uint64_t)p.epoch_j ? share : (uint64_t)p.epoch_j);

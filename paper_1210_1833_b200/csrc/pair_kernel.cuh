@@ -26,9 +26,10 @@
 //  * bin map without division or compare chains: t = S*g(q) + O - 1/2 with g = MUFU sqrt or log2; ONE
 //    round-to-nearest add of 1.5*2^23 leaves floor(t + 1/2) in the mantissa, and d = t - rint(t) is the
 //    distance of the pair from the centre of its bin in units of bins.  The float32 bin is certain iff
-//    |d| <= 1/2 - tau (tau = a proven bound on the float32 error); otherwise the provisional increment is
-//    undone and the pair is queued and recomputed in float64 (the definition), so the histogram equals
-//    the float64 definition except at float64-rounding distance of an edge.
+//    |d| <= 1/2 - tau (tau = a proven bound on the float32 error); otherwise the lane queues its BLOCK of
+//    pairs, the warp re-examines queued blocks 32 at a time, recomputes their uncertain pairs in float64 (the
+//    definition) and moves a provisional count whose float64 cell differs ("the rare path" below), so the
+//    histogram equals the float64 definition except at float64-rounding distance of an edge.
 //  * histogram: per-warp private uint32 copies in shared memory, [bin][column] (8 columns per warp;
 //    a 2-D histogram too large for that is kept once per CTA), with one row (2-D: a border) of dump
 //    cells on either side: out-of-range pairs are CLAMPED into the border instead of being predicated
@@ -297,9 +298,9 @@ __device__ __forceinline__ void flush_hist(const PairParams &p, const WarpSmem &
         }
         // border cells hold the clamped out-of-range pairs: dropped
         const bool real = k1p >= 1u && k1p <= (uint32_t)p.n1 && k2p >= 1u && (p.n2 == 0 || k2p <= (uint32_t)p.n2);
-        // a private copy can hold an undone increment of another column as 2^32 - 1: the sum is taken modulo 2^32
+        // a column can hold a count moved away before it arrived as 2^32 - 1: the sum over the columns is taken modulo 2^32
         if (!p.hist_shared) sum &= 0xffffffffull;
-        else sum = (unsigned long long)(long long)(int)(uint32_t)sum;   // shared copy: an undo may follow another warp's flush
+        else sum = (unsigned long long)(long long)(int)(uint32_t)sum;   // shared copy: a moved count may follow another warp's flush
         if (real && sum) atomicAdd(p.hist + ((k1p - 1u) * (uint32_t)p.n2eff + (p.n2 > 0 ? k2p - 1u : 0u)), sum);
     }
     __syncwarp();
