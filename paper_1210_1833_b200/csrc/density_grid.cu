@@ -147,16 +147,28 @@ __global__ void __launch_bounds__(256, 1) k_grid_corr_rows(const double *__restr
         const int LPR = 1 << lpr_log2, RPW = 32 >> lpr_log2;
         const int sub = lane >> lpr_log2, lr = lane & (LPR - 1);
         const int blen = ng + 2 * M;                       // (even: 16-byte aligned rows)
-        // 16-byte pieces are stored swizzled inside aligned groups of 8 (piece p at p ^ ((p >> 3) & 7)): the lanes of a
-        // quarter-warp read pieces 4 apart, which would otherwise share two bank groups (4-way conflicts, measured)
-        auto swz = [](int p) { return p ^ ((p >> 3) & 7); };
+        // 16-byte pieces are stored swizzled inside aligned groups of 8 (piece p at p ^ ((p >> 3) & 3)): the lanes of a
+        // quarter-warp read pieces 4 apart, which would otherwise share two bank groups (4-way conflicts, measured).  This
+        // mask makes the eight reads p = 4 lane + j conflict-free for every j (checked by enumeration; & 7 left half of them
+        // 2-way), and keeps eight consecutive pieces -- what a copy instruction writes -- on eight bank groups.
+        auto swz = [](int p) { return p ^ ((p >> 3) & 3); };
         const int blen_pad = (blen + 15) & ~15, slot = blen_pad + ((ng + 15) & ~15);   // one staged row pair: B with its halo, then A
         // B is staged in 16-byte pieces (M and ng are even, so a pair of slots never straddles the wrap): per lane
         // ceil((ng + 2M) / 2 / LPR) <= kXT / 2 + ceil(M / 8) of them
         constexpr int NST = kXT / 2 + (M + 7) / 8;
+        // The lanes of a row group copy CONSECUTIVE pieces (lr, lr + LPR, ...) of B and of A: a cp.async writes shared memory
+        // one wavefront per global line it receives, so lanes 64 bytes apart in global memory (each copying its own 8
+        // points of A) cost 4x the wavefronts (measured); a piece past the end is not copied at all.
         int xs[NST], xg[NST];                              // first slot of each piece this lane fills, and the x of B it holds
-#pragma unroll                                             // (the same for every row; pieces past the halo re-stage the last one)
-        for (int t = 0; t < NST; t++) { xs[t] = min(2 * (lr + LPR * t), blen - 2); xg[t] = stage_index(xs[t]); xs[t] = 2 * swz(xs[t] / 2); }
+        uint32_t bmask = 0, amask = 0;                     // which of its pieces exist
+#pragma unroll                                             // (the same for every row)
+        for (int t = 0; t < NST; t++) {
+            const int pc = lr + LPR * t;
+            if (2 * pc < blen) bmask |= 1u << t;
+            xs[t] = min(2 * pc, blen - 2); xg[t] = stage_index(xs[t]); xs[t] = 2 * swz(xs[t] / 2);
+        }
+        uint32_t sa_off[kXT / 2];                          // A: byte offset of piece lr + LPR t inside the staged row pair
+        int ga_off[kXT / 2];                               //    and the x it starts at
         // the lane's window: pieces xa / 2 + j of B and of A, at their swizzled places (byte offsets inside a staged row pair)
         uint32_t ob[WIN / 2], oa[kXT / 2];
         const bool live = kXT * lr < ng;
@@ -164,7 +176,13 @@ __global__ void __launch_bounds__(256, 1) k_grid_corr_rows(const double *__restr
 #pragma unroll
         for (int j = 0; j < WIN / 2; j++) ob[j] = 16u * (uint32_t)swz(xa / 2 + j);
 #pragma unroll
-        for (int k = 0; k < kXT / 2; k++) oa[k] = 8u * (uint32_t)blen_pad + 16u * (uint32_t)swz(xa / 2 + k);
+        for (int k = 0; k < kXT / 2; k++) {
+            oa[k] = 8u * (uint32_t)blen_pad + 16u * (uint32_t)swz(xa / 2 + k);
+            const int pc = lr + LPR * k;
+            if (2 * pc < ng) amask |= 1u << k;
+            ga_off[k] = min(2 * pc, ng - 2);
+            sa_off[k] = 8u * (uint32_t)blen_pad + 16u * (uint32_t)swz(ga_off[k] / 2);
+        }
         // stage s of this lane's row group: rows_sm[((s * 8 + wid) * RPW + sub) * slot]
         auto stage_ptr = [&](int st) { return rows_sm + (((size_t)st * 8 + wid) * RPW + sub) * slot; };
         // rows r0 + wid * RPW + sub + 8 RPW it: (gz, gy) advanced without a division; the slab is a whole number of trips
@@ -175,15 +193,17 @@ __global__ void __launch_bounds__(256, 1) k_grid_corr_rows(const double *__restr
             int hy = gy + v.x, hz = gzc + v.y;
             hy += hy < 0 ? ng : (hy >= ng ? -ng : 0);
             hz += hz < 0 ? ng : (hz >= ng ? -ng : 0);
-            const double *A = delta + ((size_t)gzc * ng + gy) * ng + xa, *B = delta + ((size_t)hz * ng + hy) * ng;
+            const double *A = delta + ((size_t)gzc * ng + gy) * ng, *B = delta + ((size_t)hz * ng + hy) * ng;
             double *sb = stage_ptr(st);
             const uint32_t sa = (uint32_t)__cvta_generic_to_shared(sb);
 #pragma unroll
             for (int t = 0; t < NST; t++)
-                asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(sa + 8u * (uint32_t)xs[t]), "l"(B + xg[t]) : "memory");
+                if (bmask & (1u << t))
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(sa + 8u * (uint32_t)xs[t]), "l"(B + xg[t]) : "memory");
 #pragma unroll
             for (int k = 0; k < kXT / 2; k++)
-                asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(sa + oa[k]), "l"(A + 2 * k) : "memory");
+                if (amask & (1u << k))
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(sa + sa_off[k]), "l"(A + ga_off[k]) : "memory");
             asm volatile("cp.async.commit_group;" ::: "memory");
             gy += 8 * RPW;
             while (gy >= ng) { gy -= ng; gz++; }
