@@ -282,9 +282,10 @@ __global__ void __launch_bounds__(256, 1) k_grid_corr_rows(const double *__restr
 }
 
 template <int M>
-static cudaError_t launch_rows(const double *delta, int ng, int m, const int2 *vyz, int npairs, const int *binidx, double *sum_dd, cudaStream_t s)
+static cudaError_t launch_rows(const double *delta, int ng, int m, const int2 *vyz, int npairs, int npairs_all, const int *binidx, double *sum_dd,
+                               cudaStream_t s)
 {
-    int zsplit = (8 * 148 + npairs - 1) / npairs;
+    int zsplit = (8 * 148 + npairs_all - 1) / npairs_all;   // (the launches of the classes run back to back: size the slabs for all of them)
     zsplit = zsplit < 1 ? 1 : (zsplit > ng ? ng : zsplit);
     // fast path: ng a multiple of 8, at most 256, and every slab a whole number of trips of 8 warps x (32 / LPR) rows
     int lpr_log2 = -1;
@@ -398,24 +399,44 @@ int cute_density_grid_xi(const cute_catalog *cat, double L, int ng, const cute_b
         const int Wm = 2 * m + 1;
         std::vector<int> binidx((size_t)Wm * Wm * Wm, -1);
         for (const int4 &o : offs) binidx[((size_t)(o.z + m) * Wm + (size_t)(o.y + m)) * Wm + (size_t)(o.x + m)] = o.w;
-        std::vector<int2> vyz;
+        // (vy, vz) of the half-space, grouped by the largest |vx| that still falls in a bin: a pair outside the sphere of
+        // radius r_max is not swept at all, one near its rim sweeps 9 or 17 lags instead of 2m + 1
+        std::vector<int2> vyz[4];
         for (int vz = 0; vz <= m; vz++)
-            for (int vy = (vz == 0 ? 0 : -m); vy <= m; vy++) vyz.push_back(make_int2(vy, vz));
+            for (int vy = (vz == 0 ? 0 : -m); vy <= m; vy++) {
+                int mx = -1;
+                for (int vx = -m; vx <= m; vx++)
+                    if (binidx[((size_t)(vz + m) * Wm + (size_t)(vy + m)) * Wm + (size_t)(vx + m)] >= 0 && abs(vx) > mx) mx = abs(vx);
+                if (mx < 0) continue;
+                vyz[mx <= 4 ? 0 : mx <= 8 ? 1 : mx <= 12 ? 2 : 3].push_back(make_int2(vy, vz));
+            }
+        std::vector<int2> all;
+        int first[5] = {0, 0, 0, 0, 0};
+        for (int c = 0; c < 4; c++) { all.insert(all.end(), vyz[c].begin(), vyz[c].end()); first[c + 1] = (int)all.size(); }
         int *d_binidx = (int *)d_offs;
         int2 *d_vyz = (int2 *)((unsigned char *)d_offs + dg_align(binidx.size() * 4));
         if (cudaMemcpyAsync(d_binidx, binidx.data(), binidx.size() * 4, cudaMemcpyHostToDevice, s) != cudaSuccess ||
-            cudaMemcpyAsync(d_vyz, vyz.data(), vyz.size() * 8, cudaMemcpyHostToDevice, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
+            (!all.empty() && cudaMemcpyAsync(d_vyz, all.data(), all.size() * 8, cudaMemcpyHostToDevice, s) != cudaSuccess) ||
+            cudaStreamSynchronize(s) != cudaSuccess)
             return CUTE_ERR_CUDA;   // (the host vectors go out of scope below: the copies must have left them)
-        cudaError_t e;
-        const int np = (int)vyz.size();
-        if (m <= 4) e = launch_rows<4>(rho, ng, m, d_vyz, np, d_binidx, d_sum, s);
-        else if (m <= 8) e = launch_rows<8>(rho, ng, m, d_vyz, np, d_binidx, d_sum, s);
-        else if (m <= 12) e = launch_rows<12>(rho, ng, m, d_vyz, np, d_binidx, d_sum, s);
-        else e = launch_rows<16>(rho, ng, m, d_vyz, np, d_binidx, d_sum, s);
+        cudaError_t e = cudaSuccess;
+        const int total = (int)all.size();
+        for (int c = 0; c < 4 && e == cudaSuccess; c++) {
+            const int np = first[c + 1] - first[c];
+            if (np == 0) continue;
+            const int2 *pl = d_vyz + first[c];
+            if (c == 0) e = launch_rows<4>(rho, ng, m, pl, np, total, d_binidx, d_sum, s);
+            else if (c == 1) e = launch_rows<8>(rho, ng, m, pl, np, total, d_binidx, d_sum, s);
+            else if (c == 2) e = launch_rows<12>(rho, ng, m, pl, np, total, d_binidx, d_sum, s);
+            else e = launch_rows<16>(rho, ng, m, pl, np, total, d_binidx, d_sum, s);
+            note_launches(1);
+        }
         if (e != cudaSuccess) return CUTE_ERR_CUDA;
-    } else if (!offs.empty())
+    } else if (!offs.empty()) {
         k_grid_corr<<<(unsigned)((ng3 + kCorrThreads - 1) / kCorrThreads), kCorrThreads, 0, s>>>(rho, ng, d_offs, d_bstart, nb, d_sum);
-    note_launches(3);
+        note_launches(1);
+    }
+    note_launches(2);   // k_tsc, k_overdensity
     if (cudaGetLastError() != cudaSuccess) return CUTE_ERR_CUDA;
     std::vector<double> sums((size_t)nb);
     uint32_t st = 0;
