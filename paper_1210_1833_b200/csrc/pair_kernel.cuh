@@ -787,10 +787,10 @@ __device__ __forceinline__ void compute_tile(const PairParams &p, const WarpSmem
     const uint32_t hoff = (uint32_t)lane & ((1u << cs) - 1u);
     const uint32_t hb = hist_base<KIND>(s, c, hoff, sh);
     const uint32_t cnt2 = (t_cnt + 1u) >> 1;
-    // Measured (C5): reading the NEXT block's j-points before this block's guarded bin path and four copies of the body
-    // are worth 4 % on the short monopole body and cost as much on the longer angular / r-mu bodies (registers).
-    constexpr bool PREFETCH = KIND == 1 /* CUTE_MONOPOLE */ && !WEIGHTED;
-    constexpr int kUnroll = PREFETCH ? 4 : 2;
+    // Measured: reading the NEXT block's j-points before this block's guarded bin path is worth 4 % on the short monopole body
+    // (with four copies of the body, C5) and 1 % on the angular one (two copies, C2); it costs 8 % on the r-mu body (registers).
+    constexpr bool PREFETCH = (KIND == 1 /* CUTE_MONOPOLE */ || KIND == 0 /* CUTE_ANGULAR */) && !WEIGHTED;
+    constexpr int kUnroll = KIND == 1 ? 4 : 2;
     float4 nx[2];
     if (PREFETCH) { nx[0] = th[0]; nx[1] = th[1]; }
 #pragma unroll kUnroll
