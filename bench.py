@@ -148,7 +148,7 @@ def run_reference(args, w, cfg):
 ALG = {
     "angular": dict(all=7.0, bin=15.0, fp_all=6.0, fp_bin=8.0, mufu=1.0, atom=1.0),    # 3 FADD + FMUL + 2 FFMA + range | cubic (3) + FMUL + LG2 + FFMA + 3 (rint, frac) + 2 clamps + test + address + increment
     "monopole": dict(all=7.0, bin=9.0, fp_all=6.0, fp_bin=4.0, mufu=1.0, atom=1.0),    # 3 FADD + FMUL + 2 FFMA + range | SQRT + FFMA + 3 (rint, frac) + clamp + test + address + increment
-    "monopole_minimg": dict(all=16.0, bin=9.0, fp_all=15.0, fp_bin=4.0, mufu=1.0, atom=1.0),   # + 3 per axis for the minimum image
+    "monopole_minimg": dict(all=13.0, bin=9.0, fp_all=9.0, fp_bin=4.0, mufu=1.0, atom=1.0),    # + 2 per axis for the minimum image: L - |d|, min
     "rmu": dict(all=7.0, bin=21.0, fp_all=6.0, fp_bin=15.0, mufu=2.0, atom=1.0),       # + s.l (3), |l|^2 (2), FMUL, RSQ, FMUL, second axis (4), tau (2), IMAD
     "pisigma": dict(all=7.0, bin=24.0, fp_all=6.0, fp_bin=18.0, mufu=2.0, atom=1.0),
     "radial": dict(all=8.0, bin=0.0, fp_all=6.0, fp_bin=0.0, mufu=0.0, atom=0.0),

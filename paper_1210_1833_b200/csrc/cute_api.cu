@@ -591,7 +591,7 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
         if (b->lo1 == 0.0 && b->lo2 == 0.0) p.simple = 1;
     } else if (kind == CUTE_MONOPOLE || kind == CUTE_RMU) {
         // error of one separation component: input rounding, subtraction rounding, periodic image
-        // (minimum image by d - L rint(d/L): a d within rounding of L/2 may take the other image, |d'| off by <= 2uL)
+        // (brute-force minimum image |d'| = min(|d|, L - |d|): the roundings of d and of L - |d| are <= uL each; 3uL is kept)
         double e_d = (f64in ? 2.0 * kU * M : 0.0) + kU * (minimg ? 3.0 * b->box_L : b->hi1 * 1.01);
         if (p.periodic && !minimg) {
             // the periodic image is taken by subtracting L from the larger coordinate: exact (Sterbenz) when the wrapped

@@ -365,11 +365,16 @@ __device__ __forceinline__ void separations(const Consts &c, const IPoints &ip, 
 #pragma unroll
     for (int h = 0; h < 2; h++) {
         f32x2 dx = sub2(ip.X[h], bc(pj.x)), dy = sub2(ip.Y[h], bc(pj.y)), dz = sub2(ip.Z[h], bc(pj.z));
-        if (MINIMG) {                    // periodic brute force: minimum image d - L rint(d / L)
-            const f32x2 mg = bc(CUTE_MAGIC_F), il = bc(c.invL), nl = bc(-c.Lf);
-            dx = fma2(sub2(fma2(dx, il, mg), mg), nl, dx);
-            dy = fma2(sub2(fma2(dy, il, mg), mg), nl, dy);
-            dz = fma2(sub2(fma2(dz, il, mg), mg), nl, dz);
+        if (MINIMG) {
+            // periodic brute force: minimum image.  Only d^2 is needed and the coordinates lie in [0, L) (checked
+            // when the grid is made), so |d'| = min(|d|, L - |d|): one packed add on the float32 pipe and two FMNMX on the ALU
+            // pipe per axis, instead of three packed operations for d - L rint(d / L) -- this kernel is float32-pipe-bound.
+            const f32x2 Lp = bc(c.Lf);
+            float a0, a1, b0, b1;
+            // (the absolute values are written on the scalars: ptxas folds them into the |.| operand modifiers)
+            unpk(dx, a0, a1); unpk(sub2(Lp, pk(fabsf(a0), fabsf(a1))), b0, b1); dx = pk(fminf(fabsf(a0), b0), fminf(fabsf(a1), b1));
+            unpk(dy, a0, a1); unpk(sub2(Lp, pk(fabsf(a0), fabsf(a1))), b0, b1); dy = pk(fminf(fabsf(a0), b0), fminf(fabsf(a1), b1));
+            unpk(dz, a0, a1); unpk(sub2(Lp, pk(fabsf(a0), fabsf(a1))), b0, b1); dz = pk(fminf(fabsf(a0), b0), fminf(fabsf(a1), b1));
         }
         q2[h] = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
     }
