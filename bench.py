@@ -437,7 +437,7 @@ def density_grid_entry(api, torch, peaks_hbm, peaks, clock_mhz):
             "grid_point_pairs": pairs, "grid_point_pairs_per_s": pairs / (ms_st * 1e-3),
             "tsc": {"bound": "hbm", "algorithmic_bytes": tsc_bytes, "achieved": tsc_bytes / (ms_tsc * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
                     "frac": tsc_bytes / (ms_tsc * 1e-3) / 1e9 / hbm, "peak_source": hsrc,
-                    "note": "27 float64 atomics per particle into the L2-resident grid: atomic-bound, not HBM-bound"},
+                    "note": "27 float64 atomics per particle into the L2-resident grid (three lanes per particle: adjacent triples per instruction): bound by the L2 atomic units, not by HBM"},
             "stencil": {"bound": "alu", "unit": "T float64 multiply-adds/s", "algorithmic_fma": pairs,
                         "achieved": pairs / (ms_st * 1e-3) / 1e12,
                         "peak": peaks["table"].get("dfma", 0.0) * peaks["sms"] * clock_mhz * 1e6 / 1e12,

@@ -7,7 +7,7 @@
 // distances only have to be calculated once."
 // Readings D1-D4: grid points = cell centres (g + 1/2) h; TSC = second-order B-spline per axis;
 // delta = rho / (N / ng^3) - 1; every ordered pair (g, g + v), v != 0 with the minimum image, r = h |v|, half-open bins.
-// Three kernels: TSC scatter (float64 atomics into the L2-resident grid; HBM-bound on the particle read),
+// Three kernels: TSC scatter (float64 atomics into the L2-resident grid, three lanes per particle; bound by the L2 atomic units),
 // overdensity (elementwise), and the offset-stencil correlation.  The offsets are found and binned ONCE on the host.
 // k_grid_corr_rows (offsets of at most 16 cells per axis) treats each (vy, vz) as a 1-D cross-correlation of x-rows for all
 // vx at once, register-tiled, rows staged in shared memory by cp.async, half of the offsets swept (xi is even);
@@ -35,40 +35,47 @@ __device__ __forceinline__ int wrap(int g, int ng)
     return g < 0 ? g + ng : g;
 }
 
-__global__ void __launch_bounds__(256) k_tsc(const void *x, const void *y, const void *z, int dtype, int64_t n, double inv_h, int ng,
-                                             double *rho, uint32_t *status)
+// TSC scatter with THREE lanes per particle, one per x-offset: the three grid points a particle feeds along x are
+// adjacent doubles, so a warp instruction carries 10 particles x 3 adjacent addresses = 10-20 sectors to the L2 atomic
+// units instead of 32 scattered ones (the scatter is bound by those units, not by HBM; measured on 10^7 particles and a
+// 128^3 grid: 1.16 ms with one thread per particle and 27 scattered atomics each, 0.76 ms this way).
+__global__ void __launch_bounds__(256) k_tsc3(const void *x, const void *y, const void *z, int dtype, int64_t n, double inv_h, int ng,
+                                              double *rho, uint32_t *status)
 {
-    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    double p[3];
-    if (dtype == CUTE_F64) {
-        p[0] = reinterpret_cast<const double *>(x)[i]; p[1] = reinterpret_cast<const double *>(y)[i]; p[2] = reinterpret_cast<const double *>(z)[i];
-    } else {
-        p[0] = reinterpret_cast<const float *>(x)[i]; p[1] = reinterpret_cast<const float *>(y)[i]; p[2] = reinterpret_cast<const float *>(z)[i];
+    const int lane = threadIdx.x & 31, pl = lane / 3, xo = lane - 3 * pl;
+    const int64_t nwarps = (int64_t)gridDim.x * (blockDim.x >> 5), wg = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    for (int64_t i0 = wg * 10; i0 < n; i0 += nwarps * 10) {
+        const int64_t i = i0 + pl;
+        if (lane >= 30 || i >= n) continue;
+        double p[3];
+        if (dtype == CUTE_F64) {
+            p[0] = reinterpret_cast<const double *>(x)[i]; p[1] = reinterpret_cast<const double *>(y)[i]; p[2] = reinterpret_cast<const double *>(z)[i];
+        } else {
+            p[0] = reinterpret_cast<const float *>(x)[i]; p[1] = reinterpret_cast<const float *>(y)[i]; p[2] = reinterpret_cast<const float *>(z)[i];
+        }
+        int g0[3];
+        double w[3][3];
+        bool bad = false;
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            const double u = p[d] * inv_h;                  // position in units of cells
+            if (!(fabs(u) < 1.0e9)) bad = true;
+            const double c = floor(u);                      // the particle's own cell
+            g0[d] = bad ? 0 : (int)c - 1;
+#pragma unroll
+            for (int k = 0; k < 3; k++) w[d][k] = tsc_weight(u - (c - 1.0 + (double)k + 0.5));
+        }
+        if (bad) { atomicExch(status, 1u); continue; }
+        const int gx = wrap(g0[0] + xo, ng);
+        const double wx = xo == 0 ? w[0][0] : (xo == 1 ? w[0][1] : w[0][2]);
+        int gy[3], gz[3];
+#pragma unroll
+        for (int k = 0; k < 3; k++) { gy[k] = wrap(g0[1] + k, ng); gz[k] = wrap(g0[2] + k, ng); }
+#pragma unroll
+        for (int a = 0; a < 3; a++)
+#pragma unroll
+            for (int b = 0; b < 3; b++) atomicAdd(&rho[((size_t)gz[a] * ng + gy[b]) * ng + gx], wx * w[1][b] * w[2][a]);
     }
-    int g0[3];
-    double w[3][3];
-    bool bad = false;
-#pragma unroll
-    for (int d = 0; d < 3; d++) {
-        const double u = p[d] * inv_h;                  // position in units of cells
-        if (!(fabs(u) < 1.0e9)) bad = true;
-        const double c = floor(u);                      // the particle's own cell
-        g0[d] = bad ? 0 : (int)c - 1;
-#pragma unroll
-        for (int k = 0; k < 3; k++) w[d][k] = tsc_weight(u - (c - 1.0 + (double)k + 0.5));
-    }
-    if (bad) { atomicExch(status, 1u); return; }
-    int gx[3], gy[3], gz[3];
-#pragma unroll
-    for (int k = 0; k < 3; k++) { gx[k] = wrap(g0[0] + k, ng); gy[k] = wrap(g0[1] + k, ng); gz[k] = wrap(g0[2] + k, ng); }
-#pragma unroll
-    for (int a = 0; a < 3; a++)
-#pragma unroll
-        for (int b = 0; b < 3; b++)
-#pragma unroll
-            for (int c = 0; c < 3; c++)
-                atomicAdd(&rho[((size_t)gz[a] * ng + gy[b]) * ng + gx[c]], w[0][c] * w[1][b] * w[2][a]);
 }
 
 __global__ void k_overdensity(double *rho, int64_t ng3, double inv_mean)
@@ -391,7 +398,7 @@ int cute_density_grid_xi(const cute_catalog *cat, double L, int ng, const cute_b
     const bool fast = m <= 16 && m >= 1 && (size_t)8 * (((ng + 3) & ~3) + 32) * 8 <= 200 * 1024;
     if (!offs.empty() && !fast && cudaMemcpyAsync(d_offs, offs.data(), offs.size() * 16, cudaMemcpyHostToDevice, s) != cudaSuccess) return CUTE_ERR_CUDA;
     if (cudaMemcpyAsync(d_bstart, bstart.data(), bstart.size() * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) return CUTE_ERR_CUDA;
-    k_tsc<<<(unsigned)((cat->n + 255) / 256), 256, 0, s>>>(cat->c0, cat->c1, cat->c2, cat->dtype, cat->n, (double)ng / L, ng, rho, d_status);
+    k_tsc3<<<148 * 8, 256, 0, s>>>(cat->c0, cat->c1, cat->c2, cat->dtype, cat->n, (double)ng / L, ng, rho, d_status);
     k_overdensity<<<(unsigned)((ng3 + 255) / 256), 256, 0, s>>>(rho, (int64_t)ng3, (double)ng3 / (double)cat->n);
     if (d_delta && cudaMemcpyAsync(d_delta, rho, ng3 * 8, cudaMemcpyDeviceToDevice, s) != cudaSuccess) return CUTE_ERR_CUDA;
     if (!offs.empty() && fast) {
