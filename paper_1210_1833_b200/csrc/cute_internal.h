@@ -34,7 +34,7 @@ struct Chunk {            // one work item's i side: <=128 consecutive cell-sort
 struct GridView {         // device-side view of one built grid
     const float4 *hi;     // [n] cell-sorted (x,y,z,w)
     const float4 *lo;     // [n] low parts or nullptr
-    const double *p64;    // SoA [4][n_pad] float64 canonical coordinates or nullptr
+    const double *p64;    // [n_pad][4] float64 canonical coordinates (one 32-byte record per point) or nullptr
     const uint32_t *cell_start; // [ncells+1]
     const Chunk *chunks;
     const int *row_kx;    // SPHERE: per-row half-width in cells along RA (or nullptr)

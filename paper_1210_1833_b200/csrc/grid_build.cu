@@ -289,7 +289,10 @@ __device__ __forceinline__ void emit_point(const BuildPlan &b, uint32_t slot, do
     }
     b.hi[slot] = make_float4(h[0], h[1], h[2], h[3]);
     if (b.want_lo) b.lo[slot] = make_float4(l[0], l[1], l[2], l[3]);
-    if (b.want_f64) for (int d = 0; d < 4; d++) b.p64[(size_t)d * b.n_pad + slot] = v[d];
+    if (b.want_f64) {   // one 32-byte record per point (two 16-byte stores into one sector; four separate arrays cost four)
+        double2 *q = reinterpret_cast<double2 *>(b.p64) + 2 * (size_t)slot;
+        q[0] = make_double2(v[0], v[1]); q[1] = make_double2(v[2], v[3]);
+    }
     if (b.perm) b.perm[slot] = i;
 }
 

@@ -176,7 +176,7 @@ __device__ __forceinline__ double norm2_64(double x, double y, double z)
 __device__ __forceinline__ void load64(const GridView &g, uint32_t idx, double v[4], int nload)
 {
     if (g.p64) {
-        for (int d = 0; d < nload; d++) v[d] = g.p64[(size_t)d * g.n_pad + idx];
+        for (int d = 0; d < nload; d++) v[d] = g.p64[4 * (size_t)idx + d];
     } else {   // float32 catalogue: the float32 values ARE the input
         float4 h = g.hi[idx];
         v[0] = h.x; v[1] = h.y; v[2] = h.z; v[3] = h.w;
