@@ -24,6 +24,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import sys
 import threading
@@ -448,6 +449,65 @@ def density_grid_entry(api, torch, peaks_hbm, peaks, clock_mhz):
                                 "rate by 2x.  ms_stencil includes the host-side offset table (built once per call)"}}
 
 
+def paper_table2_entry(api, torch):
+    """CONTEXT ONLY: the five shapes of the paper's Table II -- "the time to
+    fill one DR histogram by brute force" -- on a synthetic stand-in for its MICE subset: 3e5 uniform objects in the
+    wedge 0 < RA, Dec < 18 deg, 0.5 < z < 0.6, against as many randoms (the paper never states the size of its random
+    catalogue: ASSUMED equal to the data).  Not the metric, not a target; the paper's times are other hardware."""
+    from paper_1210_1833_b200 import runner, synth
+    n = 300000
+    ra, dec, z, xyz = synth.uniform_wedge(n, 18.0, 18.0, 0.5, 0.6, synth.seed_for(9, 0))
+    rra, rdec, rz, rxyz = synth.uniform_wedge(n, 18.0, 18.0, 0.5, 0.6, synth.seed_for(9, 1))
+    base = dict(log1=0, n2=0, lo2=0.0, hi2=0.0, aperture=0.0, box_L=0.0)
+    th = math.radians(30.0)
+    shapes = [
+        ("xi(r), 256 linear bins, r < 100 Mpc/h", "monopole", tuple(xyz), tuple(rxyz), dict(base, n1=256, lo1=0.0, hi1=100.0), 13.0),
+        ("xi_log(r), 256 log bins, 50 per decade, r < 100 Mpc/h", "monopole", tuple(xyz), tuple(rxyz),
+         dict(base, n1=256, lo1=100.0 / 10.0 ** (256 / 50.0), hi1=100.0, log1=1), 20.0),
+        ("w(theta), 256 linear bins, theta < 30 deg", "angular", (ra, dec), (rra, rdec), dict(base, n1=256, lo1=0.0, hi1=th), 22.0),
+        ("xi(pi,sigma), 64 x 64 bins to 100 Mpc/h", "pisigma", tuple(xyz), tuple(rxyz),
+         dict(base, n1=64, lo1=0.0, hi1=100.0, n2=64, lo2=0.0, hi2=100.0), 27.0),
+    ]
+    rows = []
+
+    def time_dr(job, reps=3):
+        job.build()
+        job.count("DR")
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            job.enqueue("DR")
+        e1.record()
+        torch.cuda.synchronize()
+        st = api.cute_count_status(job.counter)
+        return e0.elapsed_time(e1) / reps, st
+
+    for name, kind, d, r, bins, paper_s in shapes:
+        job = runner.Job(kind, d, r, bins, dict(mode="none"))
+        ms, st = time_dr(job)
+        rows.append({"shape": name, "ms_per_DR_histogram": ms, "pairs": float(n) * n, "pairs_per_s": float(n) * n / (ms * 1e-3),
+                     "refined_pairs": float(st["refined"]), "paper_server_gpu_s": paper_s})
+        del job
+    # w_pix(theta): pixels of 5e-3 sq-deg (PAPER.md:275), both catalogues pixelised on the device, weighted pixel-pixel counts
+    side = math.sqrt(5e-3)
+    nra = int(round(18.0 / side))
+    u1 = math.sin(math.radians(18.0))
+    nu = int(round(u1 / (5e-3 / (18.0 / nra) * math.pi / 180.0)))
+    pix = []
+    for a, b in ((ra, dec), (rra, rdec)):
+        cols = [torch.from_numpy(np.ascontiguousarray(c)).cuda() for c in (a, b)]
+        pra, pdec, pw = api.cute_pixelize(cols, 0.0, 18.0, 0.0, u1, nra, nu)
+        pix.append(((pra.cpu().numpy(), pdec.cpu().numpy()), pw.cpu().numpy().view(np.uint32)))
+    (cd, wd), (cr, wr) = pix
+    job = runner.Job("angular", cd, cr, dict(base, n1=256, lo1=0.0, hi1=th), dict(mode="none"), None, w_data=wd, w_rand=wr)
+    ms, st = time_dr(job)
+    rows.append({"shape": f"w_pix(theta), pixels of 5e-3 sq-deg ({len(wd)} x {len(wr)} non-empty pixels), 256 linear bins",
+                 "ms_per_DR_histogram": ms, "pairs": float(len(wd)) * len(wr), "pairs_per_s": float(len(wd)) * len(wr) / (ms * 1e-3),
+                 "refined_pairs": float(st["refined"]), "paper_server_gpu_s": 0.46})
+    return {"config": "paper_table2", "workload": "CONTEXT: the shapes of the paper's Table II on a synthetic wedge (3e5 x 3e5, randoms ASSUMED as "
+            "many as data; brute force, one DR histogram each); paper_server_gpu_s = Tesla C2070 (PAPER.md:296-302)", "rows": rows}
+
+
 def measured_peaks(api, torch):
     """Roofline denominators measured on this device in this run (cute_measure_peaks: SURVEY.md 8(d) R2)."""
     pk = api.cute_measure_peaks()
@@ -536,6 +596,7 @@ def run_ours(args):
             torch.cuda.empty_cache()
         if args.scale == 1.0:
             per_config.append(density_grid_entry(api, torch, hbm_peak(), peaks, clock_mhz))
+            per_config.append(paper_table2_entry(api, torch))
 
     cfg = {"workload": describe(head_id, w, args.scale), "scale": args.scale,
            "l2": "256 MiB buffer written between timed iterations (L2 flush)",

@@ -248,6 +248,18 @@ def gaussian_nz_cap(n: int, area_sqdeg: float, zmean: float, zsig: float, zmin: 
 
 
 # ----------------------------------------------------------------------------- the five workloads
+def uniform_wedge(n: int, ra_max: float, dec_max: float, zmin: float, zmax: float, seed: int, om: float = 0.3):
+    """Uniform in the comoving volume of the wedge 0 < RA < ra_max, 0 < Dec < dec_max, zmin < z < zmax: the footprint of
+    the MICE subset the paper times in Table II (the mock itself is not available).  Returns ra, dec, z, xyz."""
+    rng = np.random.default_rng(seed)
+    ra = ra_max * rng.random(n)
+    dec = np.degrees(np.arcsin(math.sin(math.radians(dec_max)) * rng.random(n)))
+    c0, c1 = lcdm_chi(np.array([zmin, zmax]), om)
+    chi = np.cbrt(c0 ** 3 + (c1 ** 3 - c0 ** 3) * rng.random(n))
+    z = lcdm_z_of_chi(chi, om)
+    return ra, dec, z, radecz_to_xyz(ra, dec, z, om)
+
+
 @dataclass
 class Workload:
     """One BASELINE.json configuration: catalogues + the binning it is counted with.
