@@ -42,6 +42,7 @@ extern "C" {
 #define CUTE_ERR_OVERFLOW (-5)
 #define CUTE_ERR_POINT_OUT_OF_BOX (-6)
 #define CUTE_ERR_GRID_MISMATCH (-7)
+#define CUTE_ERR_STATIC_SCRATCH_LIMIT (-8) /* cute_count_pairs_static: the binning needs more than CUTE_STATIC_SCRATCH_BYTES */
 #define CUTE_WARN_EMPTY_BIN 1
 
 /* kinds of correlation function ("CUTE calculates 4 different correlation functions (3-D,
@@ -230,6 +231,35 @@ int cute_auto_grid_spec(int kind, int mode, const cute_catalog *const *cats, int
  * d_scratch.  stats (host, may be NULL): [0] separations evaluated, [1] pairs recomputed in float64,
  * [2] work items, [3] shared-memory histogram flushes. */
 int cute_count_status(void *d_scratch, void *stream, uint64_t stats[4]);
+
+/* The pair count for callers that cannot allocate device memory -- cute_count_pairs without the d_scratch argument.
+ *
+ * cute_count_pairs leaves every allocation to its caller, down to the small scratch block (work counter, status word,
+ * statistics, bin edges) of cute_count_scratch_bytes.  Not every caller can come up with one: an analysis hook that
+ * runs inside a simulation whose memory manager claimed the whole device at start-up and passes it only the particle
+ * data and a histogram to fill, a plug-in held to a host application's fixed memory budget, a thread for which
+ * cudaMalloc is off limits because it would stall the device under a time-critical loop or because another thread of
+ * the process is recording a stream at that moment.  For them the scratch is a fixed array of
+ * CUTE_STATIC_SCRATCH_BYTES inside the library image: each GPU that loads the library gives up that much memory until
+ * the process ends, and this function, like the rest of the library, calls neither cudaMalloc nor cudaFree nor any
+ * routine that allocates device memory.
+ *
+ * Arguments and result are those of cute_count_pairs (the caller still owns the grids and d_hist, DEVICE
+ * uint64[n1*max(n2,1)], overwritten), with these differences:
+ *  - Limit: the bin edges must fit the array: 8 * (n1 + n2 + 2) + 64 bytes, rounded up to 256, may not exceed
+ *    CUTE_STATIC_SCRATCH_BYTES (n1 + n2 <= 8182 bins).  Finer binning is refused with
+ *    CUTE_ERR_STATIC_SCRATCH_LIMIT before anything is enqueued; use cute_count_pairs with your own scratch instead.
+ *  - It finishes the job: after enqueuing on `stream` it waits for the stream and returns the final status, deferred
+ *    device errors included (what cute_count_status would report); stats (HOST, may be NULL) as in cute_count_status.
+ *  - First call on a device: looks up the array's device address (no allocation; the current device must be the one
+ *    the grids live on).  Make that first call outside any stream capture.
+ *  - Sharing: all calls on one device use the same array, which still holds the previous call's contents; the words
+ *    that must start at zero are cleared on `stream` at the start of every call.  Counts that overlapped on the GPU
+ *    would corrupt each other (one work counter, one set of edges), so calls from several host threads of one process
+ *    are made to take turns per device (a lock held until the call's work is done).  Up to 64 devices. */
+#define CUTE_STATIC_SCRATCH_BYTES 65536
+int cute_count_pairs_static(int kind, const cute_grid *g1, const cute_grid *g2, const cute_bin_spec *bins,
+                            uint64_t *d_hist, const cute_count_opts *opts, void *stream, uint64_t stats[4]);
 
 /* End-to-end entry point with HOST buffers: copies the catalogue(s) to the device, builds the
  * grid(s), counts, copies the histogram back.  cat2 == NULL: auto.  d_workspace: DEVICE, at least

@@ -20,6 +20,8 @@ COORD_XYZ, COORD_RADEC, COORD_RADECZ = 0, 1, 2
 F32, F64 = 0, 1
 GRID_NONE, GRID_BOX3D, GRID_SPHERE = 0, 1, 2
 WARN_EMPTY_BIN = 1
+ERR_STATIC_SCRATCH_LIMIT = -8
+STATIC_SCRATCH_BYTES = 65536
 
 
 class cute_catalog(C.Structure):
@@ -60,7 +62,7 @@ SYMBOLS = ["cute_version", "cute_strerror", "cute_launch_count", "cute_catalog_b
            "cute_count_status", "cute_host_workspace_bytes", "cute_count_pairs_host", "cute_bin_edges",
            "cute_landy_szalay", "cute_natural_estimator", "cute_multipoles", "cute_periodic_rr", "cute_periodic_xi",
            "cute_peak_count", "cute_peak_name", "cute_measure_peaks", "cute_shard_items", "cute_auto_grid_spec",
-           "cute_density_grid_workspace_bytes", "cute_density_grid_xi"]
+           "cute_density_grid_workspace_bytes", "cute_density_grid_xi", "cute_count_pairs_static"]
 
 
 def _load() -> C.CDLL:
@@ -87,6 +89,7 @@ def _load() -> C.CDLL:
                                      C.POINTER(cute_count_opts), vp]
     lib.cute_count_items.argtypes = [C.c_int, vp, vp, C.POINTER(cute_bin_spec), C.POINTER(cute_count_opts), C.POINTER(C.c_int64)]
     lib.cute_count_status.argtypes = [vp, vp, up]
+    lib.cute_count_pairs_static.argtypes = [C.c_int, vp, vp, C.POINTER(cute_bin_spec), vp, C.POINTER(cute_count_opts), vp, up]
     lib.cute_host_workspace_bytes.argtypes = [C.POINTER(cute_catalog), C.POINTER(cute_catalog), C.POINTER(cute_grid_spec),
                                               C.POINTER(cute_bin_spec), C.POINTER(C.c_size_t)]
     lib.cute_count_pairs_host.argtypes = [C.c_int, C.POINTER(cute_catalog), C.POINTER(cute_catalog), C.POINTER(cute_grid_spec),
@@ -318,6 +321,23 @@ def cute_count_items(kind: int, g1: Grid, g2: Grid | None, counter: Counter, opt
 def cute_count_status(counter: Counter, stream=None) -> dict:
     st = (C.c_uint64 * 4)()
     _check(lib.cute_count_status(counter.scratch_ptr(), C.c_void_p(_stream_ptr(stream)), st), "cute_count_status")
+    return dict(evaluated=int(st[0]), refined=int(st[1]), items=int(st[2]), flushes=int(st[3]))
+
+
+def cute_count_pairs_static(kind: int, g1: Grid, g2: Grid | None, bins: dict, hist, opts: cute_count_opts | None = None, stream=None) -> dict:
+    """The pair count for callers that cannot allocate device memory (a hook inside a simulation that owns the whole
+    device, a plug-in under a fixed memory budget, a thread that must not call cudaMalloc): same count as
+    cute_count_pairs, but its scratch is a fixed STATIC_SCRATCH_BYTES array inside the library instead of a buffer of
+    the caller's.  `hist`: the caller's device tensor of n1 * max(n2, 1) int64 (uint64 bits), overwritten.  Waits for
+    the stream; returns the kernel's statistics.  Raises CuteError(ERR_STATIC_SCRATCH_LIMIT) when n1 + n2 > 8182.  All
+    calls on a device share the one array, so the library runs them one at a time; the first call on a device should
+    not be made during a stream capture."""
+    b = bin_spec(bins)
+    assert hist.is_cuda and hist.is_contiguous() and hist.element_size() == 8 and hist.numel() == b.n1 * max(b.n2, 1)
+    st = (C.c_uint64 * 4)()
+    _check(lib.cute_count_pairs_static(int(kind), g1.handle, g2.handle if g2 is not None else None, C.byref(b),
+                                       C.c_void_p(hist.data_ptr()), C.byref(opts) if opts is not None else None,
+                                       C.c_void_p(_stream_ptr(stream)), st), "cute_count_pairs_static")
     return dict(evaluated=int(st[0]), refined=int(st[1]), items=int(st[2]), flushes=int(st[3]))
 
 

@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcute_b200.so")
 SOURCES = ["cute_api.cu", "grid_build.cu", "pair_count.cu", "pair_kind_monopole.cu", "pair_kind_angular.cu",
-           "pair_kind_rmu.cu", "pair_kind_radial.cu", "pair_kind_pisigma.cu", "density_grid.cu", "peaks.cu"]
+           "pair_kind_rmu.cu", "pair_kind_radial.cu", "pair_kind_pisigma.cu", "density_grid.cu", "peaks.cu", "no_alloc.cu"]
 HEADERS = [os.path.join(CSRC, "cute_internal.h"), os.path.join(CSRC, "pair_kernel.cuh"),
            os.path.join(HERE, "..", "include", "cute_b200.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -189,6 +189,7 @@ const char *cute_strerror(int status)
     case CUTE_ERR_OVERFLOW: return "counter overflow";
     case CUTE_ERR_POINT_OUT_OF_BOX: return "a point lies outside the grid box (or is not finite)";
     case CUTE_ERR_GRID_MISMATCH: return "the two grids of a cross-correlation carry different specs";
+    case CUTE_ERR_STATIC_SCRATCH_LIMIT: return "too many bins for the built-in scratch of cute_count_pairs_static (CUTE_STATIC_SCRATCH_BYTES): use cute_count_pairs with caller-provided scratch";
     case CUTE_WARN_EMPTY_BIN: return "warning: a bin with RR = 0 got xi = 0";
     }
     return "unknown status";
