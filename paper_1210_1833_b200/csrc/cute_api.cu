@@ -35,7 +35,7 @@ inline int sm_count()
 struct Layout {
     size_t hi, lo, p64, perm, count, cell_start, scan_tmp, row_nchunks, row_chunk_start, chunks,
         row_kx, row_ylo, row_yhi, status, bbox, part_tmp, part_table, total;
-    int part_G;
+    int part_G, part_Bmax;   // CTAs of the coarse pass; largest bucket count the partition table has room for
     uint32_t n_pad;
     int64_t max_cells, max_rows, max_chunks;
 };
@@ -53,15 +53,18 @@ inline int part_ctas() { return 2 * sm_count(); }
 //  * float32 xyz: the partition only when there are many cells (C5, 125 000 cells: 0.89 ms against 1.09 ms one-pass; with
 //    64 000 cells the one-pass sort wins, 0.70 against 0.86 ms -- its scattered stores thrash less).
 // The workspace is sized for either (the cell count is not known before the box is); build_path = 1 / 2 force one.
-inline bool may_partition(int64_t n, const cute_grid_spec *s)
-{
-    return n > 0 && (s->build_path == 2 || (s->build_path == 0 && n >= kPartMinN));
-}
+// may_partition: can ANY cell count up to max_cells take the partition path?  (Decides whether the workspace reserves the
+// partition's record buffer, 16-32 bytes per point: a float32 xyz catalogue whose cells cannot exceed 90 000 -- brute
+// force with its <= 32^3 ordering cells, or an explicit small ncell -- never does, and does not pay for it.)
 inline bool use_partition(int64_t n, const cute_catalog *c, const cute_grid_spec *s, int64_t ncells)
 {
-    if (!may_partition(n, s)) return false;
+    if (!(n > 0 && (s->build_path == 2 || (s->build_path == 0 && n >= kPartMinN)))) return false;
     const bool f32xyz = c->dtype == CUTE_F32 && c->coord == CUTE_COORD_XYZ;
     return s->build_path == 2 || !f32xyz || ncells > 90000;
+}
+inline bool may_partition(int64_t n, const cute_catalog *c, const cute_grid_spec *s, int64_t max_cells)
+{
+    return use_partition(n, c, s, max_cells);   // use_partition is monotone in the cell count
 }
 
 Layout make_layout(int64_t n, int want_lo, int want_f64, int64_t max_cells, int64_t max_rows, int rec_bytes)
@@ -84,8 +87,13 @@ Layout make_layout(int64_t n, int want_lo, int want_f64, int64_t max_cells, int6
     int64_t m = max_cells > max_rows ? max_cells : max_rows;
     L.part_G = part_ctas();
     if (rec_bytes > 0) {
+        // The build calls part_shape with the ACTUAL cell count, known only once the box is, and the bucket count is not
+        // monotone in the cell count (it lands anywhere in (512, 1024] below the cells-per-bucket cap): size the table
+        // for the largest count any ncells <= max_cells can give, max(B(max_cells), kPartMaxBuckets).
         int B, cpb;
         part_shape(max_cells, &B, &cpb);
+        if (B < kPartMaxBuckets) B = kPartMaxBuckets;
+        L.part_Bmax = B;
         const int64_t tab = (int64_t)B * L.part_G;
         L.part_tmp = take((size_t)L.n_pad * (size_t)rec_bytes);
         L.part_table = take((size_t)(2 * tab + 128) * 4);
@@ -272,7 +280,7 @@ int cute_grid_workspace_bytes(const cute_catalog *cat, const cute_grid_spec *spe
     wants(cat, spec, &want_lo, &want_f64);
     cell_bounds(cat, spec, &mc, &mr);
     if (mc > 0x7ffffff0ll) return CUTE_ERR_INVALID_ARG;
-    *bytes = make_layout(cat->n, want_lo, want_f64, mc, mr, !may_partition(cat->n, spec) ? 0 : (cat->dtype == CUTE_F32 && cat->coord == CUTE_COORD_XYZ) ? 16 : 32).total;
+    *bytes = make_layout(cat->n, want_lo, want_f64, mc, mr, !may_partition(cat->n, cat, spec, mc) ? 0 : (cat->dtype == CUTE_F32 && cat->coord == CUTE_COORD_XYZ) ? 16 : 32).total;
     return CUTE_OK;
 }
 
@@ -289,7 +297,7 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     int64_t mc, mr;
     wants(cat, spec, &want_lo, &want_f64);
     cell_bounds(cat, spec, &mc, &mr);
-    const Layout L = make_layout(cat->n, want_lo, want_f64, mc, mr, !may_partition(cat->n, spec) ? 0 : (cat->dtype == CUTE_F32 && cat->coord == CUTE_COORD_XYZ) ? 16 : 32);
+    const Layout L = make_layout(cat->n, want_lo, want_f64, mc, mr, !may_partition(cat->n, cat, spec, mc) ? 0 : (cat->dtype == CUTE_F32 && cat->coord == CUTE_COORD_XYZ) ? 16 : 32);
     if (bytes < L.total) return CUTE_ERR_WORKSPACE_TOO_SMALL;
     unsigned char *w = (unsigned char *)d_workspace;
 
@@ -438,6 +446,7 @@ int cute_make_grid(const cute_catalog *cat, const cute_grid_spec *spec, void *d_
     if (use_partition(cat->n, cat, spec, b.ncells) && b.mode != CUTE_GRID_NONE) {   // large catalogue: two-level partition (grid_build.cu)
         b.part_tmp = w + L.part_tmp; b.part_table = (uint32_t *)(w + L.part_table); b.part_G = L.part_G;
         part_shape(b.ncells, &b.part_B, &b.part_cpb);
+        if (b.part_B > L.part_Bmax) { delete g; return CUTE_ERR_WORKSPACE_TOO_SMALL; }   // (cannot happen: make_layout)
         b.part_shift = 0;
         while ((1 << b.part_shift) < b.part_cpb) b.part_shift++;
     }

@@ -21,6 +21,17 @@
 
 namespace cute {
 
+// SMs of the current device (grid sizing only)
+static int dg_sm_count()
+{
+    static int n = 0;
+    if (!n) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+    }
+    return n;
+}
+
 __device__ __forceinline__ double tsc_weight(double s)
 {
     s = fabs(s);
@@ -292,7 +303,7 @@ template <int M>
 static cudaError_t launch_rows(const double *delta, int ng, int m, const int2 *vyz, int npairs, int npairs_all, const int *binidx, double *sum_dd,
                                cudaStream_t s)
 {
-    int zsplit = (8 * 148 + npairs_all - 1) / npairs_all;   // (the launches of the classes run back to back: size the slabs for all of them)
+    int zsplit = (8 * dg_sm_count() + npairs_all - 1) / npairs_all;   // (the launches of the classes run back to back: size the slabs for all of them)
     zsplit = zsplit < 1 ? 1 : (zsplit > ng ? ng : zsplit);
     // fast path: ng a multiple of 8, at most 256, and every slab a whole number of trips of 8 warps x (32 / LPR) rows
     int lpr_log2 = -1;
@@ -398,7 +409,7 @@ int cute_density_grid_xi(const cute_catalog *cat, double L, int ng, const cute_b
     const bool fast = m <= 16 && m >= 1 && (size_t)8 * (((ng + 3) & ~3) + 32) * 8 <= 200 * 1024;
     if (!offs.empty() && !fast && cudaMemcpyAsync(d_offs, offs.data(), offs.size() * 16, cudaMemcpyHostToDevice, s) != cudaSuccess) return CUTE_ERR_CUDA;
     if (cudaMemcpyAsync(d_bstart, bstart.data(), bstart.size() * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) return CUTE_ERR_CUDA;
-    k_tsc3<<<148 * 8, 256, 0, s>>>(cat->c0, cat->c1, cat->c2, cat->dtype, cat->n, (double)ng / L, ng, rho, d_status);
+    k_tsc3<<<dg_sm_count() * 8, 256, 0, s>>>(cat->c0, cat->c1, cat->c2, cat->dtype, cat->n, (double)ng / L, ng, rho, d_status);
     k_overdensity<<<(unsigned)((ng3 + 255) / 256), 256, 0, s>>>(rho, (int64_t)ng3, (double)ng3 / (double)cat->n);
     if (d_delta && cudaMemcpyAsync(d_delta, rho, ng3 * 8, cudaMemcpyDeviceToDevice, s) != cudaSuccess) return CUTE_ERR_CUDA;
     if (!offs.empty() && fast) {

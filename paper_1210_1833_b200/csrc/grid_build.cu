@@ -99,10 +99,12 @@ __device__ __noinline__ unsigned long long cell_fix_box(const BuildPlan &b, doub
         const double t = (v[d] - b.origin[d]) * b.inv_cell[d];
         int kk = floor_magic(t);
         // NaN / inf / far-away coordinates fail the magnitude test (their floor_magic is meaningless);
-        // a point exactly on the upper face of a non-periodic box joins the last cell
+        // a point exactly on the upper face of a non-periodic box joins the last cell; so does a point of a periodic
+        // box that lies below the upper face (in [0, L)) but whose product with 1/cell rounds up to nc
         const bool in = fabs(t) < 2147483648.0 && kk >= 0;
         if (!in || kk >= b.nc[d]) {
-            if (!in || b.periodic || !(v[d] - b.origin[d] <= b.size[d])) ok = false;
+            const double off = v[d] - b.origin[d];
+            if (!in || !(b.periodic ? off < b.size[d] : off <= b.size[d])) ok = false;
             kk = in ? b.nc[d] - 1 : 0;
         }
         k[d] = kk;

@@ -644,3 +644,60 @@ def test_density_grid_monopole(rt, oracle, dtype):
     # validation: r_max beyond L/2, a non-xyz catalogue
     with pytest.raises(api.CuteError):
         api.cute_density_grid_xi(cols, L, ng, dict(n1=4, lo1=0.0, hi1=120.0))
+
+
+def test_periodic_point_one_ulp_below_the_upper_face(rt):
+    """a float64 coordinate just below L whose product with 1/cell rounds up to nc is a legal point of the periodic
+    box [0, L): it joins the last cell; x = L itself is refused"""
+    import torch
+    api, runner, synth = rt
+    L = 1000.0
+    x_top = np.nextafter(L, 0.0)
+    nc = next(n for n in range(3, 400) if x_top * (n / L) >= n)      # the rounding the fast path trips over
+    rng = np.random.default_rng(5)
+    pts = rng.uniform(0.0, L, size=(3, 500))
+    pts[0, 0] = pts[1, 1] = pts[2, 2] = x_top
+    cols = [torch.from_numpy(np.ascontiguousarray(c)).cuda() for c in pts]
+    spec = api.grid_spec("box3d", periodic=True, size=(L, L, L), ncell=(nc, nc, nc), rmax=0.9 * L / nc)
+    g = api.cute_make_grid(cols, api.COORD_XYZ, spec)
+    inf = g.info()
+    ws = g.workspace
+    off = inf.d_cell_start - ws.data_ptr()
+    cs = ws[off:off + (inf.ncells + 1) * 4].view(torch.int32).cpu().numpy().astype(np.int64)
+    k = np.minimum(np.floor(pts / (L / nc)).astype(np.int64), nc - 1)
+    cid = (k[2] * nc + k[1]) * nc + k[0]
+    assert np.array_equal(cs, np.concatenate([[0], np.cumsum(np.bincount(cid, minlength=nc ** 3))]))
+    pts[0, 0] = L
+    cols = [torch.from_numpy(np.ascontiguousarray(c)).cuda() for c in pts]
+    with pytest.raises(api.CuteError) as err:
+        api.cute_make_grid(cols, api.COORD_XYZ, spec)
+    assert err.value.status == -6
+
+
+@pytest.mark.parametrize("bad", [float("nan"), float("inf"), -float("inf"), 1.0e30, -1.0, 2000.0])
+@pytest.mark.parametrize("mode,build_path", [("box3d", 1), ("box3d", 2), ("none", 1)])
+def test_bad_coordinates_are_refused(rt, bad, mode, build_path):
+    """NaN / Inf / out-of-box coordinates give CUTE_ERR_POINT_OUT_OF_BOX and write nothing outside the
+    workspace (the bytes after it keep their pattern); the box of PAPER.md:206 here is given explicitly, [0, 1000)^3"""
+    import torch
+    api, runner, synth = rt
+    if mode == "none" and np.isfinite(bad):
+        pytest.skip("brute force has no box: every finite point is legal")
+    rng = np.random.default_rng(11)
+    pts = rng.uniform(0.0, 1000.0, size=(3, 3000))
+    pts[1, 1234] = bad
+    cols = [torch.from_numpy(np.ascontiguousarray(c)).cuda() for c in pts]
+    spec = api.grid_spec(mode, size=(1000.0,) * 3 if mode == "box3d" else (0, 0, 0), ncell=(8, 8, 8) if mode == "box3d" else (0, 0, 0),
+                         rmax=100.0 if mode == "box3d" else 0.0, build_path=build_path)
+    cat, keep = api._catalog(cols, api.COORD_XYZ, True)
+    nbytes = api.cute_grid_workspace_bytes(cat, spec)
+    guard = 4096
+    ws = torch.full((nbytes + 256 + guard,), 0x5A, dtype=torch.uint8, device="cuda")
+    off = (-ws.data_ptr()) % 256
+    # hand the library exactly nbytes: whatever lies behind must survive
+    sub = ws[off:off + nbytes]
+    with pytest.raises(api.CuteError) as err:
+        api.cute_make_grid(cols, api.COORD_XYZ, spec, workspace=sub)
+    assert err.value.status == -6
+    torch.cuda.synchronize()
+    assert bool((ws[off + nbytes:] == 0x5A).all()) and bool((ws[:off] == 0x5A).all())

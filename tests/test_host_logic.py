@@ -179,3 +179,27 @@ def test_two_rank_gloo_histogram_allreduce(tmp_path):
     outs = [p.communicate(timeout=240)[0].decode() for p in procs]
     for p, o in zip(procs, outs):
         assert p.returncode == 0, o
+
+
+def test_grid_workspace_reserves_the_partition_only_where_it_can_run(api):
+    """the partition build's record buffer (16-32 bytes per point) and its bucket table are part of the workspace only when
+    some cell count the build may choose can take that path; and the table always has room for the largest bucket
+    count (kPartMaxBuckets = 1024 buckets x 2 SM-count CTAs x 2 tables)"""
+    n = 1 << 21
+    z = np.zeros(8, dtype=np.float32)
+
+    def nbytes(dtype, mode, build_path, ncell=(0, 0, 0)):
+        cat = api.cute_catalog(C.sizeof(api.cute_catalog), n, api.COORD_XYZ, dtype, z.ctypes.data, z.ctypes.data, z.ctypes.data, None)
+        spec = api.grid_spec(mode, size=(1000.0,) * 3 if mode == "box3d" else (0, 0, 0), ncell=ncell,
+                             rmax=50.0 if mode == "box3d" else 0.0, kind_mask=2, build_path=build_path)
+        return api.cute_grid_workspace_bytes(cat, spec)
+
+    # brute force, float32 xyz: at most 32^3 ordering cells, never partitioned unless forced
+    assert nbytes(api.F32, "none", 2) - nbytes(api.F32, "none", 0) >= 16 * n
+    assert nbytes(api.F32, "none", 0) == nbytes(api.F32, "none", 1)
+    # float64 brute force may take it (32-byte records)
+    assert nbytes(api.F64, "none", 0) - nbytes(api.F64, "none", 1) >= 32 * n
+    # cell list, float32: explicit small ncell never partitions, automatic cells may
+    assert nbytes(api.F32, "box3d", 0, (20, 20, 20)) == nbytes(api.F32, "box3d", 1, (20, 20, 20))
+    assert nbytes(api.F32, "box3d", 0, (50, 50, 50)) - nbytes(api.F32, "box3d", 1, (50, 50, 50)) >= 16 * n + 2 * 1024 * 4
+    assert nbytes(api.F32, "box3d", 0) - nbytes(api.F32, "box3d", 1) >= 16 * n + 2 * 1024 * 4
