@@ -13,9 +13,11 @@ per-count times, the three rates of SURVEY.md 8(d) (evaluated / binned / brute-e
 second), the pair kernel's roofline, the cell build against the HBM roofline, the end-to-end
 number through cute_count_pairs_host and the oracle timed on the host cores beside it.
 
-N > 1 (torchrun): the work-item list of every pair count is split over the ranks (catalogues and
-grids replicated), and the partial uint64 histograms are summed with one NCCL all-reduce -- the
-only exchange step the method has.  Total work is fixed: "scaling": "strong".
+N > 1 (torchrun): the work-item list of every pair count is split over the ranks (catalogues
+replicated; every rank builds the grids and then takes rank 0's cell-sorted arrays by one NCCL
+broadcast, because the order inside a cell differs from build to build and the shards must
+enumerate the same points), and the partial uint64 histograms are summed with one NCCL
+all-reduce.  Total work is fixed: "scaling": "strong".
 
 --impl reference times the float64 oracle (oracle/) on the host cores, as it stands, on a bounded
 sample of the same workload.
@@ -260,7 +262,9 @@ class Runner:
         torch, api, job = self.torch, self.api, self.job
         b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         b0.record()
-        job.build()                                           # G0-G4 for both catalogues
+        # G0-G4 for both catalogues; N > 1: every rank then takes rank 0's cell-sorted arrays (the order inside a cell
+        # differs from build to build, and the item shards must enumerate the same points on every rank)
+        job.build(share=(lambda t: self.dist.broadcast(t, src=0)) if self.dist is not None else None)
         b1.record()
         evs = []
         for which in self.whichs:
@@ -356,13 +360,27 @@ class Runner:
             if cat is None:
                 continue
             need = 2 if job.coord == api.COORD_RADEC else 3
-            host[name] = [(torch.from_numpy(np.ascontiguousarray(c)).pin_memory()).numpy() for c in list(cat)[:need]]
+            dt = np.float64 if np.asarray(cat[0]).dtype not in (np.float32, np.float64) else np.asarray(cat[0]).dtype
+            host[name] = [(torch.from_numpy(np.ascontiguousarray(c, dtype=dt)).pin_memory()).numpy() for c in list(cat)[:need]]
         ws = None
         h2d = d2h = 0
 
         def one():
             nonlocal ws, h2d, d2h
             h2d = d2h = 0
+            if self.world > 1:
+                # N > 1: the item shards need identical grids on every rank (Job.build(share)), which the one-call host entry
+                # point cannot give: the same public calls one by one -- pinned host -> device copies, cute_make_grid,
+                # broadcast, cute_count_pairs on this rank's items, all-reduce, histograms back to the host (Runner.step)
+                for name, dev in (("data", job.d_data), ("rand", job.d_rand)):
+                    if dev is None:
+                        continue
+                    for d, hcol in zip(dev, host[name]):
+                        d.copy_(torch.from_numpy(hcol), non_blocking=True)
+                        h2d += hcol.nbytes
+                self.step(None)
+                d2h += 8 * job.counter.nhist * len(self.whichs)
+                return
             for which in self.whichs:
                 c1 = host["data"] if which in ("DD", "DR") else host["rand"]
                 c2 = host["rand"] if which == "DR" else None
@@ -591,6 +609,9 @@ def run_ours(args):
     from paper_1210_1833_b200 import api
 
     peaks = measured_peaks(api, torch)
+    if args.n4_only:                                   # the density-grid entry alone (profiling: profiles/r03_n4.md)
+        print(json.dumps(density_grid_entry(api, torch, hbm_peak(), peaks, SM_MAX_MHZ_FALLBACK)))
+        return
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     head_id = args.config
     w = workload_for(head_id, args.scale, args)
@@ -657,7 +678,7 @@ def run_ours(args):
 
     cfg = {"workload": describe(head_id, w, args.scale), "scale": args.scale,
            "l2": "256 MiB buffer written between timed iterations (L2 flush)",
-           "parallelism": f"work items sharded over {world} GPU(s), catalogues replicated, one all-reduce of the histogram"}
+           "parallelism": f"work items sharded over {world} GPU(s), catalogues replicated, grids broadcast from rank 0, one all-reduce of the histogram"}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
            "dtype": "f32", "data": "synthetic", "config": cfg, "clocks": clocks, "gpu_launches": int(launches), "e2e": e2e,
@@ -686,6 +707,7 @@ def main():
     ap.add_argument("--scale", type=float, default=1.0, help="shrink the catalogues (debugging only; 1.0 = the named configs)")
     ap.add_argument("--only", action="store_true", help="measure the headline config only (no per_config sweep)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--n4-only", action="store_true", help="run only the density-grid monopole entry (SURVEY 8(f) N4) and print it")
     ap.add_argument("--grid", default="default", choices=["default", "none", "sphere", "box3d"],
                     help="override the headline workload's neighbour search (default: the one BASELINE.json names)")
     ap.add_argument("--pix", type=float, default=0.1, help="--grid sphere: pixel side in units of theta_max")

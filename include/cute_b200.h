@@ -215,7 +215,11 @@ int cute_count_items(int kind, const cute_grid *g1, const cute_grid *g2, const c
  * `rank` handles (pass them as cute_count_opts.item_begin / item_end with shard = 1).  Items are chunk-major (item =
  * chunk * nsplit + split, nchunks from cute_grid_info).  Cross-correlations and cell-list counts have ~uniform work per
  * item; a brute-force AUTO-correlation (auto_brute != 0) is a triangle -- chunk c meets only j > i -- so its cuts are
- * placed at equal areas, 1 - (1 - x)^2.  The shards partition [0, nitems): integer partial histograms add up exactly. */
+ * placed at equal areas, 1 - (1 - x)^2.  The shards partition [0, nitems): integer partial histograms add up exactly --
+ * PROVIDED every shard is counted on the SAME built grid or a byte copy of its workspace.  The order of the points inside
+ * a cell is decided by atomic cursors and differs from one cute_make_grid call to the next, so item k of two separate
+ * builds of one catalogue does not hold the same 128 points: ranks that each built their own grid must first overwrite
+ * their workspace with one rank's (a broadcast; layout and host handle are identical, they do not depend on that order). */
 int cute_shard_items(int64_t nitems, int64_t nchunks, int rank, int world, int auto_brute, int64_t *begin, int64_t *end);
 
 /* Grid sizing from the data ("a box encompassing the whole catalog is first determined", PAPER.md:208-215

@@ -753,11 +753,6 @@ int plan_fast_path(PairParams &p, int kind, const cute_grid *g1, const cute_grid
         if (tau1 > 0.2) p.always_refine = 1;  // bins too fine for float32 unit vectors: everything in float64
     }
     A.tau = (float)tau1;
-    A.Oa = (float)((double)A.O - tau1);
-    A.Ob = (float)((double)A.O + tau1);
-    // Oa/Ob are rounded to float32: make sure the window did not shrink
-    A.Oa = nextafterf(A.Oa, -INFINITY);
-    A.Ob = nextafterf(A.Ob, INFINITY);
     return CUTE_OK;
 }
 

@@ -71,7 +71,6 @@ namespace cute {
 struct FastAxis {
     float S, O, c1, c2, c3, c4;
     float tau, tau_w;      // tau_eff = tau + tau_w * w   (w: kind-specific, see pair_count.cu)
-    float Oa, Ob;          // O - tau, O + tau
     int n;
 };
 

@@ -47,8 +47,14 @@ class Job:
         self.g_data = self.g_rand = None
         self.spec = None
 
-    def build(self):
-        """G0-G4 for every catalogue (cute_make_grid)."""
+    def build(self, share=None):
+        """G0-G4 for every catalogue (cute_make_grid).
+
+        share: N > 1 only -- a callable that overwrites a device uint8 tensor on every rank with rank 0's copy (a broadcast).
+        The order of the points INSIDE a cell is decided by atomic cursors and differs from build to build, so the work
+        items (128 consecutive sorted points) of two ranks that each built their own grid do not hold the same points and
+        their item shards would not partition the pairs.  Every rank therefore builds (same layout, same host-side handle:
+        cell counts, chunk counts and bounds do not depend on that order) and then takes rank 0's workspace bytes."""
         cats = [self.d_data] + ([self.d_rand] if self.d_rand is not None else [])
         if self.spec is None:
             self.spec = api.auto_spec(self.kind_name, self.bins, self.grid, cats, self.coord)
@@ -69,6 +75,11 @@ class Job:
                 self.g_rand.free()
             self.g_rand = api.cute_make_grid(self.d_rand, self.coord, self.spec, workspace=getattr(self, "_ws_r", None), weight=self.w_rand)
             self._ws_r = self.g_rand.workspace
+        if share is not None:
+            for g in (self.g_data, self.g_rand):
+                if g is not None:
+                    off = (-g.workspace.data_ptr()) % 256
+                    share(g.workspace[off:])
         return self
 
     def grids(self, which: str):

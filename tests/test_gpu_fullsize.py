@@ -117,8 +117,8 @@ def _perm_of(job, torch):
     return ws[off:off + inf.n * 4].view(torch.int32).cpu().numpy().astype(np.int64)
 
 
-@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
-def test_auto_path_at_full_size(rt, oracle, cfg):
+@pytest.mark.parametrize("cfg,cat", [(2, "data"), (3, "data"), (4, "data"), (5, "data"), (2, "rand"), (3, "rand")])
+def test_auto_path_at_full_size(rt, oracle, cfg, cat):
     """The auto-correlation path (j > i mask, own-row segments) at BASELINE.json's full sizes, tied to the oracle two ways:
     (i) the exact identity cross(A, A)[k] = 2 auto(A)[k] + N [k = 0 and lo = 0] -- the cross side is oracle-checked on
     blocks by the tests above; (ii) the auto count of ~2e4 CONSECUTIVE cell-sorted points (a dense block of the real
@@ -126,6 +126,8 @@ def test_auto_path_at_full_size(rt, oracle, cfg):
     import torch
     api, runner, synth = rt
     w = synth.workload(cfg)
+    if cat == "rand":                                       # RR of C2 (400 k) and C3 (10^6): the random catalogue through the same path
+        w.data = w.rand
     n = len(w.data[0])
     grid = dict(w.grid)                                     # (keeps the permutation: no_perm is not set)
     job = runner.Job(w.kind, w.data, w.data, w.bins, grid).build()   # the same catalogue twice: two grids
@@ -158,3 +160,21 @@ def test_auto_path_at_full_size(rt, oracle, cfg):
         ok, msg = oracle.parity_ok(h, orc)
         assert ok, f"sorted block at {s0}: {msg}"
         assert h.sum() > (1000 if cfg != 4 else 0)
+
+
+def test_c5_full_in_the_benchmarked_spec(rt, oracle):
+    """bench.py builds its grids with no_perm = 1 (the sort permutation is not written): the full-size C5 counts in exactly
+    that spec equal the ones of the permutation-writing build, and a block against the whole random catalogue, built
+    with no_perm = 1 as well, satisfies the parity rule"""
+    api, runner, synth = rt
+    w = synth.workload(5)
+    ref = runner.job_for_workload(w).build()
+    want = {k: ref.count(k)[0] for k in ("DD", "DR")}
+    del ref
+    w.grid = dict(w.grid, no_perm=1)
+    job = runner.job_for_workload(w).build()
+    assert job.spec.no_perm == 1 and not job.g_data.info().d_perm
+    for k in ("DD", "DR"):
+        assert np.array_equal(job.count(k)[0], want[k])
+    nd = len(w.data[0])
+    _cross_block_check(rt, oracle, w, "DR", w.data, w.rand, _blocks(nd, 500, (4321,)), "celled")

@@ -701,3 +701,69 @@ def test_bad_coordinates_are_refused(rt, bad, mode, build_path):
     assert err.value.status == -6
     torch.cuda.synchronize()
     assert bool((ws[off + nbytes:] == 0x5A).all()) and bool((ws[:off] == 0x5A).all())
+
+
+_SHARD_WORKER = r"""
+import os, sys
+import numpy as np, torch, torch.distributed as dist
+sys.path.insert(0, sys.argv[1])
+from paper_1210_1833_b200 import api, runner, synth
+dist.init_process_group("gloo", rank=int(os.environ["RANK"]), world_size=int(os.environ["WORLD_SIZE"]))
+r, world = dist.get_rank(), dist.get_world_size()
+out = {}
+cats = np.load(sys.argv[3])
+for cfg, scale in ((5, 0.003), (2, 0.02)):
+    w = synth.workload(cfg, scale)
+    # the parent's catalogues, bit for bit (the generators use BLAS, whose rounding may depend on the threads a process gets)
+    w.data = tuple(cats[f"C{cfg}_d{k}"] for k in range(len(w.data)))
+    w.rand = tuple(cats[f"C{cfg}_r{k}"] for k in range(len(w.rand)))
+    def share(t):                                     # rank 0's cell-sorted arrays to every rank (gloo: through the host)
+        c = t.cpu()
+        dist.broadcast(c, src=0)
+        t.copy_(c)
+    job = runner.job_for_workload(w).build(share=share)   # catalogues replicated, grids identical on every rank
+    for which in w.pairs:
+        g1, g2 = job.grids(which)
+        n = api.cute_count_items(job.kind, g1, g2, job.counter)
+        b, e = api.cute_shard_items(n, g1.info().nchunks, r, world, w.grid.get("mode", "none") == "none" and g2 is None)
+        job.opts = api.count_opts(item_begin=b, item_end=e, shard=1)
+        h, st = job.count(which)                      # the real pair kernel on this rank's share of the items
+        t = torch.from_numpy(h.astype(np.int64))
+        dist.all_reduce(t)                            # the one exchange step: sum of the partial histograms
+        out[f"C{cfg}_{which}"] = t.numpy()
+        out[f"C{cfg}_{which}_items"] = np.array([b, e, n])
+if r == 0:
+    np.savez(sys.argv[2], **out)
+dist.destroy_process_group()
+"""
+
+
+def test_two_processes_count_their_shards_with_the_real_kernel(rt, tmp_path):
+    """two processes on the one GPU, each counting its cute_shard_items share with the real pair kernel (no
+    kernel waits on another process), partial uint64 histograms summed with a gloo all-reduce (the sum
+    of private histograms) == the single-process histogram, for a cell-list cross/auto count and a brute-force triangle"""
+    import os
+    import subprocess
+    import sys
+    api, runner, synth = rt
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "shard_worker.py"
+    script.write_text(_SHARD_WORKER)
+    res, cats = tmp_path / "res.npz", tmp_path / "cats.npz"
+    ws = {cfg: synth.workload(cfg, scale) for cfg, scale in ((5, 0.003), (2, 0.02))}
+    np.savez(cats, **{f"C{cfg}_{t}{k}": c for cfg, w in ws.items() for t, cat in (("d", w.data), ("r", w.rand)) for k, c in enumerate(cat)})
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29573", WORLD_SIZE="2")
+    procs = [subprocess.Popen([sys.executable, str(script), root, str(res), str(cats)], env=dict(env, RANK=str(r)), stdout=subprocess.PIPE,
+                              stderr=subprocess.STDOUT) for r in range(2)]
+    outs = [p.communicate(timeout=600)[0].decode() for p in procs]
+    for p, o in zip(procs, outs):
+        assert p.returncode == 0, o
+    got = np.load(res)
+    for cfg, w in ws.items():
+        job = runner.job_for_workload(w).build()
+        for which in w.pairs:
+            h, st = job.count(which)
+            assert np.array_equal(got[f"C{cfg}_{which}"].astype(np.uint64), h), (cfg, which)
+            b, e, n = got[f"C{cfg}_{which}_items"]
+            assert 0 < e <= n and b == 0                  # rank 0's share is a proper, non-empty prefix
+            assert e < n
