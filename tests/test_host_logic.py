@@ -203,3 +203,22 @@ def test_grid_workspace_reserves_the_partition_only_where_it_can_run(api):
     assert nbytes(api.F32, "box3d", 0, (20, 20, 20)) == nbytes(api.F32, "box3d", 1, (20, 20, 20))
     assert nbytes(api.F32, "box3d", 0, (50, 50, 50)) - nbytes(api.F32, "box3d", 1, (50, 50, 50)) >= 16 * n + 2 * 1024 * 4
     assert nbytes(api.F32, "box3d", 0) - nbytes(api.F32, "box3d", 1) >= 16 * n + 2 * 1024 * 4
+
+
+def test_static_scratch_entry_point_refuses_fine_binning_without_a_gpu(api):
+    """cute_count_pairs_static checks its size limit before it touches CUDA: more bins than the built-in 64 KiB scratch
+    holds (n1 + n2 > 8182) is CUTE_ERR_STATIC_SCRATCH_LIMIT whatever the other arguments are; the same spec with
+    caller-provided scratch is a plain size query"""
+    for n1, n2, want in ((8183, 0, api.ERR_STATIC_SCRATCH_LIMIT), (4000, 4183, api.ERR_STATIC_SCRATCH_LIMIT), (70000, 0, -1)):
+        b = api.bin_spec(dict(n1=n1, lo1=0.0, hi1=100.0, n2=n2, lo2=0.0, hi2=1.0))
+        rc = api.lib.cute_count_pairs_static(api.MONOPOLE if n2 == 0 else api.RMU, None, None, C.byref(b), None, None, None, None)
+        if want == -1:
+            assert rc < 0        # (n1 beyond what any count accepts: refused one way or the other)
+        else:
+            assert rc == want
+    b = api.bin_spec(dict(n1=8183, lo1=0.0, hi1=100.0))
+    nb = C.c_size_t(0)
+    assert api.lib.cute_count_scratch_bytes(C.byref(b), None, C.byref(nb)) == 0 and nb.value > api.STATIC_SCRATCH_BYTES
+    b = api.bin_spec(dict(n1=8182, lo1=0.0, hi1=100.0))
+    assert api.lib.cute_count_scratch_bytes(C.byref(b), None, C.byref(nb)) == 0 and nb.value == api.STATIC_SCRATCH_BYTES
+    assert "cute_count_pairs" in api.cute_strerror(api.ERR_STATIC_SCRATCH_LIMIT)
